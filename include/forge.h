@@ -1,0 +1,143 @@
+/*
+ * forge.h -- C ABI of forge-b200: FORGE's hot path (arxiv/paper_2606_22932) on NVIDIA B200 (sm_100a).
+ *
+ * The operation (sec. 2.2, Eq. 4, Algorithm 1): for one linear layer with weight
+ * W[out,in], activations X[T,in] and upstream gradient dY[T,out], every weight tile forms its
+ * block of G = dY^T X in fp32 on chip (tensor memory) and immediately applies AdamW to the
+ * matching tiles of W, m and v in place.  G is never written to device memory.
+ *
+ *   m'  = beta1*m + (1-beta1)*G                      Alg. 1 line 7
+ *   v'  = beta2*v + (1-beta2)*G*G                    Alg. 1 line 8
+ *   W'  = (1-lr*wd)*W - lr*(m'/(1-beta1^t)) / (sqrt(v'/(1-beta2^t)) + eps)     lines 9-10
+ *   store W' (bf16, round to nearest even), m', v' (storage type)              line 11
+ *
+ * All pointers are DEVICE pointers unless a parameter says "host".  The caller allocates and owns
+ * every buffer; the library allocates no O(out*in) memory and keeps no reference after a call
+ * returns ("No gradient byte reaches global memory"; Eq. 5).  Work is
+ * enqueued on `stream` and the call returns without synchronising.
+ *
+ * Caller's obligations (documented, not enforced):
+ *   - dX = dY*W must already be enqueued on the same stream: W is overwritten (
+ *     PAPER.md:74 Alg. 1 line 1; PAPER.md:296 Remark 2).
+ *   - a weight with more than one backward consumer (tied embedding / LM head) must not be passed
+ *     (PAPER.md:296).
+ *   - W, m, v, scales do not overlap each other or X, dY; problems of one group have disjoint state.
+ *
+ * Error behaviour: every argument of every problem is validated before anything is enqueued, so a
+ * non-OK return means no state was touched.  No exceptions cross this boundary.  NaN/Inf in the
+ * inputs propagate by IEEE rules.  There is no CPU or library fallback: a device that is not
+ * compute capability 10.x returns FORGE_ERR_UNSUPPORTED_ARCH.
+ */
+#ifndef FORGE_H_
+#define FORGE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FORGE_VERSION 100          /* 0.1.0 */
+#define FORGE_QBLOCK 256           /* int8 moment block: 256 contiguous elements along `in` */
+
+typedef enum {
+    FORGE_OK = 0,
+    FORGE_ERR_NULL_PTR = 1,
+    FORGE_ERR_BAD_SHAPE = 2,
+    FORGE_ERR_ALIGNMENT = 3,
+    FORGE_ERR_BAD_HYPERPARAM = 4,
+    FORGE_ERR_BAD_DTYPE = 5,
+    FORGE_ERR_UNSUPPORTED_ARCH = 6,
+    FORGE_ERR_CUDA = 7
+} forge_status_t;
+
+/* Storage type of the moments m, v ("k" of PAPER.md:19 Eq. 1):
+ *   FP32: 4+4 B/param ("fp32 optimizer state")
+ *   BF16: 2+2 B/param, round to nearest even (the "bf16-state" recipe)
+ *   INT8: 1+1 B/param + one fp32 absmax per 256-element block along `in` for each moment
+ *         (App. B with BASELINE.json's 256-blocks); m code = rint(m'*127/a) in
+ *         [-127,127] (int8), v code = max(1, rint(v'*255/a)) in [1,255] (uint8) when a > 0,
+ *         all codes 0 when a == 0; the stored scale is a = max|x| over the block (fp32).
+ *         Dequantised value = code*a/127 (m) or code*a/255 (v).  Requantised every step.
+ * In every mode the update arithmetic and G are fp32 and W' is computed from the unrounded
+ * m', v' ("the update arithmetic and the gradient remain fp32 throughout"). */
+typedef enum {
+    FORGE_MOMENT_FP32 = 0,
+    FORGE_MOMENT_BF16 = 1,
+    FORGE_MOMENT_INT8 = 2
+} forge_moment_dtype_t;
+
+/* CUDA stream handle; identical to cudaStream_t / CUstream.  NULL is the legacy default stream. */
+typedef struct CUstream_st *forge_stream_t;
+
+/* One linear layer's problem.  Layouts are row-major and dense (leading dimension = row length):
+ *   X  [T, in]   bf16, read only          dY [T, out]  bf16, read only
+ *   W  [out, in] bf16, updated in place   m, v [out, in] in the moment dtype, updated in place
+ *   m_scale, v_scale [out, in/256] fp32, INT8 mode only (must be NULL otherwise), in place.
+ * Constraints: T >= 1; out, in >= 8 and multiples of 8 (16 for BF16/INT8 moments along `in`;
+ * INT8 needs in % 256 == 0); every base pointer 16-byte aligned (X, dY: 16; state: 16). */
+typedef struct {
+    const void *X;
+    const void *dY;
+    void *W;
+    void *m;
+    void *v;
+    float *m_scale;
+    float *v_scale;
+    int32_t T, out, in;
+} forge_problem_t;
+
+/* Fused weight gradient + AdamW step for one layer (Algorithm 1).
+ * `step` is the 1-based index t of the update being applied (bias terms 1-beta^t); step < 1,
+ * lr < 0 or non-finite, beta outside [0,1), eps < 0, wd < 0 -> FORGE_ERR_BAD_HYPERPARAM. */
+forge_status_t forge_wgrad_adamw(const void *X, const void *dY, void *W, void *m, void *v,
+                                 float *m_scale, float *v_scale,
+                                 int32_t T, int32_t out, int32_t in,
+                                 int64_t step, float lr, float beta1, float beta2, float eps, float wd,
+                                 forge_moment_dtype_t moment_dtype, forge_stream_t stream);
+
+/* The same for `count` layers in as few launches as possible (one for count <= 8): all seven
+ * projections of a Llama-style decoder layer go in one persistent launch (the paper pays one
+ * launch per linear).  `problems` is a HOST array, read before the call returns. */
+forge_status_t forge_wgrad_adamw_grouped(const forge_problem_t *problems, int32_t count,
+                                         int64_t step, float lr, float beta1, float beta2,
+                                         float eps, float wd,
+                                         forge_moment_dtype_t moment_dtype, forge_stream_t stream);
+
+/* End-to-end convenience entry with HOST buffers (used for the e2e measurement): copies X, dY and
+ * the state to device scratch it allocates and frees itself, runs forge_wgrad_adamw, copies the
+ * state back and synchronises.  Same validation and return codes; all pointers are host pointers. */
+forge_status_t forge_wgrad_adamw_host(const void *X, const void *dY, void *W, void *m, void *v,
+                                      float *m_scale, float *v_scale,
+                                      int32_t T, int32_t out, int32_t in,
+                                      int64_t step, float lr, float beta1, float beta2, float eps, float wd,
+                                      forge_moment_dtype_t moment_dtype);
+
+/* TEST-ONLY twin (the paper's "store-G control", App. D): the identical mainloop
+ * but the fp32 tile is written to G[out,in] instead of consumed.  Never on the product path. */
+forge_status_t forge_wgrad_store_g(const void *X, const void *dY, float *G,
+                                   int32_t T, int32_t out, int32_t in, forge_stream_t stream);
+
+/* TEST/BENCH-ONLY unfused optimizer pass (the paper's standalone "FORGE optimizer kernel",
+ * PAPER.md:354; 86): applies the same per-element update function as the fused epilogue to a
+ * materialised fp32 G[out,in].  forge_wgrad_store_g + this must be bit-identical to
+ * forge_wgrad_adamw ("the operands are bit-identical and so are the results"). */
+forge_status_t forge_adamw_from_g(const float *G, void *W, void *m, void *v,
+                                  float *m_scale, float *v_scale, int32_t out, int32_t in,
+                                  int64_t step, float lr, float beta1, float beta2, float eps, float wd,
+                                  forge_moment_dtype_t moment_dtype, forge_stream_t stream);
+
+/* Device bytes the library itself holds between calls: a constant with no O(out*in) term (0). */
+size_t forge_workspace_bytes(void);
+/* Kernel launches issued by this library since load (for bench.py's gpu_launches). */
+uint64_t forge_launch_count(void);
+/* Detail of the last CUDA error seen by this library (cudaError_t value), 0 if none. */
+int forge_last_cuda_error(void);
+const char *forge_status_string(forge_status_t status);
+int forge_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FORGE_H_ */

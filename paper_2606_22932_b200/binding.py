@@ -1,0 +1,179 @@
+"""Thin ctypes binding of include/forge.h -- argument marshalling only; every step of the path
+runs in the CUDA kernels of libforge_b200.so.  There is no fallback: if the library is missing
+or a call fails, this module raises.
+
+Tensors are torch CUDA tensors (PyTorch only allocates device memory and provides streams):
+X [T,in] bf16, dY [T,out] bf16, W [out,in] bf16, m/v [out,in] in float32 | bfloat16 | int8+uint8,
+scales [out,in/256] float32 for int8.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import c_float, c_int32, c_int64, c_void_p
+
+import torch
+
+from . import build as _build
+
+FP32, BF16, INT8 = 0, 1, 2
+QBLOCK = 256
+STATUS_NAMES = ["FORGE_OK", "FORGE_ERR_NULL_PTR", "FORGE_ERR_BAD_SHAPE", "FORGE_ERR_ALIGNMENT",
+                "FORGE_ERR_BAD_HYPERPARAM", "FORGE_ERR_BAD_DTYPE", "FORGE_ERR_UNSUPPORTED_ARCH",
+                "FORGE_ERR_CUDA"]
+EXPORTS = ["forge_wgrad_adamw", "forge_wgrad_adamw_grouped", "forge_wgrad_adamw_host",
+           "forge_wgrad_store_g", "forge_adamw_from_g", "forge_workspace_bytes", "forge_launch_count",
+           "forge_last_cuda_error", "forge_status_string", "forge_version"]
+
+
+class ForgeError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        name = STATUS_NAMES[status] if 0 <= status < len(STATUS_NAMES) else str(status)
+        super().__init__(f"{where}: {name} (cuda error {lib().forge_last_cuda_error()})")
+
+
+class forge_problem_t(ctypes.Structure):
+    _fields_ = [("X", c_void_p), ("dY", c_void_p), ("W", c_void_p), ("m", c_void_p), ("v", c_void_p),
+                ("m_scale", c_void_p), ("v_scale", c_void_p),
+                ("T", c_int32), ("out", c_int32), ("in_", c_int32)]
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libforge_b200.so (built in-tree by build.build()); raises if it cannot be loaded."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB_PATH
+        if not os.path.exists(path):
+            raise FileNotFoundError(f"{path} not built: run `python -m paper_2606_22932_b200.build` "
+                                    "(there is no fallback path)")
+        L = ctypes.CDLL(path)
+        hp = [c_int64, c_float, c_float, c_float, c_float, c_float]
+        L.forge_wgrad_adamw.restype = ctypes.c_int
+        L.forge_wgrad_adamw.argtypes = [c_void_p] * 7 + [c_int32] * 3 + hp + [ctypes.c_int, c_void_p]
+        L.forge_wgrad_adamw_grouped.restype = ctypes.c_int
+        L.forge_wgrad_adamw_grouped.argtypes = [ctypes.POINTER(forge_problem_t), c_int32] + hp + [ctypes.c_int, c_void_p]
+        L.forge_wgrad_adamw_host.restype = ctypes.c_int
+        L.forge_wgrad_adamw_host.argtypes = [c_void_p] * 7 + [c_int32] * 3 + hp + [ctypes.c_int]
+        L.forge_wgrad_store_g.restype = ctypes.c_int
+        L.forge_wgrad_store_g.argtypes = [c_void_p] * 3 + [c_int32] * 3 + [c_void_p]
+        L.forge_adamw_from_g.restype = ctypes.c_int
+        L.forge_adamw_from_g.argtypes = [c_void_p] * 6 + [c_int32] * 2 + hp + [ctypes.c_int, c_void_p]
+        L.forge_workspace_bytes.restype = ctypes.c_size_t
+        L.forge_launch_count.restype = ctypes.c_uint64
+        L.forge_last_cuda_error.restype = ctypes.c_int
+        L.forge_status_string.restype = ctypes.c_char_p
+        L.forge_status_string.argtypes = [ctypes.c_int]
+        L.forge_version.restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+def _ptr(t):
+    return None if t is None else c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return c_void_p(s.cuda_stream)
+
+
+def moment_dtype_of(m: torch.Tensor) -> int:
+    return {torch.float32: FP32, torch.bfloat16: BF16, torch.int8: INT8}[m.dtype]
+
+
+def _check(status: int, where: str):
+    if status != 0:
+        raise ForgeError(status, where)
+
+
+def forge_wgrad_adamw(X, dY, W, m, v, step, lr, beta1, beta2, eps, wd, m_scale=None, v_scale=None,
+                      moment_dtype=None, stream=None, check=True) -> int:
+    """include/forge.h forge_wgrad_adamw (Algorithm 1). In place on W, m, v."""
+    T, inn = X.shape
+    out = dY.shape[1]
+    mdt = moment_dtype_of(m) if moment_dtype is None else moment_dtype
+    st = lib().forge_wgrad_adamw(_ptr(X), _ptr(dY), _ptr(W), _ptr(m), _ptr(v), _ptr(m_scale), _ptr(v_scale),
+                                 T, out, inn, int(step), lr, beta1, beta2, eps, wd, mdt, _stream(stream))
+    if check:
+        _check(st, "forge_wgrad_adamw")
+    return st
+
+
+def make_problem_array(problems):
+    """problems: iterable of dicts/objects with X, dY, W, m, v (and m_scale, v_scale for int8)."""
+    arr = (forge_problem_t * len(problems))()
+    for i, p in enumerate(problems):
+        g = p.get if isinstance(p, dict) else (lambda k, d=None, p=p: getattr(p, k, d))
+        X, dY = g("X"), g("dY")
+        arr[i].X, arr[i].dY = X.data_ptr(), dY.data_ptr()
+        arr[i].W, arr[i].m, arr[i].v = g("W").data_ptr(), g("m").data_ptr(), g("v").data_ptr()
+        ms, vs = g("m_scale"), g("v_scale")
+        arr[i].m_scale = None if ms is None else ms.data_ptr()
+        arr[i].v_scale = None if vs is None else vs.data_ptr()
+        arr[i].T, arr[i].in_ = X.shape
+        arr[i].out = dY.shape[1]
+    return arr
+
+
+def forge_wgrad_adamw_grouped(problems, step, lr, beta1, beta2, eps, wd, moment_dtype, stream=None,
+                              check=True, _arr=None) -> int:
+    """include/forge.h forge_wgrad_adamw_grouped: all projections of a layer in one launch."""
+    arr = make_problem_array(problems) if _arr is None else _arr
+    st = lib().forge_wgrad_adamw_grouped(arr, len(arr), int(step), lr, beta1, beta2, eps, wd, moment_dtype,
+                                         _stream(stream))
+    if check:
+        _check(st, "forge_wgrad_adamw_grouped")
+    return st
+
+
+def forge_wgrad_adamw_host(X, dY, W, m, v, step, lr, beta1, beta2, eps, wd, m_scale=None, v_scale=None,
+                           check=True) -> int:
+    """Host-buffer entry (CPU tensors, ideally pinned): H2D, fused step, D2H inside the call."""
+    T, inn = X.shape
+    out = dY.shape[1]
+    st = lib().forge_wgrad_adamw_host(_ptr(X), _ptr(dY), _ptr(W), _ptr(m), _ptr(v), _ptr(m_scale), _ptr(v_scale),
+                                      T, out, inn, int(step), lr, beta1, beta2, eps, wd, moment_dtype_of(m))
+    if check:
+        _check(st, "forge_wgrad_adamw_host")
+    return st
+
+
+def forge_wgrad_store_g(X, dY, G, stream=None, check=True) -> int:
+    """TEST-ONLY store-G twin: G[out,in] fp32 = dY^T X."""
+    T, inn = X.shape
+    out = dY.shape[1]
+    st = lib().forge_wgrad_store_g(_ptr(X), _ptr(dY), _ptr(G), T, out, inn, _stream(stream))
+    if check:
+        _check(st, "forge_wgrad_store_g")
+    return st
+
+
+def forge_adamw_from_g(G, W, m, v, step, lr, beta1, beta2, eps, wd, m_scale=None, v_scale=None, stream=None,
+                       check=True) -> int:
+    """TEST/BENCH-ONLY unfused optimizer pass over a materialised fp32 G."""
+    out, inn = W.shape
+    st = lib().forge_adamw_from_g(_ptr(G), _ptr(W), _ptr(m), _ptr(v), _ptr(m_scale), _ptr(v_scale), out, inn,
+                                  int(step), lr, beta1, beta2, eps, wd, moment_dtype_of(m), _stream(stream))
+    if check:
+        _check(st, "forge_adamw_from_g")
+    return st
+
+
+def forge_launch_count() -> int:
+    return int(lib().forge_launch_count())
+
+
+def forge_workspace_bytes() -> int:
+    return int(lib().forge_workspace_bytes())
+
+
+def forge_version() -> int:
+    return int(lib().forge_version())
+
+
+def forge_status_string(status: int) -> str:
+    return lib().forge_status_string(status).decode()

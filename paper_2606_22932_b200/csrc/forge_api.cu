@@ -1,0 +1,401 @@
+// forge_api.cu -- the C ABI of include/forge.h: argument validation, host-side scalars, tensor-map
+// construction and kernel launches.  Allocates no device memory (except the scratch of the
+// explicitly host-buffer entry point forge_wgrad_adamw_host, freed before it returns).
+#include <atomic>
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <mutex>
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "../../include/forge.h"
+#include "elementwise_kernel.cuh"
+#include "fused_kernel.cuh"
+
+namespace {
+
+using namespace forge;
+
+std::atomic<uint64_t> g_launches{0};
+std::atomic<int> g_last_cuda_error{0};
+
+forge_status_t cuda_fail(cudaError_t e) {
+    g_last_cuda_error.store(static_cast<int>(e));
+    return FORGE_ERR_CUDA;
+}
+
+// ---------------------------------------------------------------------------------------------
+// driver entry point for tensor-map encoding (no link-time dependency on libcuda)
+// ---------------------------------------------------------------------------------------------
+using EncodeTiledFn = CUresult (*)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                   CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                   CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static std::once_flag once;
+    std::call_once(once, [] {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    });
+    return fn;
+}
+
+// 2D row-major tensor [rows, cols] of `esize`-byte elements; box {box_cols, box_rows}.
+bool encode_2d(CUtensorMap *map, CUtensorMapDataType dt, int esize, const void *base, uint64_t rows,
+               uint64_t cols, uint32_t box_cols, uint32_t box_rows, CUtensorMapSwizzle swz) {
+    EncodeTiledFn fn = get_encode_fn();
+    if (!fn) return false;
+    cuuint64_t dims[2] = {cols, rows};
+    cuuint64_t strides[1] = {cols * static_cast<uint64_t>(esize)};
+    cuuint32_t box[2] = {box_cols, box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(map, dt, 2, const_cast<void *>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    swz, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+CUtensorMapSwizzle swizzle_for_row_bytes(int row_bytes) {
+    return row_bytes == 128 ? CU_TENSOR_MAP_SWIZZLE_128B
+                            : (row_bytes == 64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_32B);
+}
+
+// ---------------------------------------------------------------------------------------------
+// validation and scalars
+// ---------------------------------------------------------------------------------------------
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+forge_status_t validate_hp(int64_t step, float lr, float b1, float b2, float eps, float wd) {
+    if (step < 1) return FORGE_ERR_BAD_HYPERPARAM;
+    if (!std::isfinite(lr) || lr < 0.f) return FORGE_ERR_BAD_HYPERPARAM;
+    if (!(b1 >= 0.f && b1 < 1.f) || !(b2 >= 0.f && b2 < 1.f)) return FORGE_ERR_BAD_HYPERPARAM;
+    if (!std::isfinite(eps) || eps < 0.f) return FORGE_ERR_BAD_HYPERPARAM;
+    if (!std::isfinite(wd) || wd < 0.f) return FORGE_ERR_BAD_HYPERPARAM;
+    return FORGE_OK;
+}
+
+forge_status_t validate_state(const void *W, const void *m, const void *v, const float *ms, const float *vs,
+                              int32_t out, int32_t in, int mdt) {
+    if (mdt < 0 || mdt > 2) return FORGE_ERR_BAD_DTYPE;
+    if (!W || !m || !v) return FORGE_ERR_NULL_PTR;
+    if (mdt == FORGE_MOMENT_INT8) {
+        if (!ms || !vs) return FORGE_ERR_NULL_PTR;
+    } else if (ms || vs) {
+        return FORGE_ERR_BAD_DTYPE;   // scales are meaningful for INT8 only
+    }
+    if (out < 8 || in < 8 || (out % 8) != 0 || (in % 8) != 0) return FORGE_ERR_BAD_SHAPE;
+    if (mdt == FORGE_MOMENT_BF16 && (in % 8) != 0) return FORGE_ERR_BAD_SHAPE;
+    if (mdt == FORGE_MOMENT_INT8 && (in % FORGE_QBLOCK) != 0) return FORGE_ERR_BAD_SHAPE;
+    if (!aligned16(W) || !aligned16(m) || !aligned16(v)) return FORGE_ERR_ALIGNMENT;
+    if (mdt == FORGE_MOMENT_INT8 && ((reinterpret_cast<uintptr_t>(ms) & 3u) || (reinterpret_cast<uintptr_t>(vs) & 3u)))
+        return FORGE_ERR_ALIGNMENT;
+    return FORGE_OK;
+}
+
+forge_status_t validate_problem(const forge_problem_t &p, int mdt) {
+    if (!p.X || !p.dY) return FORGE_ERR_NULL_PTR;
+    forge_status_t s = validate_state(p.W, p.m, p.v, p.m_scale, p.v_scale, p.out, p.in, mdt);
+    if (s != FORGE_OK) return s;
+    if (p.T < 1) return FORGE_ERR_BAD_SHAPE;
+    if (!aligned16(p.X) || !aligned16(p.dY)) return FORGE_ERR_ALIGNMENT;
+    return FORGE_OK;
+}
+
+// Alg. 1 line 9 bias terms and the folded constants, computed in double from the float
+// hyper-parameters the ABI carries, rounded to float once.
+AdamWScalars make_scalars(int64_t step, float lr, float b1, float b2, float eps, float wd) {
+    AdamWScalars h;
+    const double bc1 = 1.0 - std::pow(static_cast<double>(b1), static_cast<double>(step));
+    const double bc2 = 1.0 - std::pow(static_cast<double>(b2), static_cast<double>(step));
+    h.beta1 = b1;
+    h.one_minus_beta1 = 1.0f - b1;
+    h.beta2 = b2;
+    h.one_minus_beta2 = 1.0f - b2;
+    h.step_size = static_cast<float>(static_cast<double>(lr) / bc1);
+    h.inv_sqrt_bc2 = static_cast<float>(1.0 / std::sqrt(bc2));
+    h.eps = eps;
+    h.decay = static_cast<float>(1.0 - static_cast<double>(lr) * static_cast<double>(wd));
+    return h;
+}
+
+struct DeviceInfo {
+    int device = -1, sm_count = 0, cc_major = 0;
+};
+forge_status_t device_info(DeviceInfo &d) {
+    cudaError_t e = cudaGetDevice(&d.device);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = cudaDeviceGetAttribute(&d.cc_major, cudaDevAttrComputeCapabilityMajor, d.device);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, d.device);
+    if (e != cudaSuccess) return cuda_fail(e);
+    if (d.cc_major != 10) return FORGE_ERR_UNSUPPORTED_ARCH;
+    return FORGE_OK;
+}
+
+int env_int(const char *name, int dflt) {
+    const char *s = std::getenv(name);
+    return s ? std::atoi(s) : dflt;
+}
+
+// ---------------------------------------------------------------------------------------------
+// launch of one fused-kernel instantiation over <= kMaxProblems problems
+// ---------------------------------------------------------------------------------------------
+template <int MDT, int MODE, int BK, int ST, int SS>
+forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamWScalars &hp,
+                            const DeviceInfo &dev, cudaStream_t stream) {
+    using Cfg = KernelCfg<MDT, BK, ST, SS>;
+    auto kernel = forge_fused_kernel<MDT, MODE, BK, ST, SS>;
+    static std::once_flag once;
+    static cudaError_t attr_err = cudaSuccess;
+    std::call_once(once, [&] {
+        attr_err = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
+    });
+    if (attr_err != cudaSuccess) return cuda_fail(attr_err);
+
+    KernelParams P;
+    std::memset(&P, 0, sizeof(P));
+    P.hp = hp;
+    P.num_problems = count;
+    int tiles = 0;
+    constexpr CUtensorMapDataType mom_dt = (MDT == MDT_FP32) ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
+                                           : (MDT == MDT_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16
+                                                              : CU_TENSOR_MAP_DATA_TYPE_UINT8);
+    for (int i = 0; i < count; ++i) {
+        const forge_problem_t &p = probs[i];
+        ProblemDesc &d = P.prob[i];
+        bool ok = true;
+        ok &= encode_2d(&d.map_dY, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.dY, p.T, p.out, 64, BK, CU_TENSOR_MAP_SWIZZLE_128B);
+        ok &= encode_2d(&d.map_X, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.X, p.T, p.in, 64, BK, CU_TENSOR_MAP_SWIZZLE_128B);
+        if (MODE == MODE_ADAMW) {
+            ok &= encode_2d(&d.map_W, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.W, p.out, p.in, CHUNK_N, BLOCK_M,
+                            swizzle_for_row_bytes(Cfg::W_ROW));
+            ok &= encode_2d(&d.map_m, mom_dt, Cfg::kMomBytes, p.m, p.out, p.in, CHUNK_N, BLOCK_M,
+                            swizzle_for_row_bytes(Cfg::M_ROW));
+            ok &= encode_2d(&d.map_v, mom_dt, Cfg::kMomBytes, p.v, p.out, p.in, CHUNK_N, BLOCK_M,
+                            swizzle_for_row_bytes(Cfg::M_ROW));
+        } else {  // store-G twin: p.m carries the fp32 G output
+            ok &= encode_2d(&d.map_m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, p.m, p.out, p.in, CHUNK_N, BLOCK_M,
+                            CU_TENSOR_MAP_SWIZZLE_128B);
+        }
+        if (!ok) return cuda_fail(cudaErrorInvalidValue);
+        d.m_scale = p.m_scale;
+        d.v_scale = p.v_scale;
+        d.T = p.T;
+        d.out = p.out;
+        d.in = p.in;
+        d.tiles_n = (p.in + BLOCK_N - 1) / BLOCK_N;
+        d.tile_begin = tiles;
+        tiles += ((p.out + BLOCK_M - 1) / BLOCK_M) * d.tiles_n;
+    }
+    P.total_tiles = tiles;
+    int grid = dev.sm_count;
+    const int forced = env_int("FORGE_GRID", 0);   // debug/determinism tests only
+    if (forced > 0) grid = forced;
+    if (grid > tiles) grid = tiles;
+    kernel<<<grid, kThreads, Cfg::SMEM_BYTES, stream>>>(P);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e);
+    g_launches.fetch_add(1);
+    return FORGE_OK;
+}
+
+// Static per-shape configuration table (the paper searches this space with an autotuner,
+// PAPER.md:706-710 App. H; here the choice is fixed per moment dtype and token count):
+//   small T : HBM-bound -> short token chunks, deep state ring
+//   large T : tensor-bound -> 64-token chunks, deeper operand ring, shallow state ring
+forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, const AdamWScalars &hp,
+                              const DeviceInfo &dev, cudaStream_t stream) {
+    int maxT = 0;
+    for (int i = 0; i < count; ++i) maxT = probs[i].T > maxT ? probs[i].T : maxT;
+    int variant = maxT > 1024 ? 1 : 0;
+    const int forced = env_int("FORGE_CFG", -1);   // debug only
+    if (forced >= 0) variant = forced;
+    switch (mdt) {
+    case FORGE_MOMENT_FP32:
+        if (variant == 1) return launch_fused<MDT_FP32, MODE_ADAMW, 64, 3, 2>(probs, count, hp, dev, stream);
+        if (variant == 2) return launch_fused<MDT_FP32, MODE_ADAMW, 32, 2, 4>(probs, count, hp, dev, stream);
+        return launch_fused<MDT_FP32, MODE_ADAMW, 32, 3, 3>(probs, count, hp, dev, stream);
+    case FORGE_MOMENT_BF16:
+        if (variant == 1) return launch_fused<MDT_BF16, MODE_ADAMW, 64, 3, 3>(probs, count, hp, dev, stream);
+        return launch_fused<MDT_BF16, MODE_ADAMW, 32, 3, 6>(probs, count, hp, dev, stream);
+    case FORGE_MOMENT_INT8:
+        if (variant == 1) return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 9>(probs, count, hp, dev, stream);
+        return launch_fused<MDT_INT8, MODE_ADAMW, 32, 2, 10>(probs, count, hp, dev, stream);
+    default:
+        return FORGE_ERR_BAD_DTYPE;
+    }
+}
+
+}  // namespace
+
+// =============================================================================================
+// C ABI
+// =============================================================================================
+extern "C" {
+
+forge_status_t forge_wgrad_adamw_grouped(const forge_problem_t *problems, int32_t count, int64_t step, float lr,
+                                         float beta1, float beta2, float eps, float wd,
+                                         forge_moment_dtype_t moment_dtype, forge_stream_t stream) {
+    if (!problems) return FORGE_ERR_NULL_PTR;
+    if (count < 1) return FORGE_ERR_BAD_SHAPE;
+    const int mdt = static_cast<int>(moment_dtype);
+    if (mdt < 0 || mdt > 2) return FORGE_ERR_BAD_DTYPE;
+    forge_status_t s = validate_hp(step, lr, beta1, beta2, eps, wd);
+    if (s != FORGE_OK) return s;
+    for (int i = 0; i < count; ++i) {
+        s = validate_problem(problems[i], mdt);
+        if (s != FORGE_OK) return s;
+    }
+    DeviceInfo dev;
+    s = device_info(dev);
+    if (s != FORGE_OK) return s;
+    const AdamWScalars hp = make_scalars(step, lr, beta1, beta2, eps, wd);
+    for (int i = 0; i < count; i += kMaxProblems) {
+        const int n = (count - i) < kMaxProblems ? (count - i) : kMaxProblems;
+        s = dispatch_fused(problems + i, n, mdt, hp, dev, reinterpret_cast<cudaStream_t>(stream));
+        if (s != FORGE_OK) return s;
+    }
+    return FORGE_OK;
+}
+
+forge_status_t forge_wgrad_adamw(const void *X, const void *dY, void *W, void *m, void *v, float *m_scale,
+                                 float *v_scale, int32_t T, int32_t out, int32_t in, int64_t step, float lr,
+                                 float beta1, float beta2, float eps, float wd,
+                                 forge_moment_dtype_t moment_dtype, forge_stream_t stream) {
+    forge_problem_t p;
+    p.X = X; p.dY = dY; p.W = W; p.m = m; p.v = v; p.m_scale = m_scale; p.v_scale = v_scale;
+    p.T = T; p.out = out; p.in = in;
+    return forge_wgrad_adamw_grouped(&p, 1, step, lr, beta1, beta2, eps, wd, moment_dtype, stream);
+}
+
+forge_status_t forge_wgrad_store_g(const void *X, const void *dY, float *G, int32_t T, int32_t out, int32_t in,
+                                   forge_stream_t stream) {
+    if (!X || !dY || !G) return FORGE_ERR_NULL_PTR;
+    if (T < 1 || out < 8 || in < 8 || (out % 8) || (in % 8)) return FORGE_ERR_BAD_SHAPE;
+    if (!aligned16(X) || !aligned16(dY) || !aligned16(G)) return FORGE_ERR_ALIGNMENT;
+    DeviceInfo dev;
+    forge_status_t s = device_info(dev);
+    if (s != FORGE_OK) return s;
+    forge_problem_t p;
+    std::memset(&p, 0, sizeof(p));
+    p.X = X; p.dY = dY; p.m = G; p.T = T; p.out = out; p.in = in;
+    AdamWScalars hp;
+    std::memset(&hp, 0, sizeof(hp));
+    // same token-chunk length as the fused variant chosen for this T: identical summation order
+    int variant = T > 1024 ? 1 : 0;
+    const int forced = env_int("FORGE_CFG", -1);
+    if (forced >= 0) variant = forced;
+    if (variant == 1)
+        return launch_fused<MDT_FP32, MODE_STORE_G, 64, 3, 2>(&p, 1, hp, dev, reinterpret_cast<cudaStream_t>(stream));
+    return launch_fused<MDT_FP32, MODE_STORE_G, 32, 3, 3>(&p, 1, hp, dev, reinterpret_cast<cudaStream_t>(stream));
+}
+
+forge_status_t forge_adamw_from_g(const float *G, void *W, void *m, void *v, float *m_scale, float *v_scale,
+                                  int32_t out, int32_t in, int64_t step, float lr, float beta1, float beta2,
+                                  float eps, float wd, forge_moment_dtype_t moment_dtype, forge_stream_t stream) {
+    if (!G) return FORGE_ERR_NULL_PTR;
+    const int mdt = static_cast<int>(moment_dtype);
+    forge_status_t s = validate_hp(step, lr, beta1, beta2, eps, wd);
+    if (s != FORGE_OK) return s;
+    s = validate_state(W, m, v, m_scale, v_scale, out, in, mdt);
+    if (s != FORGE_OK) return s;
+    if (!aligned16(G)) return FORGE_ERR_ALIGNMENT;
+    DeviceInfo dev;
+    s = device_info(dev);
+    if (s != FORGE_OK) return s;
+    const AdamWScalars hp = make_scalars(step, lr, beta1, beta2, eps, wd);
+    const size_t n = static_cast<size_t>(out) * static_cast<size_t>(in);
+    const size_t groups = n / 8;
+    const unsigned blocks = static_cast<unsigned>((groups + 255) / 256);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    uint16_t *Wp = static_cast<uint16_t *>(W);
+    if (mdt == FORGE_MOMENT_FP32)
+        forge_adamw_from_g_kernel<MDT_FP32><<<blocks, 256, 0, st>>>(G, Wp, m, v, m_scale, v_scale, n, hp);
+    else if (mdt == FORGE_MOMENT_BF16)
+        forge_adamw_from_g_kernel<MDT_BF16><<<blocks, 256, 0, st>>>(G, Wp, m, v, m_scale, v_scale, n, hp);
+    else
+        forge_adamw_from_g_kernel<MDT_INT8><<<blocks, 256, 0, st>>>(G, Wp, m, v, m_scale, v_scale, n, hp);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e);
+    g_launches.fetch_add(1);
+    return FORGE_OK;
+}
+
+forge_status_t forge_wgrad_adamw_host(const void *X, const void *dY, void *W, void *m, void *v, float *m_scale,
+                                      float *v_scale, int32_t T, int32_t out, int32_t in, int64_t step, float lr,
+                                      float beta1, float beta2, float eps, float wd,
+                                      forge_moment_dtype_t moment_dtype) {
+    const int mdt = static_cast<int>(moment_dtype);
+    if (mdt < 0 || mdt > 2) return FORGE_ERR_BAD_DTYPE;
+    forge_problem_t hp_;
+    hp_.X = X; hp_.dY = dY; hp_.W = W; hp_.m = m; hp_.v = v; hp_.m_scale = m_scale; hp_.v_scale = v_scale;
+    hp_.T = T; hp_.out = out; hp_.in = in;
+    forge_status_t s = validate_hp(step, lr, beta1, beta2, eps, wd);
+    if (s != FORGE_OK) return s;
+    s = validate_problem(hp_, mdt);
+    if (s != FORGE_OK) return s;
+    const size_t n = static_cast<size_t>(out) * in;
+    const size_t mom = mdt == FORGE_MOMENT_FP32 ? 4 : (mdt == FORGE_MOMENT_BF16 ? 2 : 1);
+    const size_t bX = static_cast<size_t>(T) * in * 2, bY = static_cast<size_t>(T) * out * 2, bW = n * 2,
+                 bM = n * mom, bS = mdt == FORGE_MOMENT_INT8 ? n / FORGE_QBLOCK * 4 : 0;
+    auto up = [](size_t b) { return (b + 255) / 256 * 256; };
+    const size_t total = up(bX) + up(bY) + up(bW) + 2 * up(bM) + 2 * up(bS);
+    uint8_t *d = nullptr;
+    cudaError_t e = cudaMalloc(&d, total);
+    if (e != cudaSuccess) return cuda_fail(e);
+    uint8_t *dX = d, *dYp = dX + up(bX), *dW = dYp + up(bY), *dM = dW + up(bW), *dV = dM + up(bM),
+            *dMs = dV + up(bM), *dVs = dMs + up(bS);
+    cudaStream_t st = nullptr;
+    auto fail = [&](cudaError_t err) { cudaFree(d); return cuda_fail(err); };
+    if ((e = cudaMemcpyAsync(dX, X, bX, cudaMemcpyHostToDevice, st)) != cudaSuccess) return fail(e);
+    if ((e = cudaMemcpyAsync(dYp, dY, bY, cudaMemcpyHostToDevice, st)) != cudaSuccess) return fail(e);
+    if ((e = cudaMemcpyAsync(dW, W, bW, cudaMemcpyHostToDevice, st)) != cudaSuccess) return fail(e);
+    if ((e = cudaMemcpyAsync(dM, m, bM, cudaMemcpyHostToDevice, st)) != cudaSuccess) return fail(e);
+    if ((e = cudaMemcpyAsync(dV, v, bM, cudaMemcpyHostToDevice, st)) != cudaSuccess) return fail(e);
+    if (bS) {
+        if ((e = cudaMemcpyAsync(dMs, m_scale, bS, cudaMemcpyHostToDevice, st)) != cudaSuccess) return fail(e);
+        if ((e = cudaMemcpyAsync(dVs, v_scale, bS, cudaMemcpyHostToDevice, st)) != cudaSuccess) return fail(e);
+    }
+    s = forge_wgrad_adamw(dX, dYp, dW, dM, dV, bS ? reinterpret_cast<float *>(dMs) : nullptr,
+                          bS ? reinterpret_cast<float *>(dVs) : nullptr, T, out, in, step, lr, beta1, beta2, eps, wd,
+                          moment_dtype, nullptr);
+    if (s != FORGE_OK) { cudaFree(d); return s; }
+    if ((e = cudaMemcpyAsync(W, dW, bW, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return fail(e);
+    if ((e = cudaMemcpyAsync(m, dM, bM, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return fail(e);
+    if ((e = cudaMemcpyAsync(v, dV, bM, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return fail(e);
+    if (bS) {
+        if ((e = cudaMemcpyAsync(m_scale, dMs, bS, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return fail(e);
+        if ((e = cudaMemcpyAsync(v_scale, dVs, bS, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return fail(e);
+    }
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return fail(e);
+    cudaFree(d);
+    return FORGE_OK;
+}
+
+size_t forge_workspace_bytes(void) { return 0; }
+uint64_t forge_launch_count(void) { return g_launches.load(); }
+int forge_last_cuda_error(void) { return g_last_cuda_error.load(); }
+int forge_version(void) { return FORGE_VERSION; }
+
+const char *forge_status_string(forge_status_t status) {
+    switch (status) {
+    case FORGE_OK: return "FORGE_OK";
+    case FORGE_ERR_NULL_PTR: return "FORGE_ERR_NULL_PTR";
+    case FORGE_ERR_BAD_SHAPE: return "FORGE_ERR_BAD_SHAPE";
+    case FORGE_ERR_ALIGNMENT: return "FORGE_ERR_ALIGNMENT";
+    case FORGE_ERR_BAD_HYPERPARAM: return "FORGE_ERR_BAD_HYPERPARAM";
+    case FORGE_ERR_BAD_DTYPE: return "FORGE_ERR_BAD_DTYPE";
+    case FORGE_ERR_UNSUPPORTED_ARCH: return "FORGE_ERR_UNSUPPORTED_ARCH";
+    case FORGE_ERR_CUDA: return "FORGE_ERR_CUDA";
+    }
+    return "FORGE_ERR_UNKNOWN";
+}
+
+}  // extern "C"
