@@ -1,0 +1,104 @@
+"""Tolerance arithmetic for GPU-vs-oracle parity (BASELINE.json north_star).
+
+e_ij = T * 2^-23 * sum_t |dY_ti||X_tj| bounds the fp32 accumulation error of g.
+  m : |dm| <= 1e-4*|m| + (1-b1)*e
+  v : |dv| <= 1e-4*v   + (1-b2)*(2|g|e + e^2)
+  W : <= 1 bf16 ulp of the oracle's W where |g| > 4e, <= 2*lr (+1 ulp) elsewhere
+  bf16 moments: + 1 bf16 ulp of the oracle value;  int8: codes +-1, scales rel 1e-3.
+All expected values come from oracle/ only.
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from oracle import forge_oracle as fo
+from paper_2606_22932_b200 import synth
+
+F = np.float32
+
+
+def hp_tuple(hp):
+    return (hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
+
+
+def bf16_ulp(x: np.ndarray) -> np.ndarray:
+    """Spacing of bf16 numbers at |x| (8 significant bits)."""
+    a = np.maximum(np.abs(x), 2.0 ** -126)
+    return 2.0 ** (np.floor(np.log2(a)) - 7)
+
+
+def to_np(t: torch.Tensor) -> np.ndarray:
+    if t.dtype == torch.bfloat16:
+        return synth.bf16_bits(t)
+    return t.detach().cpu().numpy()
+
+
+class Tol:
+    """Accumulates the state-error budget over chained steps (errors decay with beta)."""
+
+    def __init__(self, shape):
+        self.m = np.zeros(shape)
+        self.v = np.zeros(shape)
+        self.w_ulps = 0
+
+    def step(self, G, E, T, hp):
+        b1, b2 = float(F(hp["beta1"])), float(F(hp["beta2"]))
+        e = T * 2.0 ** -23 * E
+        self.m = b1 * self.m + (1 - b1) * e
+        self.v = b2 * self.v + (1 - b2) * (2 * np.abs(G) * e + e * e)
+        self.w_ulps += 1
+        return e
+
+
+def check_fp(W_gpu, m_gpu, v_gpu, W_or, m_or, v_or, G, e, tol: Tol, hp, moment="fp32", label=""):
+    """W_* uint16 bf16 bits; m_*, v_* float32 arrays or uint16 bits (bf16 moments)."""
+    lr = float(F(hp["lr"]))
+    Wg, Wr = fo.bf16_to_f64(W_gpu), fo.bf16_to_f64(W_or)
+    if moment == "bf16":
+        mg, mr, vg, vr = (fo.bf16_to_f64(x) for x in (m_gpu, m_or, v_gpu, v_or))
+        extra_m, extra_v = bf16_ulp(mr), bf16_ulp(vr)
+    else:
+        mg, mr, vg, vr = (x.astype(np.float64) for x in (m_gpu, m_or, v_gpu, v_or))
+        extra_m = extra_v = 0.0
+    dm, dv, dW = np.abs(mg - mr), np.abs(vg - vr), np.abs(Wg - Wr)
+    bad_m = dm > 1e-4 * np.abs(mr) + tol.m + extra_m
+    bad_v = dv > 1e-4 * np.abs(vr) + tol.v + extra_v
+    sure = np.abs(G) > 4 * e
+    ulp = bf16_ulp(Wr)
+    bad_W = np.where(sure, dW > tol.w_ulps * ulp, dW > 2 * lr * tol.w_ulps + ulp)
+    assert not bad_m.any(), f"{label} m: {bad_m.sum()} outside tolerance, worst {dm.max():.3e}"
+    assert not bad_v.any(), f"{label} v: {bad_v.sum()} outside tolerance, worst {dv.max():.3e}"
+    assert not bad_W.any(), f"{label} W: {bad_W.sum()} outside tolerance, worst {dW.max():.3e}"
+    # the tolerance must not be hiding a systematic error: almost everything is bit-identical
+    exact = float((W_gpu == W_or).mean())
+    assert exact > 0.99, f"{label} only {exact:.4f} of W bit-identical to the oracle"
+    return dict(w_exact=exact, sure=float(sure.mean()), m_rel=float((dm / (np.abs(mr) + 1e-30)).max()))
+
+
+def check_int8(W_gpu, mq_gpu, vq_gpu, ms_gpu, vs_gpu, W_or, mq_or, vq_or, ms_or, vs_or, G, e, hp, label=""):
+    lr = float(F(hp["lr"]))
+    dq = np.abs(mq_gpu.astype(np.int32) - mq_or.astype(np.int32))
+    dvq = np.abs(vq_gpu.astype(np.int32) - vq_or.astype(np.int32))
+    assert dq.max() <= 1 and dvq.max() <= 1, f"{label} codes differ by more than 1 ({dq.max()}, {dvq.max()})"
+    assert float((dq == 0).mean()) > 0.99 and float((dvq == 0).mean()) > 0.99, f"{label} too many code flips"
+    assert np.allclose(ms_gpu, ms_or, rtol=1e-3, atol=0) and np.allclose(vs_gpu, vs_or, rtol=1e-3, atol=0), \
+        f"{label} block scales off"
+    Wg, Wr = fo.bf16_to_f64(W_gpu), fo.bf16_to_f64(W_or)
+    dW = np.abs(Wg - Wr)
+    sure = np.abs(G) > 4 * e
+    ulp = bf16_ulp(Wr)
+    bad_W = np.where(sure, dW > ulp, dW > 2 * lr + ulp)
+    assert not bad_W.any(), f"{label} W: {bad_W.sum()} outside tolerance, worst {dW.max():.3e}"
+    assert float((W_gpu == W_or).mean()) > 0.99
+
+
+def sample_rows(out: int, n_ranges: int = 3, width: int = 8, seed: int = 0):
+    """Deterministic row ranges spanning the first tile, a middle tile boundary and the last rows."""
+    rng = np.random.default_rng(seed + out)
+    starts = {0, max(0, out - width)}
+    if out > 256:
+        starts.add(128 - width // 2)            # straddles the first 128-row tile boundary
+    while len(starts) < n_ranges + 2 and out > width:
+        starts.add(int(rng.integers(0, out - width)))
+    return [(s, min(out, s + width)) for s in sorted(starts)]

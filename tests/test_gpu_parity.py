@@ -1,0 +1,259 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+BASELINE.json configs 0-3 and the edge cases; tolerances from tests/parity_util.py."""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import forge_oracle as fo
+from paper_2606_22932_b200 import binding as fb
+from paper_2606_22932_b200 import synth
+import parity_util as pu
+
+pytestmark = pytest.mark.gpu
+HP = synth.HP_DEFAULT
+DEV = "cuda"
+
+
+def hp_args(step):
+    return (step,) + pu.hp_tuple(HP)
+
+
+def gpu_state(p: synth.Problem, moment: str):
+    """Device copies of one problem's tensors + the oracle-side numpy twins (same bits)."""
+    d = dict(X=p.X.to(DEV), dY=p.dY.to(DEV), W=p.W.to(DEV).clone())
+    o = dict(X=synth.bf16_bits(p.X), dY=synth.bf16_bits(p.dY), W=synth.bf16_bits(p.W).copy())
+    if moment == "fp32":
+        d["m"], d["v"] = p.m.to(DEV).clone(), p.v.to(DEV).clone()
+        o["m"], o["v"] = p.m.numpy().copy(), p.v.numpy().copy()
+    elif moment == "bf16":
+        mb, vb = p.m.to(torch.bfloat16), p.v.to(torch.bfloat16)
+        d["m"], d["v"] = mb.to(DEV), vb.to(DEV)
+        o["m"], o["v"] = synth.bf16_bits(mb).copy(), synth.bf16_bits(vb).copy()
+    else:  # int8: the oracle's quantiser produces the seeds for both sides (reading S8)
+        mq, ms, vq, vs = fo.quantize(p.m.numpy(), p.v.numpy())
+        o.update(m=mq, v=vq, m_scale=ms, v_scale=vs)
+        d.update(m=torch.from_numpy(mq.copy()).to(DEV), v=torch.from_numpy(vq.copy()).to(DEV),
+                 m_scale=torch.from_numpy(ms.copy()).to(DEV), v_scale=torch.from_numpy(vs.copy()).to(DEV))
+    return d, o
+
+
+def oracle_step(o, moment, step, rows=None):
+    """Oracle on all rows or on a row range; returns (state after the step on those rows, G, E)."""
+    G, E = fo.wgrad(o["dY"], o["X"], rows=rows, with_abs=True)
+    sl = slice(None) if rows is None else slice(*rows)
+    W = np.ascontiguousarray(o["W"][sl]); m = np.ascontiguousarray(o["m"][sl]); v = np.ascontiguousarray(o["v"][sl])
+    if moment == "fp32":
+        fo.adamw_fp32(W, m, v, G, *hp_args(step))
+        return dict(W=W, m=m, v=v), G, E
+    if moment == "bf16":
+        fo.adamw_bf16(W, m, v, G, *hp_args(step))
+        return dict(W=W, m=m, v=v), G, E
+    ms = np.ascontiguousarray(o["m_scale"][sl]); vs = np.ascontiguousarray(o["v_scale"][sl])
+    fo.adamw_int8(W, m, v, ms, vs, G, *hp_args(step))
+    return dict(W=W, m=m, v=v, m_scale=ms, v_scale=vs), G, E
+
+
+def compare(d, ref, G, E, T, moment, rows=None, label=""):
+    sl = slice(None) if rows is None else slice(*rows)
+    tol = pu.Tol(G.shape)
+    e = tol.step(G, E, T, HP)
+    g = {k: pu.to_np(d[k][sl]) for k in ref}
+    if moment == "int8":
+        pu.check_int8(g["W"], g["m"], g["v"], g["m_scale"], g["v_scale"], ref["W"], ref["m"], ref["v"],
+                      ref["m_scale"], ref["v_scale"], G, e, HP, label)
+    else:
+        pu.check_fp(g["W"], g["m"], g["v"], ref["W"], ref["m"], ref["v"], G, e, tol, HP, moment, label)
+
+
+# ------------------------------------------------------------------------------ config 0 -----
+def test_config0_three_chained_steps_fp32():
+    """BASELINE.json cfg 0: W[384,256], T=128, zero state, fresh inputs per step, 3 steps."""
+    W = synth.config0_weight()
+    Wo, mo, vo = synth.bf16_bits(W).copy(), np.zeros((384, 256), np.float32), np.zeros((384, 256), np.float32)
+    Wg, mg, vg = W.to(DEV), torch.zeros(384, 256, device=DEV), torch.zeros(384, 256, device=DEV)
+    tol = pu.Tol((384, 256))
+    for step in (1, 2, 3):
+        X, dY = synth.config0_step_inputs(step)
+        fb.forge_wgrad_adamw(X.to(DEV), dY.to(DEV), Wg, mg, vg, step, **HP)
+        G, E = fo.wgrad(synth.bf16_bits(dY), synth.bf16_bits(X), with_abs=True)
+        fo.adamw_fp32(Wo, mo, vo, G, *hp_args(step))
+        e = tol.step(G, E, 128, HP)
+        torch.cuda.synchronize()
+        pu.check_fp(pu.to_np(Wg), pu.to_np(mg), pu.to_np(vg), Wo, mo, vo, G, e, tol, HP, "fp32", f"cfg0 step {step}")
+
+
+# ------------------------------------------------------------------------------ small shapes -
+@pytest.mark.parametrize("moment", ["fp32", "bf16", "int8"])
+@pytest.mark.parametrize("T,out,inn", [(512, 384, 768), (200, 136, 264), (1, 128, 256), (33, 8, 16), (2048, 256, 512)])
+def test_small_shapes_full_compare(moment, T, out, inn):
+    """Several tiles + ragged tails in every dimension (T not a multiple of the token chunk, out
+    not a multiple of 128, in not a multiple of 256), T=1, tiny W, and the large-T kernel variant."""
+    if moment == "int8" and inn % 256:
+        inn = 512 if inn > 256 else 256
+    p = synth.make_problem("t", T, out, inn, seed=100 + T + out)
+    d, o = gpu_state(p, moment)
+    fb.forge_wgrad_adamw(d["X"], d["dY"], d["W"], d["m"], d["v"], 10, m_scale=d.get("m_scale"),
+                         v_scale=d.get("v_scale"), **HP)
+    torch.cuda.synchronize()
+    ref, G, E = oracle_step(o, moment, 10)
+    compare(d, ref, G, E, T, moment, label=f"{moment} T={T} {out}x{inn}")
+
+
+# ------------------------------------------------------------------------------ configs 1, 2 -
+@pytest.fixture(scope="module")
+def layer_cpu():
+    return synth.make_layer(512, seed=synth.BASE_SEED + 1)
+
+
+@pytest.mark.parametrize("moment", ["fp32", "bf16", "int8"])
+def test_config1_2_llama_layer_grouped_sampled_rows(layer_cpu, moment):
+    """BASELINE.json cfg 1 (fp32) and cfg 2 (bf16, int8): the 7 projections of a Llama-3.1-8B layer
+    at full size in ONE grouped launch (the configuration bench.py times); the oracle is exact on
+    a deterministic sample of rows of every projection (rows are independent)."""
+    ds, os_ = zip(*[gpu_state(p, moment) for p in layer_cpu])
+    before = fb.forge_launch_count()
+    fb.forge_wgrad_adamw_grouped(list(ds), 10, *pu.hp_tuple(HP), {"fp32": 0, "bf16": 1, "int8": 2}[moment])
+    torch.cuda.synchronize()
+    assert fb.forge_launch_count() - before == 1
+    for p, d, o in zip(layer_cpu, ds, os_):
+        for rows in pu.sample_rows(p.out):
+            ref, G, E = oracle_step(o, moment, 10, rows)
+            compare(d, ref, G, E, 512, moment, rows, label=f"{moment} {p.name} rows {rows}")
+
+
+def test_config2_low_precision_moments_track_fp32_moments(layer_cpu):
+    """cfg 2 'each compared against fp32 moments': one step from the same seeds, the bf16 and int8
+    results stay within their storage resolution of the fp32-moment result (k projection)."""
+    p = layer_cpu[1]
+    res = {}
+    for moment in ("fp32", "bf16", "int8"):
+        d, _ = gpu_state(p, moment)
+        fb.forge_wgrad_adamw(d["X"], d["dY"], d["W"], d["m"], d["v"], 10, m_scale=d.get("m_scale"),
+                             v_scale=d.get("v_scale"), **HP)
+        res[moment] = d
+    torch.cuda.synchronize()
+    m32 = res["fp32"]["m"].double()
+    mb = res["bf16"]["m"].double()
+    assert ((mb - m32).abs() <= m32.abs() * 2.0 ** -7 + 1e-12).all()
+    mq = fo.dequantize_m(pu.to_np(res["int8"]["m"]), pu.to_np(res["int8"]["m_scale"]))
+    s = np.repeat(pu.to_np(res["int8"]["m_scale"]).astype(np.float64) / 127, 256, 1)
+    assert (np.abs(mq - m32.cpu().numpy()) <= 1.01 * s).all()       # old + new quantisation step
+    w32 = res["fp32"]["W"].double()
+    for k in ("bf16", "int8"):
+        assert ((res[k]["W"].double() - w32).abs() <= 4 * HP["lr"]).all()
+
+
+# ------------------------------------------------------------------------------ config 3 -----
+@pytest.mark.parametrize("T", [512, 2048, 8192])
+def test_config3_gate_proj_token_sweep_sampled_rows(T):
+    """BASELINE.json cfg 3: gate_proj W[14336,4096], fp32 moments, T in {512, 2048, 8192}."""
+    p = synth.make_problem("gate", T, 14336, 4096, seed=synth.BASE_SEED + 3)
+    d, o = gpu_state(p, "fp32")
+    fb.forge_wgrad_adamw(d["X"], d["dY"], d["W"], d["m"], d["v"], 10, **HP)
+    torch.cuda.synchronize()
+    for rows in pu.sample_rows(14336, n_ranges=2, width=4):
+        ref, G, E = oracle_step(o, "fp32", 10, rows)
+        compare(d, ref, G, E, T, "fp32", rows, label=f"gate T={T} rows {rows}")
+
+
+# ------------------------------------------------------------------------------ exactness ----
+@pytest.mark.parametrize("moment", ["fp32", "bf16", "int8"])
+@pytest.mark.parametrize("T", [512, 2048])
+def test_fused_equals_store_g_twin_plus_same_update_bitwise(moment, T):
+    """PAPER.md:294 / gate T0 ('max dW = 0'): the fused kernel vs the store-G twin
+    followed by the same per-element update must be bit-identical."""
+    p = synth.make_problem("x", T, 640, 768, seed=7)
+    d1, _ = gpu_state(p, moment)
+    d2 = {k: v.clone() for k, v in d1.items()}
+    fb.forge_wgrad_adamw(d1["X"], d1["dY"], d1["W"], d1["m"], d1["v"], 5, m_scale=d1.get("m_scale"),
+                         v_scale=d1.get("v_scale"), **HP)
+    G = torch.full((640, 768), float("nan"), device=DEV)
+    fb.forge_wgrad_store_g(d2["X"], d2["dY"], G)
+    assert not torch.isnan(G).any()
+    fb.forge_adamw_from_g(G, d2["W"], d2["m"], d2["v"], 5, m_scale=d2.get("m_scale"), v_scale=d2.get("v_scale"), **HP)
+    torch.cuda.synchronize()
+    for k in d1:
+        assert torch.equal(d1[k].view(torch.uint8), d2[k].view(torch.uint8)), f"{moment}: {k} differs from the unfused twin"
+
+
+def test_store_g_matches_oracle_gradient():
+    p = synth.make_problem("x", 300, 264, 520, seed=9)
+    G = torch.empty(264, 520, device=DEV)
+    fb.forge_wgrad_store_g(p.X.to(DEV), p.dY.to(DEV), G)
+    Go, E = fo.wgrad(synth.bf16_bits(p.dY), synth.bf16_bits(p.X), with_abs=True)
+    assert (np.abs(G.cpu().numpy().astype(np.float64) - Go) <= 300 * 2.0 ** -23 * E + 1e-30).all()
+
+
+def test_result_independent_of_grid_size_and_repeatable():
+    """Determinism (cf. identical digits across the paper's three variants): the
+    result is bitwise independent of how many CTAs share the tile list."""
+    p = synth.make_problem("x", 512, 1024, 1536, seed=11)
+    outs = []
+    for grid in (None, "1", "37", None):
+        if grid:
+            os.environ["FORGE_GRID"] = grid
+        else:
+            os.environ.pop("FORGE_GRID", None)
+        d, _ = gpu_state(p, "fp32")
+        fb.forge_wgrad_adamw(d["X"], d["dY"], d["W"], d["m"], d["v"], 3, **HP)
+        torch.cuda.synchronize()
+        outs.append(d)
+    os.environ.pop("FORGE_GRID", None)
+    for d in outs[1:]:
+        for k in ("W", "m", "v"):
+            assert torch.equal(outs[0][k], d[k])
+
+
+# ------------------------------------------------------------------------------ properties ---
+def test_lr_zero_keeps_w_and_inputs_untouched_moments_move():
+    p = synth.make_problem("x", 256, 256, 512, seed=13)
+    d, _ = gpu_state(p, "fp32")
+    X0, dY0, W0, m0 = d["X"].clone(), d["dY"].clone(), d["W"].clone(), d["m"].clone()
+    fb.forge_wgrad_adamw(d["X"], d["dY"], d["W"], d["m"], d["v"], 4, 0.0, HP["beta1"], HP["beta2"], HP["eps"], HP["wd"])
+    torch.cuda.synchronize()
+    assert torch.equal(d["W"], W0) and torch.equal(d["X"], X0) and torch.equal(d["dY"], dY0)
+    assert not torch.equal(d["m"], m0)
+
+
+def test_grouped_more_than_eight_problems_and_no_workspace():
+    probs = [synth.make_problem(f"p{i}", 64, 128, 256, seed=200 + i) for i in range(11)]
+    ds, os_ = zip(*[gpu_state(p, "fp32") for p in probs])
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    before = fb.forge_launch_count()
+    fb.forge_wgrad_adamw_grouped(list(ds), 2, *pu.hp_tuple(HP), 0)
+    torch.cuda.synchronize()
+    assert fb.forge_launch_count() - before == 2               # 8 + 3
+    assert torch.cuda.mem_get_info()[0] == free0               # the library allocated nothing: no dW
+    for p, d, o in zip(probs, ds, os_):
+        G, E = fo.wgrad(o["dY"], o["X"], with_abs=True)
+        fo.adamw_fp32(o["W"], o["m"], o["v"], G, 2, *pu.hp_tuple(HP))
+        tol = pu.Tol(G.shape)
+        e = tol.step(G, E, 64, HP)
+        pu.check_fp(pu.to_np(d["W"]), pu.to_np(d["m"]), pu.to_np(d["v"]), o["W"], o["m"], o["v"], G, e, tol, HP)
+
+
+def test_bad_arguments_leave_state_untouched_on_gpu():
+    p = synth.make_problem("x", 64, 128, 256, seed=17)
+    d, _ = gpu_state(p, "fp32")
+    W0, m0 = d["W"].clone(), d["m"].clone()
+    st = fb.forge_wgrad_adamw(d["X"], d["dY"], d["W"], d["m"], d["v"], 0, check=False, **HP)
+    assert st == 4
+    with pytest.raises(fb.ForgeError):
+        fb.forge_wgrad_adamw(d["X"], d["dY"], d["W"], d["m"][:, 1:], d["v"], 1, **HP)   # misaligned
+    torch.cuda.synchronize()
+    assert torch.equal(d["W"], W0) and torch.equal(d["m"], m0)
+
+
+def test_host_buffer_entry_point_matches_device_path():
+    p = synth.make_problem("x", 128, 256, 512, seed=19)
+    d, _ = gpu_state(p, "fp32")
+    fb.forge_wgrad_adamw(d["X"], d["dY"], d["W"], d["m"], d["v"], 6, **HP)
+    h = dict(X=p.X.clone().pin_memory(), dY=p.dY.clone().pin_memory(), W=p.W.clone().pin_memory(),
+             m=p.m.clone().pin_memory(), v=p.v.clone().pin_memory())
+    fb.forge_wgrad_adamw_host(h["X"], h["dY"], h["W"], h["m"], h["v"], 6, **HP)
+    torch.cuda.synchronize()
+    for k in ("W", "m", "v"):
+        assert torch.equal(d[k].cpu(), h[k])
