@@ -1,0 +1,376 @@
+#!/usr/bin/env python
+"""bench.py -- measures BASELINE.json's metric: fused wgrad+AdamW microseconds per Llama-3.1-8B layer
+(7 projections as one grouped launch, T=512, bf16 W, fp32 m/v; BASELINE.json configs[1]) and its
+fraction of the HBM roofline on one B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--moments fp32|bf16|int8] [--impl reference]
+
+A "step" is one pass of the whole hot path over one synthetic layer:
+one forge_wgrad_adamw_grouped call.  Inputs are resident in HBM before the timed region; the
+working set (4.4 GB of state per layer) is far larger than the 126 MB L2, so no flush is needed.
+With N > 1 (torchrun) every rank runs its own layer (weak scaling, no collective on the data
+path: the tiles are independent); `value` is then us per layer over all
+ranks.  `--impl reference` times the CPU oracle (the only "reference implementation" this build
+has) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fused wgrad+AdamW us/layer (Llama-3.1-8B layer, 7 projections, BT=512, 1xB200)"
+UNIT = "us/layer"
+MOMENT_BYTES = {"fp32": 20.0, "bf16": 12.0, "int8": 8.0 + 2 * 2 * 4 / 256}   # SURVEY.md 8(d), B/element
+MOMENT_ENUM = {"fp32": 0, "bf16": 1, "int8": 2}
+T_TOKENS = 512
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed
+# ncu --set full capture (profiles/); None until a capture of the current kernel exists.
+NCU_TRAFFIC_BYTES = {"fp32": None, "bf16": None, "int8": None}
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def layer_counts():
+    from paper_2606_22932_b200 import synth
+    params = sum(o * i for _, o, i in synth.LLAMA8B_LAYER)
+    xs = {}
+    for name, o, i in synth.LLAMA8B_LAYER:
+        xs[(synth.X_GROUP[name], i)] = i
+    in_bytes = 2 * T_TOKENS * (sum(xs.values()) + sum(o for _, o, _ in synth.LLAMA8B_LAYER))
+    flops = 2 * params * T_TOKENS
+    return params, in_bytes, flops
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons with NVML during the timed region."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.sm, self.reasons, self.max_mhz = index, False, [], set(), None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap"}
+        while not self.stop_flag:
+            try:
+                self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, n in names.items():
+                    if r & bit:
+                        self.reasons.add(n)
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def result(self):
+        sm = sorted(self.sm)
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+# workload construction (synthetic, seeded; shapes of BASELINE.json configs[1] / [2])
+# ------------------------------------------------------------------------------------------------
+def make_device_layer(moments: str, seed: int, device):
+    """One Llama-3.1-8B layer's 7 problems on the device (inputs resident in HBM)."""
+    import torch
+    from paper_2606_22932_b200 import synth
+    probs = synth.make_layer(T_TOKENS, seed, device=device)
+    out = []
+    for p in probs:
+        d = dict(X=p.X, dY=p.dY, W=p.W)
+        if moments == "fp32":
+            d["m"], d["v"] = p.m, p.v
+        elif moments == "bf16":
+            d["m"], d["v"] = p.m.to(torch.bfloat16), p.v.to(torch.bfloat16)
+        else:
+            # seed codes/scales with torch ops only (initial state; the method's arithmetic starts at step 1)
+            nb = p.inn // 256
+            ms = p.m.view(p.out, nb, 256).abs().amax(-1)
+            vs = p.v.view(p.out, nb, 256).amax(-1)
+            d["m"] = torch.round(p.m.view(p.out, nb, 256) * (127.0 / ms)[..., None]).clamp(-127, 127).to(torch.int8).view(p.out, p.inn)
+            d["v"] = torch.round(p.v.view(p.out, nb, 256) * (255.0 / vs)[..., None]).clamp(1, 255).to(torch.uint8).view(p.out, p.inn)
+            d["m_scale"], d["v_scale"] = ms.contiguous(), vs.contiguous()
+        out.append(d)
+    return out
+
+
+def make_host_layer(moments: str, seed: int):
+    """The same layer in pinned host memory for the end-to-end (host buffer) measurement."""
+    layer = make_device_layer(moments, seed, "cpu")
+    return [{k: v.contiguous().pin_memory() for k, v in d.items()} for d in layer]
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle timing (cpu_baseline leg and --impl reference)
+# ------------------------------------------------------------------------------------------------
+_CPU_LAYER = {}
+
+
+def oracle_time_sample(frac_den: int, seed: int):
+    """Times the oracle, as it stands, on rows [0, out/frac_den) of every projection of one layer.
+    Returns (seconds, description, threads)."""
+    from oracle import forge_oracle as fo
+    from paper_2606_22932_b200 import synth
+    hp = synth.HP_DEFAULT
+    if seed not in _CPU_LAYER:
+        _CPU_LAYER[seed] = synth.make_layer(T_TOKENS, seed)
+    layer = _CPU_LAYER[seed]
+    work = []
+    for p in layer:
+        r = max(1, p.out // frac_den)
+        work.append((synth.bf16_bits(p.dY), synth.bf16_bits(p.X), synth.bf16_bits(p.W)[:r].copy(),
+                     p.m.numpy()[:r].copy(), p.v.numpy()[:r].copy(), r))
+    fo.lib()
+    t0 = time.perf_counter()
+    for dY, X, W, m, v, r in work:
+        G = fo.wgrad(dY, X, rows=(0, r))
+        fo.adamw_fp32(W, m, v, G, 10, hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
+    dt = time.perf_counter() - t0
+    return dt, f"first 1/{frac_den} of the rows of each of the 7 projections, T=512, fp32 moments, scaled x{frac_den}", fo.num_threads()
+
+
+def cpu_baseline(seed: int):
+    den = 16
+    dt, desc, threads = oracle_time_sample(den, seed)
+    if dt * 4 < 20.0:                      # aim at ~10-30 s of CPU work
+        den = 4
+        dt, desc, threads = oracle_time_sample(den, seed)
+    return {"value": dt * den * 1e6, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
+            "sample_seconds": round(dt, 3)}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    den = 16
+    times = []
+    for i in range(args.warmup + args.steps):
+        dt, desc, threads = oracle_time_sample(den, 20260622 + 1)
+        if i >= args.warmup:
+            times.append(dt)
+        if sum(times) > 150:
+            break
+    us = sum(times) / len(times) * den * 1e6
+    line = {"impl": "reference", "metric": METRIC, "value": us, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": len(times), "warmup": args.warmup, "ms_per_step": us / 1e3, "higher_is_better": False,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "configs[1]: Llama-3.1-8B layer, 7 projections, T=512, fp32 m/v",
+                       "moments": "fp32", "params_per_layer": layer_counts()[0]},
+            "cpu_baseline": {"value": us, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
+            "e2e": {"value": us, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ------------------------------------------------------------------------------------------------
+def time_unfused_baselines(layer, hp, steps):
+    """Context arms on the same GPU: cuBLAS dW then a separate optimizer pass.
+    B3: fp32 dW (cuBLAS via torch.mm) + this library's elementwise kernel over the materialised G
+        (byte-matched control, 28 B/element + the GEMM);
+    B1: all-bf16 cuBLAS dW + torch._fused_adamw_ on bf16 W/m/v (the paper's "fused AdamW" arm)."""
+    import torch
+    from paper_2606_22932_b200 import binding as fb
+    res = {}
+    Gs = [torch.empty(d["W"].shape, dtype=torch.float32, device=d["W"].device) for d in layer]
+
+    def run_b3():
+        for d, G in zip(layer, Gs):
+            if HAS_OUT_DTYPE[0]:
+                torch.mm(d["dY"].t(), d["X"], out_dtype=torch.float32, out=G)
+            else:   # bf16 cuBLAS output widened afterwards (torch build without out_dtype)
+                G.copy_(torch.mm(d["dY"].t(), d["X"]))
+            fb.forge_adamw_from_g(G, d["W"], d["m"], d["v"], 10, hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
+
+    HAS_OUT_DTYPE = [True]
+    try:
+        torch.mm(layer[1]["dY"].t(), layer[1]["X"], out_dtype=torch.float32)
+    except Exception:
+        HAS_OUT_DTYPE[0] = False
+
+    def timeit(fn, n):
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n * 1e3
+
+    if layer[0]["m"].dtype == torch.float32:
+        res["cublas_dw_fp32_plus_elementwise_adamw_us"] = timeit(run_b3, steps)
+        res["cublas_dw_out_dtype_fp32"] = HAS_OUT_DTYPE[0]
+    try:
+        Wb = [d["W"].clone() for d in layer]
+        mb = [torch.zeros_like(w) for w in Wb]
+        vb = [torch.zeros_like(w) for w in Wb]
+        st = [torch.tensor(9.0, device=w.device) for w in Wb]
+
+        def run_b1():
+            grads = [torch.mm(d["dY"].t(), d["X"]) for d in layer]
+            torch._fused_adamw_(Wb, grads, mb, vb, [], st, lr=hp["lr"], beta1=hp["beta1"], beta2=hp["beta2"],
+                                weight_decay=hp["wd"], eps=hp["eps"], amsgrad=False, maximize=False)
+        res["cublas_dw_bf16_plus_torch_fused_adamw_bf16_us"] = timeit(run_b1, steps)
+    except Exception as ex:  # pragma: no cover
+        res["cublas_dw_bf16_plus_torch_fused_adamw_bf16_us"] = None
+        res["b1_error"] = str(ex)[:200]
+    return res
+
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_22932_b200 import binding as fb
+    from paper_2606_22932_b200 import synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; there is no CPU fallback for the product path")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    fb.lib()                                       # fails loudly if the CUDA library is missing
+    hp = synth.HP_DEFAULT
+    mdt = MOMENT_ENUM[args.moments]
+    layer = make_device_layer(args.moments, 20260622 + 1 + rank, dev)
+    arr = fb.make_problem_array(layer)
+    hpt = (hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
+    stream = torch.cuda.current_stream()
+
+    def step(t):
+        fb.forge_wgrad_adamw_grouped(layer, t, *hpt, mdt, stream=stream, _arr=arr)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for i in range(args.warmup):
+        step(1 + i)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    launches0 = fb.forge_launch_count()
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    evs[0].record(stream)
+    for i in range(args.steps):
+        step(1 + args.warmup + i)
+        evs[i + 1].record(stream)
+    barrier()
+    sampler.stop_flag = True
+    launches = fb.forge_launch_count() - launches0
+    total_ms = evs[0].elapsed_time(evs[-1])
+    per_launch_ms = sorted(evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps))
+    t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    us_per_layer = ms_per_step * 1e3 / world       # layers processed by all ranks per step = world
+
+    params, in_bytes, flops = layer_counts()
+    alg_bytes = params * MOMENT_BYTES[args.moments] + in_bytes
+    peak, peak_src = measured_peaks()
+    kernel_ms = (evs[0].elapsed_time(evs[-1])) / args.steps       # this rank's average launch duration
+    achieved = alg_bytes / (kernel_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": NCU_TRAFFIC_BYTES[args.moments], "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg_bytes, "launch_us_avg": kernel_ms * 1e3,
+                "launch_us_median": per_launch_ms[len(per_launch_ms) // 2] * 1e3,
+                "tflops": flops / (kernel_ms * 1e-3) / 1e12,
+                "frac_of_datasheet_8TBs": achieved / 8000.0}
+
+    line = {"metric": METRIC, "value": us_per_layer, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "configs[1]: Llama-3.1-8B layer, 7 projections in one grouped launch, T=512"
+                                   if args.moments == "fp32" else f"configs[2]: same layer, {args.moments} moments",
+                       "moments": args.moments, "params_per_layer": params, "tokens": T_TOKENS,
+                       "l2": "working set 4.4 GB/layer >> 126 MB L2, no flush needed",
+                       "parallelism": f"replicated layers x{world}, no collective"},
+            "roofline": roofline, "gpu_launches": int(launches), "clocks": sampler.result(),
+            "dw_bytes_allocated": 0, "library_workspace_bytes": fb.forge_workspace_bytes()}
+
+    if rank == 0 and not args.no_extras:
+        # ---- end to end through the C ABI with HOST buffers (H2D + kernel + D2H inside the call)
+        host = make_host_layer(args.moments, 20260622 + 1)
+        h2d = sum(sum(v.numel() * v.element_size() for v in d.values()) for d in host)
+        d2h = sum(sum(d[k].numel() * d[k].element_size() for k in d if k not in ("X", "dY")) for d in host)
+        def e2e_step(tt):
+            for d in host:
+                fb.forge_wgrad_adamw_host(d["X"], d["dY"], d["W"], d["m"], d["v"], tt, *hpt,
+                                          m_scale=d.get("m_scale"), v_scale=d.get("v_scale"))
+        e2e_step(1)
+        n_e2e = max(1, min(3, args.steps))
+        t0 = time.perf_counter()
+        for i in range(n_e2e):
+            e2e_step(2 + i)
+        torch.cuda.synchronize()
+        e2e_us = (time.perf_counter() - t0) / n_e2e * 1e6
+        line["e2e"] = {"value": e2e_us, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                       "steps": n_e2e, "api": "forge_wgrad_adamw_host x7 (pinned host buffers)"}
+        del host
+        line["baselines_same_gpu"] = time_unfused_baselines(layer, hp, max(3, min(10, args.steps)))
+        if world == 1:
+            line["cpu_baseline"] = cpu_baseline(20260622 + 1)
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--moments", choices=["fp32", "bf16", "int8"], default="fp32")
+    ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
+    ap.add_argument("--no-extras", action="store_true", help="skip e2e, same-GPU baselines and the CPU oracle leg")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -55,16 +55,17 @@ def oracle_step(o, moment, step, rows=None):
     return dict(W=W, m=m, v=v, m_scale=ms, v_scale=vs), G, E
 
 
-def compare(d, ref, G, E, T, moment, rows=None, label=""):
+def compare(d, ref, G, E, T, moment, rows=None, label="", W_prev=None):
     sl = slice(None) if rows is None else slice(*rows)
+    W_prev = None if W_prev is None else W_prev[sl]
     tol = pu.Tol(G.shape)
     e = tol.step(G, E, T, HP)
     g = {k: pu.to_np(d[k][sl]) for k in ref}
     if moment == "int8":
         pu.check_int8(g["W"], g["m"], g["v"], g["m_scale"], g["v_scale"], ref["W"], ref["m"], ref["v"],
-                      ref["m_scale"], ref["v_scale"], G, e, HP, label)
+                      ref["m_scale"], ref["v_scale"], G, e, HP, label, W_prev=W_prev)
     else:
-        pu.check_fp(g["W"], g["m"], g["v"], ref["W"], ref["m"], ref["v"], G, e, tol, HP, moment, label)
+        pu.check_fp(g["W"], g["m"], g["v"], ref["W"], ref["m"], ref["v"], G, e, tol, HP, moment, label, W_prev=W_prev)
 
 
 # ------------------------------------------------------------------------------ config 0 -----
@@ -78,10 +79,12 @@ def test_config0_three_chained_steps_fp32():
         X, dY = synth.config0_step_inputs(step)
         fb.forge_wgrad_adamw(X.to(DEV), dY.to(DEV), Wg, mg, vg, step, **HP)
         G, E = fo.wgrad(synth.bf16_bits(dY), synth.bf16_bits(X), with_abs=True)
+        W_prev = Wo.copy()
         fo.adamw_fp32(Wo, mo, vo, G, *hp_args(step))
         e = tol.step(G, E, 128, HP)
         torch.cuda.synchronize()
-        pu.check_fp(pu.to_np(Wg), pu.to_np(mg), pu.to_np(vg), Wo, mo, vo, G, e, tol, HP, "fp32", f"cfg0 step {step}")
+        pu.check_fp(pu.to_np(Wg), pu.to_np(mg), pu.to_np(vg), Wo, mo, vo, G, e, tol, HP, "fp32", f"cfg0 step {step}",
+                    W_prev=W_prev)
 
 
 # ------------------------------------------------------------------------------ small shapes -
@@ -98,7 +101,7 @@ def test_small_shapes_full_compare(moment, T, out, inn):
                          v_scale=d.get("v_scale"), **HP)
     torch.cuda.synchronize()
     ref, G, E = oracle_step(o, moment, 10)
-    compare(d, ref, G, E, T, moment, label=f"{moment} T={T} {out}x{inn}")
+    compare(d, ref, G, E, T, moment, label=f"{moment} T={T} {out}x{inn}", W_prev=o["W"])
 
 
 # ------------------------------------------------------------------------------ configs 1, 2 -
@@ -120,7 +123,7 @@ def test_config1_2_llama_layer_grouped_sampled_rows(layer_cpu, moment):
     for p, d, o in zip(layer_cpu, ds, os_):
         for rows in pu.sample_rows(p.out):
             ref, G, E = oracle_step(o, moment, 10, rows)
-            compare(d, ref, G, E, 512, moment, rows, label=f"{moment} {p.name} rows {rows}")
+            compare(d, ref, G, E, 512, moment, rows, label=f"{moment} {p.name} rows {rows}", W_prev=o["W"])
 
 
 def test_config2_low_precision_moments_track_fp32_moments(layer_cpu):
@@ -155,7 +158,7 @@ def test_config3_gate_proj_token_sweep_sampled_rows(T):
     torch.cuda.synchronize()
     for rows in pu.sample_rows(14336, n_ranges=2, width=4):
         ref, G, E = oracle_step(o, "fp32", 10, rows)
-        compare(d, ref, G, E, T, "fp32", rows, label=f"gate T={T} rows {rows}")
+        compare(d, ref, G, E, T, "fp32", rows, label=f"gate T={T} rows {rows}", W_prev=o["W"])
 
 
 # ------------------------------------------------------------------------------ exactness ----
@@ -229,10 +232,11 @@ def test_grouped_more_than_eight_problems_and_no_workspace():
     assert torch.cuda.mem_get_info()[0] == free0               # the library allocated nothing: no dW
     for p, d, o in zip(probs, ds, os_):
         G, E = fo.wgrad(o["dY"], o["X"], with_abs=True)
+        W_prev = o["W"].copy()
         fo.adamw_fp32(o["W"], o["m"], o["v"], G, 2, *pu.hp_tuple(HP))
         tol = pu.Tol(G.shape)
         e = tol.step(G, E, 64, HP)
-        pu.check_fp(pu.to_np(d["W"]), pu.to_np(d["m"]), pu.to_np(d["v"]), o["W"], o["m"], o["v"], G, e, tol, HP)
+        pu.check_fp(pu.to_np(d["W"]), pu.to_np(d["m"]), pu.to_np(d["v"]), o["W"], o["m"], o["v"], G, e, tol, HP, W_prev=W_prev)
 
 
 def test_bad_arguments_leave_state_untouched_on_gpu():
