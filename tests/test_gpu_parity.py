@@ -43,14 +43,14 @@ def oracle_step(o, moment, step, rows=None):
     """Oracle on all rows or on a row range; returns (state after the step on those rows, G, E)."""
     G, E = fo.wgrad(o["dY"], o["X"], rows=rows, with_abs=True)
     sl = slice(None) if rows is None else slice(*rows)
-    W = np.ascontiguousarray(o["W"][sl]); m = np.ascontiguousarray(o["m"][sl]); v = np.ascontiguousarray(o["v"][sl])
+    W, m, v = o["W"][sl].copy(), o["m"][sl].copy(), o["v"][sl].copy()      # the seeds stay untouched
     if moment == "fp32":
         fo.adamw_fp32(W, m, v, G, *hp_args(step))
         return dict(W=W, m=m, v=v), G, E
     if moment == "bf16":
         fo.adamw_bf16(W, m, v, G, *hp_args(step))
         return dict(W=W, m=m, v=v), G, E
-    ms = np.ascontiguousarray(o["m_scale"][sl]); vs = np.ascontiguousarray(o["v_scale"][sl])
+    ms, vs = o["m_scale"][sl].copy(), o["v_scale"][sl].copy()
     fo.adamw_int8(W, m, v, ms, vs, G, *hp_args(step))
     return dict(W=W, m=m, v=v, m_scale=ms, v_scale=vs), G, E
 
@@ -139,7 +139,9 @@ def test_config2_low_precision_moments_track_fp32_moments(layer_cpu):
     torch.cuda.synchronize()
     m32 = res["fp32"]["m"].double()
     mb = res["bf16"]["m"].double()
-    assert ((mb - m32).abs() <= m32.abs() * 2.0 ** -7 + 1e-12).all()
+    m0 = p.m.to(DEV).double().abs()
+    # bf16 seeds differ from the fp32 seeds by <= 2^-9 |m0|, the bf16 store adds <= 2^-9 |m'|
+    assert ((mb - m32).abs() <= 2.0 ** -8 * (m0 + m32.abs()) + 1e-12).all()
     mq = fo.dequantize_m(pu.to_np(res["int8"]["m"]), pu.to_np(res["int8"]["m_scale"]))
     s = np.repeat(pu.to_np(res["int8"]["m_scale"]).astype(np.float64) / 127, 256, 1)
     assert (np.abs(mq - m32.cpu().numpy()) <= 1.01 * s).all()       # old + new quantisation step
