@@ -23,12 +23,26 @@ struct AdamWScalars {
 // m' = b1 m + (1-b1) g ; v' = b2 v + (1-b2) g^2 ;
 // W' = (1 - lr wd) W - lr * (m'/bc1) / (sqrt(v'/bc2) + eps)          (Alg. 1 lines 7-10)
 // sqrt(v'/bc2) is evaluated as sqrt(v') * (1/sqrt(bc2)); W' uses the unrounded m', v'.
+// The square root and the reciprocal are the hardware approximations (MUFU.SQRT / MUFU.RCP,
+// <= 1-2 ulp of fp32 each): the ratio is off by <= ~2^-21 relative, i.e. W' by <= lr*2^-21*|ratio|,
+// four orders of magnitude below a bf16 ulp of W; the IEEE sequences cost ~4x the instructions
+// and made the epilogue, not HBM, the bottleneck (profiles/r01_fp32_first.md).
+__device__ __forceinline__ float sqrt_fast(float x) {
+    float y;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_fast(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 __device__ __forceinline__ void adamw_update(const AdamWScalars &h, float g, float &w, float &m,
                                              float &v) {
     m = __fmaf_rn(h.beta1, m, __fmul_rn(h.one_minus_beta1, g));
     v = __fmaf_rn(h.beta2, v, __fmul_rn(__fmul_rn(h.one_minus_beta2, g), g));
-    const float denom = __fmaf_rn(__fsqrt_rn(v), h.inv_sqrt_bc2, h.eps);
-    const float ratio = __fdiv_rn(m, denom);
+    const float denom = __fmaf_rn(sqrt_fast(v), h.inv_sqrt_bc2, h.eps);
+    const float ratio = __fmul_rn(m, rcp_fast(denom));
     w = __fmaf_rn(-h.step_size, ratio, __fmul_rn(h.decay, w));
 }
 

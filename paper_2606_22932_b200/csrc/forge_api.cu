@@ -147,11 +147,11 @@ int env_int(const char *name, int dflt) {
 // ---------------------------------------------------------------------------------------------
 // launch of one fused-kernel instantiation over <= kMaxProblems problems
 // ---------------------------------------------------------------------------------------------
-template <int MDT, int MODE, int BK, int ST, int SS>
+template <int MDT, int MODE, int BK, int ST, int SS, int CG = 1>
 forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamWScalars &hp,
                             const DeviceInfo &dev, cudaStream_t stream) {
-    using Cfg = KernelCfg<MDT, BK, ST, SS>;
-    auto kernel = forge_fused_kernel<MDT, MODE, BK, ST, SS>;
+    using Cfg = KernelCfg<MDT, BK, ST, SS, CG>;
+    auto kernel = forge_fused_kernel<MDT, MODE, BK, ST, SS, CG>;
     static std::once_flag once;
     static cudaError_t attr_err = cudaSuccess;
     std::call_once(once, [&] {
@@ -192,15 +192,27 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
         d.in = p.in;
         d.tiles_n = (p.in + BLOCK_N - 1) / BLOCK_N;
         d.tile_begin = tiles;
-        tiles += ((p.out + BLOCK_M - 1) / BLOCK_M) * d.tiles_n;
+        tiles += ((p.out + BLOCK_M * CG - 1) / (BLOCK_M * CG)) * d.tiles_n;   // (128*CG) x 256 work units
     }
     P.total_tiles = tiles;
-    int grid = dev.sm_count;
+    int grid = dev.sm_count / CG;                  // persistent: one CTA (or CTA pair) per SM (pair)
     const int forced = env_int("FORGE_GRID", 0);   // debug/determinism tests only
-    if (forced > 0) grid = forced;
+    if (forced > 0) grid = (forced + CG - 1) / CG;
     if (grid > tiles) grid = tiles;
-    kernel<<<grid, kThreads, Cfg::SMEM_BYTES, stream>>>(P);
-    cudaError_t e = cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(grid * CG));
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CG;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kernel, P);
+    if (e == cudaSuccess) e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
     g_launches.fetch_add(1);
     return FORGE_OK;
@@ -221,13 +233,18 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
     case FORGE_MOMENT_FP32:
         if (variant == 1) return launch_fused<MDT_FP32, MODE_ADAMW, 64, 3, 2>(probs, count, hp, dev, stream);
         if (variant == 2) return launch_fused<MDT_FP32, MODE_ADAMW, 32, 2, 4>(probs, count, hp, dev, stream);
-        return launch_fused<MDT_FP32, MODE_ADAMW, 32, 3, 3>(probs, count, hp, dev, stream);
+        if (variant == 3) return launch_fused<MDT_FP32, MODE_ADAMW, 32, 3, 4, 2>(probs, count, hp, dev, stream);
+        if (variant == 4) return launch_fused<MDT_FP32, MODE_ADAMW, 64, 2, 4, 2>(probs, count, hp, dev, stream);
+        if (variant == 5) return launch_fused<MDT_FP32, MODE_ADAMW, 64, 4, 2, 2>(probs, count, hp, dev, stream);
+        return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 4, 2>(probs, count, hp, dev, stream);
     case FORGE_MOMENT_BF16:
-        if (variant == 1) return launch_fused<MDT_BF16, MODE_ADAMW, 64, 3, 3>(probs, count, hp, dev, stream);
-        return launch_fused<MDT_BF16, MODE_ADAMW, 32, 3, 6>(probs, count, hp, dev, stream);
+        if (variant == 1) return launch_fused<MDT_BF16, MODE_ADAMW, 64, 3, 2>(probs, count, hp, dev, stream);
+        if (variant == 2) return launch_fused<MDT_BF16, MODE_ADAMW, 32, 3, 6>(probs, count, hp, dev, stream);
+        if (variant == 3) return launch_fused<MDT_BF16, MODE_ADAMW, 64, 2, 6, 2>(probs, count, hp, dev, stream);
+        return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 6, 2>(probs, count, hp, dev, stream);
     case FORGE_MOMENT_INT8:
-        if (variant == 1) return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 9>(probs, count, hp, dev, stream);
-        return launch_fused<MDT_INT8, MODE_ADAMW, 32, 2, 10>(probs, count, hp, dev, stream);
+        if (variant == 2) return launch_fused<MDT_INT8, MODE_ADAMW, 32, 2, 10>(probs, count, hp, dev, stream);
+        return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 10, 2>(probs, count, hp, dev, stream);
     default:
         return FORGE_ERR_BAD_DTYPE;
     }
@@ -294,7 +311,7 @@ forge_status_t forge_wgrad_store_g(const void *X, const void *dY, float *G, int3
     if (forced >= 0) variant = forced;
     if (variant == 1)
         return launch_fused<MDT_FP32, MODE_STORE_G, 64, 3, 2>(&p, 1, hp, dev, reinterpret_cast<cudaStream_t>(stream));
-    return launch_fused<MDT_FP32, MODE_STORE_G, 32, 3, 3>(&p, 1, hp, dev, reinterpret_cast<cudaStream_t>(stream));
+    return launch_fused<MDT_FP32, MODE_STORE_G, 32, 2, 4>(&p, 1, hp, dev, reinterpret_cast<cudaStream_t>(stream));
 }
 
 forge_status_t forge_adamw_from_g(const float *G, void *W, void *m, void *v, float *m_scale, float *v_scale,

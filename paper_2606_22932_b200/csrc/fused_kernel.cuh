@@ -65,11 +65,16 @@ struct alignas(64) KernelParams {
     int32_t total_tiles;
 };
 
-template <int MDT, int kBlockK, int kStages, int kStateStages>
+// CG = 1: one CTA per 128x256 tile.  CG = 2: a CTA pair (cluster of 2, tcgen05 cta_group::2) shares
+// a 256x256 tile: each CTA stages its own 128 rows of A = dY^T and only HALF of B = X (128 of the
+// 256 columns), the pair's leader issues one M=256 MMA that reads both CTAs' shared memory, and
+// each CTA's TMEM receives its own 128 x 256 accumulator.  Operand bytes per CTA fall by a third
+// (L2 -> SM traffic and smem per stage), the state path stays CTA-local.
+template <int MDT, int kBlockK, int kStages, int kStateStages, int CG = 1>
 struct KernelCfg {
     static constexpr int kMomBytes = (MDT == MDT_FP32) ? 4 : (MDT == MDT_BF16 ? 2 : 1);
     static constexpr int A_STAGE = kBlockK * 128 * (BLOCK_M / 64);
-    static constexpr int B_STAGE = kBlockK * 128 * (BLOCK_N / 64);
+    static constexpr int B_STAGE = kBlockK * 128 * (BLOCK_N / 64) / CG;
     static constexpr int ML_STAGE = A_STAGE + B_STAGE;
     static constexpr int W_ROW = CHUNK_N * 2;
     static constexpr int M_ROW = CHUNK_N * kMomBytes;
@@ -83,20 +88,28 @@ struct KernelCfg {
                                       kStateStages * ST_STAGE + kNumBars * 8 + 16 + XCHG_BYTES;
     static_assert(SMEM_BYTES <= 232448, "shared memory budget exceeded");
     static_assert(kBlockK % 16 == 0 && kBlockK >= 16, "kBlockK must be a multiple of UMMA_K");
+    static_assert(CG == 1 || CG == 2, "CTA group is 1 or 2");
     static_assert(MDT != MDT_INT8 || kStateStages >= CHUNKS + 1, "int8 needs a whole tile resident");
+    // Chunk ci lives in ring slot ci % kStateStages and is consumed by epilogue warpgroup ci % 2.
+    // With an even ring every slot always belongs to the same warpgroup, so a warpgroup observes
+    // every phase of the slot barriers it waits on; with an odd ring it would skip the other
+    // warpgroup's phases and an mbarrier parity wait could alias to a phase two steps back.
+    static_assert(kStateStages % 2 == 0, "state ring must be even (one consumer warpgroup per slot)");
 };
 
 struct TileCoord {
-    int p, tm, tn;
+    int p, tm, tn;   // problem, 128-row block of THIS CTA, 256-column block
 };
-__device__ __forceinline__ TileCoord decode_tile(const KernelParams &P, int tile) {
+// `tile` indexes (128*CG) x 256 work units; rank is this CTA's rank in its pair (0 when CG = 1)
+template <int CG>
+__device__ __forceinline__ TileCoord decode_tile(const KernelParams &P, int tile, uint32_t rank) {
     int p = 0;
 #pragma unroll 1
     for (int i = 1; i < P.num_problems; ++i)
         if (tile >= P.prob[i].tile_begin) p = i;
     const int local = tile - P.prob[p].tile_begin;
     const int tn_count = P.prob[p].tiles_n;
-    return TileCoord{p, local / tn_count, local % tn_count};
+    return TileCoord{p, (local / tn_count) * CG + static_cast<int>(rank), local % tn_count};
 }
 
 // byte offset of 16-byte chunk j of row r in a TMA-swizzled box whose rows are ROW bytes long
@@ -182,12 +195,12 @@ __device__ __forceinline__ uint4 pack_codes(const int (&c)[16]) {
     return make_uint4(w[0], w[1], w[2], w[3]);
 }
 
-template <class Cfg, int kStateStages>
-__device__ __forceinline__ void epi_tile_int8(const KernelParams &P, const AdamWScalars &hp, int tile,
+template <class Cfg, int kStateStages, int CG>
+__device__ __forceinline__ void epi_tile_int8(const KernelParams &P, const AdamWScalars &hp, int tile, uint32_t rank,
                                               uint32_t titer, uint32_t taddr, uint32_t sST,
                                               uint32_t bar_st_full, uint32_t bar_st_done, uint32_t row,
                                               int wg, uint32_t s_xchg) {
-    const TileCoord tc = decode_tile(P, tile);
+    const TileCoord tc = decode_tile<CG>(P, tile, rank);
     const ProblemDesc &pd = P.prob[tc.p];
     const int row_g = tc.tm * BLOCK_M + static_cast<int>(row);
     const bool valid = row_g < pd.out;
@@ -272,10 +285,11 @@ __device__ __forceinline__ void epi_tile_int8(const KernelParams &P, const AdamW
 // ---------------------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------------------
-template <int MDT, int MODE, int kBlockK, int kStages, int kStateStages>
+template <int MDT, int MODE, int kBlockK, int kStages, int kStateStages, int CG>
 __global__ void __launch_bounds__(kThreads, 1)
 forge_fused_kernel(const __grid_constant__ KernelParams P) {
-    using Cfg = KernelCfg<MDT, kBlockK, kStages, kStateStages>;
+    using Cfg = KernelCfg<MDT, kBlockK, kStages, kStateStages, CG>;
+    const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;   // rank 0 = the pair's leader
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t sML = smem_base;                                   // mainloop ring
@@ -302,7 +316,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         }
         for (int i = 0; i < 2; ++i) {
             mbar_init(bar_tm_full + 8 * i, 1);
-            mbar_init(bar_tm_empty + 8 * i, kEpiWarps * 32);
+            mbar_init(bar_tm_empty + 8 * i, kEpiWarps * CG);   // one arrival per epilogue warp of the pair
         }
         for (int i = 0; i < kStateStages; ++i) {
             mbar_init(bar_st_full + 8 * i, 1);
@@ -311,47 +325,66 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         }
         mbar_fence_init();
     }
-    if (warp == 2) tmem_alloc(s_tmem_ptr, kTmemCols);
+    if (warp == 2) {
+        if constexpr (CG == 2) tmem_alloc_cg2(s_tmem_ptr, kTmemCols);
+        else tmem_alloc(s_tmem_ptr, kTmemCols);
+    }
     tc_fence_before();
-    __syncthreads();
+    if constexpr (CG == 2) cluster_sync_all();   // the peer's barriers exist before any remote signal
+    else __syncthreads();
     tc_fence_after();
     uint32_t tmem_base;
     asm volatile("ld.shared.b32 %0, [%1];\n" : "=r"(tmem_base) : "r"(s_tmem_ptr));
 
-    const int first_tile = blockIdx.x, tile_step = gridDim.x;
+    const int first_tile = blockIdx.x / CG, tile_step = gridDim.x / CG;
 
     if (warp == 0) {
         // ================= operand producer (Alg. 1 lines 3-5: stream dY_k,i and X_k,j) ==========
         if (lane == 0) {
             uint32_t it = 0;  // running k-block counter over all tiles of this CTA
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step) {
-                const TileCoord tc = decode_tile(P, tile);
+                const TileCoord tc = decode_tile<CG>(P, tile, rank);
                 const ProblemDesc &pd = P.prob[tc.p];
                 const int num_kb = (pd.T + kBlockK - 1) / kBlockK;
                 for (int kb = 0; kb < num_kb; ++kb, ++it) {
                     const uint32_t s = it % kStages, ph = (it / kStages) & 1u;
                     mbar_wait(bar_ml_empty + 8 * s, ph ^ 1u);
-                    const uint32_t full = bar_ml_full + 8 * s;
-                    mbar_expect_tx(full, Cfg::ML_STAGE);
                     const uint32_t a = sML + s * Cfg::ML_STAGE, b = a + Cfg::A_STAGE;
+                    if constexpr (CG == 1) {
+                        const uint32_t full = bar_ml_full + 8 * s;
+                        mbar_expect_tx(full, Cfg::ML_STAGE);
 #pragma unroll
-                    for (int i = 0; i < BLOCK_M / 64; ++i)
-                        tma_load_2d(a + i * kBlockK * 128, &pd.map_dY, full, tc.tm * BLOCK_M + i * 64,
-                                    kb * kBlockK, kEvictLast);
+                        for (int i = 0; i < BLOCK_M / 64; ++i)
+                            tma_load_2d(a + i * kBlockK * 128, &pd.map_dY, full, tc.tm * BLOCK_M + i * 64,
+                                        kb * kBlockK, kEvictLast);
 #pragma unroll
-                    for (int i = 0; i < BLOCK_N / 64; ++i)
-                        tma_load_2d(b + i * kBlockK * 128, &pd.map_X, full, tc.tn * BLOCK_N + i * 64,
-                                    kb * kBlockK, kEvictLast);
+                        for (int i = 0; i < BLOCK_N / 64; ++i)
+                            tma_load_2d(b + i * kBlockK * 128, &pd.map_X, full, tc.tn * BLOCK_N + i * 64,
+                                        kb * kBlockK, kEvictLast);
+                    } else {
+                        // both CTAs' bytes are counted on the LEADER's full barrier
+                        if (rank == 0) mbar_expect_tx(bar_ml_full + 8 * s, 2 * Cfg::ML_STAGE);
+                        const uint32_t full = mapa_shared(bar_ml_full + 8 * s, 0);
+#pragma unroll
+                        for (int i = 0; i < BLOCK_M / 64; ++i)
+                            tma_load_2d_cg2(a + i * kBlockK * 128, &pd.map_dY, full, tc.tm * BLOCK_M + i * 64,
+                                            kb * kBlockK, kEvictLast);
+#pragma unroll
+                        for (int i = 0; i < BLOCK_N / 128; ++i)   // this CTA's half of the 256 columns
+                            tma_load_2d_cg2(b + i * kBlockK * 128, &pd.map_X, full,
+                                            tc.tn * BLOCK_N + static_cast<int>(rank) * (BLOCK_N / 2) + i * 64,
+                                            kb * kBlockK, kEvictLast);
+                    }
                 }
             }
         }
     } else if (warp == 1) {
         // ================= MMA issuer (Alg. 1 line 4: G_ij += dY_k,i^T X_k,j) =====================
-        if (lane == 0) {
-            constexpr uint32_t idesc = make_idesc_bf16_f32_mnmn(BLOCK_M, BLOCK_N);
+        if (lane == 0 && rank == 0) {
+            constexpr uint32_t idesc = make_idesc_bf16_f32_mnmn(BLOCK_M * CG, BLOCK_N);
             uint32_t it = 0, titer = 0;
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step, ++titer) {
-                const TileCoord tc = decode_tile(P, tile);
+                const TileCoord tc = decode_tile<CG>(P, tile, rank);
                 const int num_kb = (P.prob[tc.p].T + kBlockK - 1) / kBlockK;
                 const uint32_t as = titer & 1u, aph = (titer >> 1) & 1u;
                 mbar_wait(bar_tm_empty + 8 * as, aph ^ 1u);   // epilogue has drained this buffer
@@ -367,11 +400,16 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                         // 16 tokens further = 16 rows of 128 B inside every 64-wide MN block
                         const uint64_t ad = make_smem_desc_mn_sw128(a + k * 2048, kBlockK * 128, 1024);
                         const uint64_t bd = make_smem_desc_mn_sw128(b + k * 2048, kBlockK * 128, 1024);
-                        umma_bf16(tmem_d, ad, bd, idesc, (kb | k) != 0 ? 1u : 0u);
+                        if constexpr (CG == 2) umma_bf16_cg2(tmem_d, ad, bd, idesc, (kb | k) != 0 ? 1u : 0u);
+                        else umma_bf16(tmem_d, ad, bd, idesc, (kb | k) != 0 ? 1u : 0u);
                     }
-                    umma_commit(bar_ml_empty + 8 * s);        // smem slot free once these MMAs retire
+                    // smem slot free (in both CTAs of a pair) once these MMAs retire
+                    if constexpr (CG == 2) umma_commit_cg2(bar_ml_empty + 8 * s, 3);
+                    else umma_commit(bar_ml_empty + 8 * s);
                 }
-                umma_commit(bar_tm_full + 8 * as);            // G_ij complete (all of T, exactly once)
+                // G_ij complete (all of T, exactly once) -- signalled to each CTA's epilogue
+                if constexpr (CG == 2) umma_commit_cg2(bar_tm_full + 8 * as, 3);
+                else umma_commit(bar_tm_full + 8 * as);
             }
         }
     } else if (warp == 2) {
@@ -379,7 +417,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         if (MODE == MODE_ADAMW && lane == 0) {
             uint32_t ci = 0;  // running chunk counter
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step) {
-                const TileCoord tc = decode_tile(P, tile);
+                const TileCoord tc = decode_tile<CG>(P, tile, rank);
                 const ProblemDesc &pd = P.prob[tc.p];
                 for (int c = 0; c < CHUNKS; ++c, ++ci) {
                     const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
@@ -399,7 +437,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         if (lane == 0) {
             uint32_t ci = 0;
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step) {
-                const TileCoord tc = decode_tile(P, tile);
+                const TileCoord tc = decode_tile<CG>(P, tile, rank);
                 const ProblemDesc &pd = P.prob[tc.p];
                 for (int c = 0; c < CHUNKS; ++c, ++ci) {
                     const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
@@ -454,19 +492,27 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                     mbar_arrive(bar_st_done + 8 * s);
                 }
             } else {
-                epi_tile_int8<Cfg, kStateStages>(P, hp, tile, titer, taddr, sST, bar_st_full,
+                epi_tile_int8<Cfg, kStateStages, CG>(P, hp, tile, rank, titer, taddr, sST, bar_st_full,
                                                  bar_st_done, row, wg, s_xchg);
             }
+            // this warp has drained the accumulator: tell the (leader's) MMA issuer
             tc_fence_before();
-            mbar_arrive(bar_tm_empty + 8 * as);
+            __syncwarp();
+            if (lane == 0) {
+                if constexpr (CG == 2) mbar_arrive_cluster(mapa_shared(bar_tm_empty + 8 * as, 0));
+                else mbar_arrive(bar_tm_empty + 8 * as);
+            }
         }
     }
 
+    __syncwarp();                                // lanes 1-31 of the single-thread roles rejoin lane 0
     tc_fence_before();
-    __syncthreads();
+    if constexpr (CG == 2) cluster_sync_all();   // the peer may still read this CTA's smem / signal its barriers
+    else __syncthreads();
     if (warp == 2) {
         tc_fence_after();
-        tmem_dealloc(tmem_base, kTmemCols);
+        if constexpr (CG == 2) tmem_dealloc_cg2(tmem_base, kTmemCols);
+        else tmem_dealloc(tmem_base, kTmemCols);
     }
 }
 
