@@ -255,7 +255,7 @@ def run_cuda(args):
     import torch
     import torch.distributed as dist
     from paper_2606_22932_b200 import binding as fb
-    from paper_2606_22932_b200 import synth
+    from paper_2606_22932_b200 import shard, synth
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -298,10 +298,7 @@ def run_cuda(args):
     launches = fb.forge_launch_count() - launches0
     total_ms = evs[0].elapsed_time(evs[-1])
     per_launch_ms = sorted(evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps))
-    t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = shard.max_over_ranks(total_ms, device=dev)
     ms_per_step = total_ms / args.steps
     us_per_layer = ms_per_step * 1e3 / world       # layers processed by all ranks per step = world
 
