@@ -37,22 +37,33 @@ NCU_TRAFFIC_BYTES = {"fp32": 4530391000, "bf16": None, "int8": None}
 
 
 def measured_peaks():
+    """(HBM GB/s, bf16 TF/s burst, bf16 TF/s sustained, source)."""
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
         with open(path) as f:
             d = json.load(f)
-        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
-    return 6650.0, "fallback (B200_PROFILING.md)"
+        return (float(d["hbm_gbs"]), float(d["bf16_tflops"]), float(d.get("bf16_tflops_sustained", d["bf16_tflops"])),
+                "measured (MEASURED_PEAKS.json)")
+    return 6650.0, 1590.0, 1400.0, "fallback (B200_PROFILING.md)"
 
 
-def layer_counts():
+def workload_shapes(workload: str):
+    """configs[1]/[2]: the whole layer (default, the headline); configs[3]: gate_proj alone."""
     from paper_2606_22932_b200 import synth
-    params = sum(o * i for _, o, i in synth.LLAMA8B_LAYER)
+    if workload == "layer":
+        return synth.LLAMA8B_LAYER
+    return tuple(s for s in synth.LLAMA8B_LAYER if s[0] == workload)
+
+
+def layer_counts(workload: str = "layer", tokens: int = T_TOKENS):
+    from paper_2606_22932_b200 import synth
+    shapes = workload_shapes(workload)
+    params = sum(o * i for _, o, i in shapes)
     xs = {}
-    for name, o, i in synth.LLAMA8B_LAYER:
+    for name, o, i in shapes:
         xs[(synth.X_GROUP[name], i)] = i
-    in_bytes = 2 * T_TOKENS * (sum(xs.values()) + sum(o for _, o, _ in synth.LLAMA8B_LAYER))
-    flops = 2 * params * T_TOKENS
+    in_bytes = 2 * tokens * (sum(xs.values()) + sum(o for _, o, _ in shapes))
+    flops = 2 * params * tokens
     return params, in_bytes, flops
 
 
@@ -99,11 +110,11 @@ class ClockSampler(threading.Thread):
 # ------------------------------------------------------------------------------------------------
 # workload construction (synthetic, seeded; shapes of BASELINE.json configs[1] / [2])
 # ------------------------------------------------------------------------------------------------
-def make_device_layer(moments: str, seed: int, device):
-    """One Llama-3.1-8B layer's 7 problems on the device (inputs resident in HBM)."""
+def make_device_layer(moments: str, seed: int, device, workload: str = "layer", tokens: int = T_TOKENS):
+    """One Llama-3.1-8B layer's 7 problems (or one projection of it) on the device (inputs resident in HBM)."""
     import torch
     from paper_2606_22932_b200 import synth
-    probs = synth.make_layer(T_TOKENS, seed, device=device)
+    probs = synth.make_layer(tokens, seed, shapes=workload_shapes(workload), device=device)
     out = []
     for p in probs:
         d = dict(X=p.X, dY=p.dY, W=p.W)
@@ -269,7 +280,7 @@ def run_cuda(args):
     fb.lib()                                       # fails loudly if the CUDA library is missing
     hp = synth.HP_DEFAULT
     mdt = MOMENT_ENUM[args.moments]
-    layer = make_device_layer(args.moments, 20260622 + 1 + rank, dev)
+    layer = make_device_layer(args.moments, 20260622 + 1 + rank, dev, args.workload, args.tokens)
     arr = fb.make_problem_array(layer)
     hpt = (hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
     stream = torch.cuda.current_stream()
@@ -302,30 +313,42 @@ def run_cuda(args):
     ms_per_step = total_ms / args.steps
     us_per_layer = ms_per_step * 1e3 / world       # layers processed by all ranks per step = world
 
-    params, in_bytes, flops = layer_counts()
+    params, in_bytes, flops = layer_counts(args.workload, args.tokens)
     alg_bytes = params * MOMENT_BYTES[args.moments] + in_bytes
-    peak, peak_src = measured_peaks()
+    hbm_peak, tf_burst, tf_sustained, peak_src = measured_peaks()
     kernel_ms = (evs[0].elapsed_time(evs[-1])) / args.steps       # this rank's average launch duration
-    achieved = alg_bytes / (kernel_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES[args.moments], "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": alg_bytes, "launch_us_avg": kernel_ms * 1e3,
-                "launch_us_median": per_launch_ms[len(per_launch_ms) // 2] * 1e3,
-                "tflops": flops / (kernel_ms * 1e-3) / 1e12,
-                "frac_of_datasheet_8TBs": achieved / 8000.0}
+    gbs = alg_bytes / (kernel_ms * 1e-3) / 1e9
+    tfs = flops / (kernel_ms * 1e-3) / 1e12
+    # per-shape roofline max(flops / P_bf16, bytes / B_HBM) (north_star); the kernel runs inside a long
+    # back-to-back loop, so the tensor term uses the SUSTAINED cuBLAS figure (B200_PROFILING.md)
+    t_hbm_us, t_tensor_us = alg_bytes / hbm_peak / 1e3, flops / tf_sustained / 1e6
+    if t_hbm_us >= t_tensor_us:
+        roofline = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak}
+    else:
+        roofline = {"bound": "tensor", "achieved": tfs, "peak": tf_sustained, "unit": "TFLOP/s", "frac": tfs / tf_sustained,
+                    "frac_of_burst_peak": tfs / tf_burst, "burst_peak": tf_burst}
+    is_headline = args.workload == "layer" and args.tokens == T_TOKENS
+    roofline.update({"traffic": NCU_TRAFFIC_BYTES[args.moments] if is_headline else None, "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": alg_bytes, "flops_per_launch": flops,
+                     "roofline_us": max(t_hbm_us, t_tensor_us), "hbm_term_us": t_hbm_us, "tensor_term_us": t_tensor_us,
+                     "launch_us_avg": kernel_ms * 1e3,
+                     "launch_us_median": per_launch_ms[len(per_launch_ms) // 2] * 1e3,
+                     "gbs": gbs, "tflops": tfs, "frac_of_datasheet_8TBs": gbs / 8000.0,
+                     "frac_of_datasheet_2250TF": tfs / 2250.0})
 
     line = {"metric": METRIC, "value": us_per_layer, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": "configs[1]: Llama-3.1-8B layer, 7 projections in one grouped launch, T=512"
-                                   if args.moments == "fp32" else f"configs[2]: same layer, {args.moments} moments",
-                       "moments": args.moments, "params_per_layer": params, "tokens": T_TOKENS,
+            "config": {"workload": (("configs[1]: Llama-3.1-8B layer, 7 projections in one grouped launch, T=512"
+                                     if args.moments == "fp32" else f"configs[2]: same layer, {args.moments} moments")
+                                    if is_headline else f"configs[3]-style: {args.workload} of a Llama-3.1-8B layer, T={args.tokens}, {args.moments} moments"),
+                       "moments": args.moments, "params_per_layer": params, "tokens": args.tokens,
                        "l2": "working set 4.4 GB/layer >> 126 MB L2, no flush needed",
                        "parallelism": f"replicated layers x{world}, no collective"},
             "roofline": roofline, "gpu_launches": int(launches), "clocks": sampler.result(),
             "dw_bytes_allocated": 0, "library_workspace_bytes": fb.forge_workspace_bytes()}
 
-    if rank == 0 and not args.no_extras:
+    if rank == 0 and not args.no_extras and is_headline:
         # ---- end to end through the C ABI with HOST buffers (H2D + kernel + D2H inside the call)
         host = make_host_layer(args.moments, 20260622 + 1)
         h2d = sum(sum(v.numel() * v.element_size() for v in d.values()) for d in host)
@@ -360,6 +383,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--moments", choices=["fp32", "bf16", "int8"], default="fp32")
     ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
+    ap.add_argument("--workload", choices=["layer", "q", "k", "v", "o", "gate", "up", "down"], default="layer",
+                    help="layer = BASELINE.json configs[1] (the metric); a projection name = that problem alone (configs[3])")
+    ap.add_argument("--tokens", type=int, default=T_TOKENS, help="T (configs[3] sweeps 512/2048/8192 on gate)")
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, same-GPU baselines and the CPU oracle leg")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)

@@ -195,6 +195,8 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
         tiles += ((p.out + BLOCK_M * CG - 1) / (BLOCK_M * CG)) * d.tiles_n;   // (128*CG) x 256 work units
     }
     P.total_tiles = tiles;
+    P.pf_chunks = env_int("FORGE_PF", 0);
+    P.debug = env_int("FORGE_ABLATE", 0);          // profiling ablations only (profiles/): results are wrong when set
     int grid = dev.sm_count / CG;                  // persistent: one CTA (or CTA pair) per SM (pair)
     const int forced = env_int("FORGE_GRID", 0);   // debug/determinism tests only
     if (forced > 0) grid = (forced + CG - 1) / CG;

@@ -63,7 +63,11 @@ struct alignas(64) KernelParams {
     AdamWScalars hp;
     int32_t num_problems;
     int32_t total_tiles;
+    int32_t pf_chunks;   // state chunks prefetched into L2 ahead of the shared-memory ring
+    int32_t debug;       // ablation switches for profiling ONLY (results are wrong when set):
+                         // 1 = no operand loads / MMA, 2 = no state loads / stores, 4 = no epilogue math
 };
+enum : int { DBG_NO_MAINLOOP = 1, DBG_NO_STATE = 2, DBG_NO_EPILOGUE = 4 };
 
 // CG = 1: one CTA per 128x256 tile.  CG = 2: a CTA pair (cluster of 2, tcgen05 cta_group::2) shares
 // a 256x256 tile: each CTA stages its own 128 rows of A = dY^T and only HALF of B = X (128 of the
@@ -340,7 +344,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
 
     if (warp == 0) {
         // ================= operand producer (Alg. 1 lines 3-5: stream dY_k,i and X_k,j) ==========
-        if (lane == 0) {
+        if (lane == 0 && !(P.debug & DBG_NO_MAINLOOP)) {
             uint32_t it = 0;  // running k-block counter over all tiles of this CTA
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step) {
                 const TileCoord tc = decode_tile<CG>(P, tile, rank);
@@ -380,7 +384,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         }
     } else if (warp == 1) {
         // ================= MMA issuer (Alg. 1 line 4: G_ij += dY_k,i^T X_k,j) =====================
-        if (lane == 0 && rank == 0) {
+        if (lane == 0 && rank == 0 && !(P.debug & DBG_NO_MAINLOOP)) {
             constexpr uint32_t idesc = make_idesc_bf16_f32_mnmn(BLOCK_M * CG, BLOCK_N);
             uint32_t it = 0, titer = 0;
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step, ++titer) {
@@ -414,12 +418,41 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         }
     } else if (warp == 2) {
         // ================= state loader (Alg. 1 line 6: load W_ij, m_ij, v_ij) ===================
-        if (MODE == MODE_ADAMW && lane == 0) {
+        if (MODE == MODE_ADAMW && lane == 0 && !(P.debug & DBG_NO_STATE)) {
+            // The ring holds only kStateStages chunks, and a slot stays busy through load latency,
+            // epilogue and store read; an L2 prefetch cursor runs pf_chunks further ahead so that
+            // the DRAM requests in flight are not bounded by shared memory (126 MB of L2 absorb it).
+            int pf_tile = first_tile, pf_c = 0;
+            TileCoord pf_tc = decode_tile<CG>(P, pf_tile < P.total_tiles ? pf_tile : first_tile, rank);
+            auto prefetch_next = [&]() {
+                if (pf_tile >= P.total_tiles) return;
+                const ProblemDesc &pd = P.prob[pf_tc.p];
+                const int x = pf_tc.tn * BLOCK_N + pf_c * CHUNK_N, y = pf_tc.tm * BLOCK_M;
+                tma_prefetch_l2_2d(&pd.map_W, x, y);
+                tma_prefetch_l2_2d(&pd.map_m, x, y);
+                tma_prefetch_l2_2d(&pd.map_v, x, y);
+                if (++pf_c == CHUNKS) {
+                    pf_c = 0;
+                    pf_tile += tile_step;
+                    if (pf_tile < P.total_tiles) pf_tc = decode_tile<CG>(P, pf_tile, rank);
+                }
+            };
+            for (int i = 0; i < P.pf_chunks + kStateStages; ++i) {
+                if (i >= kStateStages) prefetch_next();
+                else if (P.pf_chunks > 0) {   // the first ring fill is loaded directly: skip, do not prefetch
+                    if (++pf_c == CHUNKS) {
+                        pf_c = 0;
+                        pf_tile += tile_step;
+                        if (pf_tile < P.total_tiles) pf_tc = decode_tile<CG>(P, pf_tile, rank);
+                    }
+                }
+            }
             uint32_t ci = 0;  // running chunk counter
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step) {
                 const TileCoord tc = decode_tile<CG>(P, tile, rank);
                 const ProblemDesc &pd = P.prob[tc.p];
                 for (int c = 0; c < CHUNKS; ++c, ++ci) {
+                    if (P.pf_chunks > 0) prefetch_next();
                     const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
                     mbar_wait(bar_st_empty + 8 * s, ph ^ 1u);
                     const uint32_t full = bar_st_full + 8 * s;
@@ -435,16 +468,27 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
     } else if (warp == 3) {
         // ================= state storer (Alg. 1 line 11: store W_ij, m_ij, v_ij) ================
         if (lane == 0) {
+            // One store group may stay in flight while the next chunk is stored (look-ahead 1): the
+            // ~0.8 us a TMA store needs before its shared-memory source is reusable is then hidden
+            // behind the next chunk instead of serialising the ring.  A slot is released as soon as
+            // its own group has been read; if no further chunk is ready the storer drains at once.
             uint32_t ci = 0;
+            int held = -1;                                 // slot whose store group is still unreleased
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step) {
                 const TileCoord tc = decode_tile<CG>(P, tile, rank);
                 const ProblemDesc &pd = P.prob[tc.p];
                 for (int c = 0; c < CHUNKS; ++c, ++ci) {
                     const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
+                    if (held >= 0 && !mbar_test_wait(bar_st_done + 8 * s, ph)) {
+                        tma_store_wait_read<0>();
+                        mbar_arrive(bar_st_empty + 8 * held);
+                        held = -1;
+                    }
                     mbar_wait(bar_st_done + 8 * s, ph);
                     const uint32_t base = sST + s * Cfg::ST_STAGE;
                     const int x = tc.tn * BLOCK_N + c * CHUNK_N, y = tc.tm * BLOCK_M;
-                    if constexpr (MODE == MODE_ADAMW) {
+                    if (P.debug & DBG_NO_STATE) {
+                    } else if constexpr (MODE == MODE_ADAMW) {
                         tma_store_2d(&pd.map_W, base, x, y, kEvictFirst);
                         tma_store_2d(&pd.map_m, base + Cfg::W_CHUNK, x, y, kEvictFirst);
                         tma_store_2d(&pd.map_v, base + Cfg::W_CHUNK + Cfg::M_CHUNK, x, y, kEvictFirst);
@@ -452,11 +496,15 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                         tma_store_2d(&pd.map_m, base + Cfg::W_CHUNK, x, y, kEvictFirst);
                     }
                     tma_store_commit();
-                    tma_store_wait_read<0>();                 // smem has been read: slot reusable
-                    mbar_arrive(bar_st_empty + 8 * s);
+                    if (held >= 0) {
+                        tma_store_wait_read<1>();             // the previous group's source has been read
+                        mbar_arrive(bar_st_empty + 8 * held);
+                    }
+                    held = static_cast<int>(s);
                 }
             }
             tma_store_wait_all<0>();
+            if (held >= 0) mbar_arrive(bar_st_empty + 8 * held);
         }
     } else {
         // ================= epilogue warpgroups (Alg. 1 lines 7-10 on the TMEM tile) ==============
@@ -468,7 +516,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         uint32_t titer = 0;
         for (int tile = first_tile; tile < P.total_tiles; tile += tile_step, ++titer) {
             const uint32_t as = titer & 1u, aph = (titer >> 1) & 1u;
-            mbar_wait(bar_tm_full + 8 * as, aph);
+            if (!(P.debug & DBG_NO_MAINLOOP)) mbar_wait(bar_tm_full + 8 * as, aph);
             tc_fence_after();
             const uint32_t taddr = tmem_base + ((quad * 32u) << 16) + as * BLOCK_N;
             if constexpr (MDT != MDT_INT8) {
@@ -479,10 +527,12 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                     tmem_ld_32x32b_x32(taddr + c * CHUNK_N, g);
                     const uint32_t base = sST + s * Cfg::ST_STAGE;
                     if constexpr (MODE == MODE_ADAMW) {
-                        mbar_wait(bar_st_full + 8 * s, ph);
+                        if (!(P.debug & DBG_NO_STATE)) mbar_wait(bar_st_full + 8 * s, ph);
+                        else mbar_wait(bar_st_empty + 8 * s, ph ^ 1u);
                         tmem_ld_wait();
-                        epi_chunk_fp<MDT>(hp, g, base, base + Cfg::W_CHUNK,
-                                          base + Cfg::W_CHUNK + Cfg::M_CHUNK, row);
+                        if (!(P.debug & DBG_NO_EPILOGUE))
+                            epi_chunk_fp<MDT>(hp, g, base, base + Cfg::W_CHUNK,
+                                              base + Cfg::W_CHUNK + Cfg::M_CHUNK, row);
                     } else {
                         mbar_wait(bar_st_empty + 8 * s, ph ^ 1u);
                         tmem_ld_wait();
