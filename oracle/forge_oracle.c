@@ -187,9 +187,10 @@ void forge_oracle_adamw_bf16(uint16_t *W, uint16_t *m, uint16_t *v, const double
 #define FORGE_ORACLE_QBLOCK 256   /* BASELINE.json: 256-element blocks along `in` (reading S4) */
 
 /* App. B: per-block absmax a, scale s = a/127, q(x) = s*round(x/s).
- * The decision that produces an integer code is taken in fp32, the kernel's precision:
- *   xf = fp32(x);  a = max|xf|;  code = rint(xf * (127/a)) with the quotient and the product
- *   each rounded to fp32, ties to even (S7), clamped to [-127,127].
+ * The decision that produces an integer code is taken in the kernel's precision (S7):
+ *   xf = fp32(x);  a = max|xf|;  inv = fp32(127/a);  code = rint(xf * inv), where the product of the
+ *   two fp32 values is EXACT (it fits a double) and is rounded once, to the nearest integer, ties
+ *   to even; clamped to [-127,127].
  * An all-zero block stores a = 0 and codes 0. */
 void forge_oracle_quant_m_block(const double *x, int n, int8_t *code, float *scale)
 {
@@ -199,10 +200,9 @@ void forge_oracle_quant_m_block(const double *x, int n, int8_t *code, float *sca
     if (!(a > 0.0f)) { for (int i = 0; i < n; ++i) code[i] = 0; return; }
     volatile float inv = 127.0f / a;
     for (int i = 0; i < n; ++i) {
-        volatile float y = (float)x[i] * inv;
-        float r = rintf(y);
-        if (r > 127.0f) r = 127.0f;
-        if (r < -127.0f) r = -127.0f;
+        double r = rint((double)(float)x[i] * (double)inv);
+        if (r > 127.0) r = 127.0;
+        if (r < -127.0) r = -127.0;
         code[i] = (int8_t)r;
     }
 }
@@ -217,10 +217,9 @@ void forge_oracle_quant_v_block(const double *x, int n, uint8_t *code, float *sc
     if (!(a > 0.0f)) { for (int i = 0; i < n; ++i) code[i] = 0; return; }
     volatile float inv = 255.0f / a;
     for (int i = 0; i < n; ++i) {
-        volatile float y = (float)x[i] * inv;
-        float r = rintf(y);
-        if (r > 255.0f) r = 255.0f;
-        if (r < 1.0f) r = 1.0f;
+        double r = rint((double)(float)x[i] * (double)inv);
+        if (r > 255.0) r = 255.0;
+        if (r < 1.0) r = 1.0;
         code[i] = (uint8_t)r;
     }
 }

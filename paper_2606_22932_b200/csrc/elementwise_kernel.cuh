@@ -29,77 +29,75 @@ forge_adamw_from_g_kernel(const float *__restrict__ G, uint16_t *__restrict__ W,
     const size_t group = (static_cast<size_t>(blockIdx.x) * blockDim.x + threadIdx.x);
     const size_t base = group * 8;
     const bool active = base < n_elems;      // n_elems % 8 == 0
-    float g[8], w[8], m[8], v[8];
-    float a_m_old = 0.f, a_v_old = 0.f;
+    f32x2 g[4], w[4], m[4], v[4];           // 8 consecutive elements as 4 coordinate pairs
     if (active) {
-        const float4 g0 = *reinterpret_cast<const float4 *>(G + base), g1 = *reinterpret_cast<const float4 *>(G + base + 4);
-        g[0] = g0.x; g[1] = g0.y; g[2] = g0.z; g[3] = g0.w; g[4] = g1.x; g[5] = g1.y; g[6] = g1.z; g[7] = g1.w;
+        const uint4 g0 = *reinterpret_cast<const uint4 *>(G + base), g1 = *reinterpret_cast<const uint4 *>(G + base + 4);
+        g[0] = pk2u(g0.x, g0.y); g[1] = pk2u(g0.z, g0.w); g[2] = pk2u(g1.x, g1.y); g[3] = pk2u(g1.z, g1.w);
         const uint4 wq = *reinterpret_cast<const uint4 *>(W + base);
-        w[0] = bf16lo(wq.x); w[1] = bf16hi(wq.x); w[2] = bf16lo(wq.y); w[3] = bf16hi(wq.y);
-        w[4] = bf16lo(wq.z); w[5] = bf16hi(wq.z); w[6] = bf16lo(wq.w); w[7] = bf16hi(wq.w);
+        w[0] = bf16x2_to_f32x2(wq.x); w[1] = bf16x2_to_f32x2(wq.y); w[2] = bf16x2_to_f32x2(wq.z); w[3] = bf16x2_to_f32x2(wq.w);
         if constexpr (MDT == MDT_FP32) {
             const float *mf = static_cast<const float *>(mp), *vf = static_cast<const float *>(vp);
-            const float4 a = *reinterpret_cast<const float4 *>(mf + base), b = *reinterpret_cast<const float4 *>(mf + base + 4);
-            const float4 c = *reinterpret_cast<const float4 *>(vf + base), d = *reinterpret_cast<const float4 *>(vf + base + 4);
-            m[0] = a.x; m[1] = a.y; m[2] = a.z; m[3] = a.w; m[4] = b.x; m[5] = b.y; m[6] = b.z; m[7] = b.w;
-            v[0] = c.x; v[1] = c.y; v[2] = c.z; v[3] = c.w; v[4] = d.x; v[5] = d.y; v[6] = d.z; v[7] = d.w;
+            const uint4 a = *reinterpret_cast<const uint4 *>(mf + base), b = *reinterpret_cast<const uint4 *>(mf + base + 4);
+            const uint4 c = *reinterpret_cast<const uint4 *>(vf + base), d = *reinterpret_cast<const uint4 *>(vf + base + 4);
+            m[0] = pk2u(a.x, a.y); m[1] = pk2u(a.z, a.w); m[2] = pk2u(b.x, b.y); m[3] = pk2u(b.z, b.w);
+            v[0] = pk2u(c.x, c.y); v[1] = pk2u(c.z, c.w); v[2] = pk2u(d.x, d.y); v[3] = pk2u(d.z, d.w);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) adamw_update2(hp, g[e], w[e], m[e], v[e]);
+            float *mo = static_cast<float *>(mp), *vo = static_cast<float *>(vp);
+            *reinterpret_cast<uint4 *>(mo + base) = make_uint4(lo2u(m[0]), hi2u(m[0]), lo2u(m[1]), hi2u(m[1]));
+            *reinterpret_cast<uint4 *>(mo + base + 4) = make_uint4(lo2u(m[2]), hi2u(m[2]), lo2u(m[3]), hi2u(m[3]));
+            *reinterpret_cast<uint4 *>(vo + base) = make_uint4(lo2u(v[0]), hi2u(v[0]), lo2u(v[1]), hi2u(v[1]));
+            *reinterpret_cast<uint4 *>(vo + base + 4) = make_uint4(lo2u(v[2]), hi2u(v[2]), lo2u(v[3]), hi2u(v[3]));
         } else if constexpr (MDT == MDT_BF16) {
             const uint4 a = *reinterpret_cast<const uint4 *>(static_cast<const uint16_t *>(mp) + base);
             const uint4 c = *reinterpret_cast<const uint4 *>(static_cast<const uint16_t *>(vp) + base);
-            m[0] = bf16lo(a.x); m[1] = bf16hi(a.x); m[2] = bf16lo(a.y); m[3] = bf16hi(a.y);
-            m[4] = bf16lo(a.z); m[5] = bf16hi(a.z); m[6] = bf16lo(a.w); m[7] = bf16hi(a.w);
-            v[0] = bf16lo(c.x); v[1] = bf16hi(c.x); v[2] = bf16lo(c.y); v[3] = bf16hi(c.y);
-            v[4] = bf16lo(c.z); v[5] = bf16hi(c.z); v[6] = bf16lo(c.w); v[7] = bf16hi(c.w);
+            m[0] = bf16x2_to_f32x2(a.x); m[1] = bf16x2_to_f32x2(a.y); m[2] = bf16x2_to_f32x2(a.z); m[3] = bf16x2_to_f32x2(a.w);
+            v[0] = bf16x2_to_f32x2(c.x); v[1] = bf16x2_to_f32x2(c.y); v[2] = bf16x2_to_f32x2(c.z); v[3] = bf16x2_to_f32x2(c.w);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) adamw_update2(hp, g[e], w[e], m[e], v[e]);
+            *reinterpret_cast<uint4 *>(static_cast<uint16_t *>(mp) + base) =
+                make_uint4(f32x2_to_bf16x2(m[0]), f32x2_to_bf16x2(m[1]), f32x2_to_bf16x2(m[2]), f32x2_to_bf16x2(m[3]));
+            *reinterpret_cast<uint4 *>(static_cast<uint16_t *>(vp) + base) =
+                make_uint4(f32x2_to_bf16x2(v[0]), f32x2_to_bf16x2(v[1]), f32x2_to_bf16x2(v[2]), f32x2_to_bf16x2(v[3]));
         } else {
-            a_m_old = m_scale[base / 256];
-            a_v_old = v_scale[base / 256];
-            const float dm = dequant_step(a_m_old, 127.0f), dv = dequant_step(a_v_old, 255.0f);
+            const float bm = __fmul_rn(hp.beta1, dequant_step(m_scale[base / 256], 127.0f));
+            const float bv = __fmul_rn(hp.beta2, dequant_step(v_scale[base / 256], 255.0f));
             const uint2 a = *reinterpret_cast<const uint2 *>(static_cast<const uint8_t *>(mp) + base);
             const uint2 c = *reinterpret_cast<const uint2 *>(static_cast<const uint8_t *>(vp) + base);
-            const uint32_t aw[2] = {a.x, a.y}, cw[2] = {c.x, c.y};
+            f32x2 cm[4], cv[4];
+            codes4_to_f32(a.x, true, cm[0], cm[1]);
+            codes4_to_f32(a.y, true, cm[2], cm[3]);
+            codes4_to_f32(c.x, false, cv[0], cv[1]);
+            codes4_to_f32(c.y, false, cv[2], cv[3]);
 #pragma unroll
-            for (int e = 0; e < 8; ++e) {
-                const int mc = static_cast<int>(static_cast<int8_t>((aw[e >> 2] >> (8 * (e & 3))) & 0xFFu));
-                const int vc = static_cast<int>((cw[e >> 2] >> (8 * (e & 3))) & 0xFFu);
-                m[e] = __fmul_rn(static_cast<float>(mc), dm);
-                v[e] = __fmul_rn(static_cast<float>(vc), dv);
+            for (int e = 0; e < 4; ++e) {
+                adamw_moments2_q(hp, g[e], cm[e], cv[e], bm, bv, m[e], v[e]);
+                adamw_weight2(hp, m[e], v[e], w[e]);
             }
         }
-#pragma unroll
-        for (int e = 0; e < 8; ++e) adamw_update(hp, g[e], w[e], m[e], v[e]);
-        *reinterpret_cast<uint4 *>(W + base) = make_uint4(pack_bf16(w[0], w[1]), pack_bf16(w[2], w[3]),
-                                                          pack_bf16(w[4], w[5]), pack_bf16(w[6], w[7]));
-        if constexpr (MDT == MDT_FP32) {
-            float *mf = static_cast<float *>(mp), *vf = static_cast<float *>(vp);
-            *reinterpret_cast<float4 *>(mf + base) = make_float4(m[0], m[1], m[2], m[3]);
-            *reinterpret_cast<float4 *>(mf + base + 4) = make_float4(m[4], m[5], m[6], m[7]);
-            *reinterpret_cast<float4 *>(vf + base) = make_float4(v[0], v[1], v[2], v[3]);
-            *reinterpret_cast<float4 *>(vf + base + 4) = make_float4(v[4], v[5], v[6], v[7]);
-        } else if constexpr (MDT == MDT_BF16) {
-            *reinterpret_cast<uint4 *>(static_cast<uint16_t *>(mp) + base) =
-                make_uint4(pack_bf16(m[0], m[1]), pack_bf16(m[2], m[3]), pack_bf16(m[4], m[5]), pack_bf16(m[6], m[7]));
-            *reinterpret_cast<uint4 *>(static_cast<uint16_t *>(vp) + base) =
-                make_uint4(pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]), pack_bf16(v[4], v[5]), pack_bf16(v[6], v[7]));
-        }
+        *reinterpret_cast<uint4 *>(W + base) = make_uint4(f32x2_to_bf16x2(w[0]), f32x2_to_bf16x2(w[1]),
+                                                          f32x2_to_bf16x2(w[2]), f32x2_to_bf16x2(w[3]));
     }
     if constexpr (MDT == MDT_INT8) {
         // n_elems % 256 == 0, so a warp is either fully active or fully idle
         float pm = 0.f, pv = 0.f;
         if (active) {
 #pragma unroll
-            for (int e = 0; e < 8; ++e) { pm = fmaxf(pm, fabsf(m[e])); pv = fmaxf(pv, fabsf(v[e])); }
+            for (int e = 0; e < 4; ++e) {
+                pm = fmaxf(pm, fmaxf(fabsf(lo2(m[e])), fabsf(hi2(m[e]))));
+                pv = fmaxf(pv, fmaxf(lo2(v[e]), hi2(v[e])));
+            }
         }
         const float a_m = warp_max(pm), a_v = warp_max(pv);
         if (active) {
             const float inv_m = quant_inv_scale(a_m, 127.0f), inv_v = quant_inv_scale(a_v, 255.0f);
-            uint32_t mo[2] = {0, 0}, vo[2] = {0, 0};
-#pragma unroll
-            for (int e = 0; e < 8; ++e) {
-                mo[e >> 2] |= (static_cast<uint32_t>(quant_m_code(m[e], inv_m)) & 0xFFu) << (8 * (e & 3));
-                vo[e >> 2] |= (static_cast<uint32_t>(quant_v_code(v[e], inv_v)) & 0xFFu) << (8 * (e & 3));
-            }
-            *reinterpret_cast<uint2 *>(static_cast<uint8_t *>(mp) + base) = make_uint2(mo[0], mo[1]);
-            *reinterpret_cast<uint2 *>(static_cast<uint8_t *>(vp) + base) = make_uint2(vo[0], vo[1]);
+            const float v_floor = quant_v_floor(inv_v);
+            const uint32_t m0 = pack_codes4(quant_m2(m[0], inv_m), quant_m2(m[1], inv_m));
+            const uint32_t m1 = pack_codes4(quant_m2(m[2], inv_m), quant_m2(m[3], inv_m));
+            const uint32_t v0 = pack_codes4(quant_v2(v[0], inv_v, v_floor), quant_v2(v[1], inv_v, v_floor));
+            const uint32_t v1 = pack_codes4(quant_v2(v[2], inv_v, v_floor), quant_v2(v[3], inv_v, v_floor));
+            *reinterpret_cast<uint2 *>(static_cast<uint8_t *>(mp) + base) = make_uint2(m0, m1);
+            *reinterpret_cast<uint2 *>(static_cast<uint8_t *>(vp) + base) = make_uint2(v0, v1);
             if ((threadIdx.x & 31) == 0) {
                 m_scale[base / 256] = a_m;
                 v_scale[base / 256] = a_v;

@@ -147,11 +147,11 @@ int env_int(const char *name, int dflt) {
 // ---------------------------------------------------------------------------------------------
 // launch of one fused-kernel instantiation over <= kMaxProblems problems
 // ---------------------------------------------------------------------------------------------
-template <int MDT, int MODE, int BK, int ST, int SS, int CG = 1>
+template <int MDT, int MODE, int BK, int ST, int SS, int CG = 1, int CM = 64, int CN = 64>
 forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamWScalars &hp,
                             const DeviceInfo &dev, cudaStream_t stream) {
-    using Cfg = KernelCfg<MDT, BK, ST, SS, CG>;
-    auto kernel = forge_fused_kernel<MDT, MODE, BK, ST, SS, CG>;
+    using Cfg = KernelCfg<MDT, BK, ST, SS, CG, CM, CN>;
+    auto kernel = forge_fused_kernel<MDT, MODE, BK, ST, SS, CG, CM, CN>;
     static std::once_flag once;
     static cudaError_t attr_err = cudaSuccess;
     std::call_once(once, [&] {
@@ -174,15 +174,15 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
         ok &= encode_2d(&d.map_dY, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.dY, p.T, p.out, 64, BK, CU_TENSOR_MAP_SWIZZLE_128B);
         ok &= encode_2d(&d.map_X, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.X, p.T, p.in, 64, BK, CU_TENSOR_MAP_SWIZZLE_128B);
         if (MODE == MODE_ADAMW) {
-            ok &= encode_2d(&d.map_W, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.W, p.out, p.in, CHUNK_N, BLOCK_M,
+            ok &= encode_2d(&d.map_W, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.W, p.out, p.in, Cfg::W_BOX_COLS, CM,
                             swizzle_for_row_bytes(Cfg::W_ROW));
-            ok &= encode_2d(&d.map_m, mom_dt, Cfg::kMomBytes, p.m, p.out, p.in, CHUNK_N, BLOCK_M,
+            ok &= encode_2d(&d.map_m, mom_dt, Cfg::kMomBytes, p.m, p.out, p.in, Cfg::M_BOX_COLS, CM,
                             swizzle_for_row_bytes(Cfg::M_ROW));
-            ok &= encode_2d(&d.map_v, mom_dt, Cfg::kMomBytes, p.v, p.out, p.in, CHUNK_N, BLOCK_M,
+            ok &= encode_2d(&d.map_v, mom_dt, Cfg::kMomBytes, p.v, p.out, p.in, Cfg::M_BOX_COLS, CM,
                             swizzle_for_row_bytes(Cfg::M_ROW));
         } else {  // store-G twin: p.m carries the fp32 G output
-            ok &= encode_2d(&d.map_m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, p.m, p.out, p.in, CHUNK_N, BLOCK_M,
-                            CU_TENSOR_MAP_SWIZZLE_128B);
+            ok &= encode_2d(&d.map_m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, p.m, p.out, p.in, Cfg::M_BOX_COLS, CM,
+                            swizzle_for_row_bytes(Cfg::M_ROW));
         }
         if (!ok) return cuda_fail(cudaErrorInvalidValue);
         d.m_scale = p.m_scale;
@@ -195,7 +195,6 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
         tiles += ((p.out + BLOCK_M * CG - 1) / (BLOCK_M * CG)) * d.tiles_n;   // (128*CG) x 256 work units
     }
     P.total_tiles = tiles;
-    P.pf_chunks = env_int("FORGE_PF", 0);
     P.debug = env_int("FORGE_ABLATE", 0);          // profiling ablations only (profiles/): results are wrong when set
     int grid = dev.sm_count / CG;                  // persistent: one CTA (or CTA pair) per SM (pair)
     const int forced = env_int("FORGE_GRID", 0);   // debug/determinism tests only
@@ -222,31 +221,51 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
 
 // Static per-shape configuration table (the paper searches this space with an autotuner,
 // PAPER.md:706-710 App. H; here the choice is fixed per moment dtype and token count):
-//   small T : HBM-bound -> short token chunks, deep state ring
-//   large T : tensor-bound -> 64-token chunks, deeper operand ring, shallow state ring
+//   small T : HBM-bound -> short token chunks, state ring as deep as shared memory allows
+//   large T : tensor-bound -> 64-token chunks, 4-stage operand ring, shallow state ring
+// Template arguments: <moments, mode, token chunk, operand stages, state stages, CTA group, chunk rows, chunk cols>.
+// FORGE_CFG selects the other instantiations for tuning sweeps and the determinism tests only.
+int pick_variant(int maxT) {
+    const int forced = env_int("FORGE_CFG", -1);   // debug only
+    return forced >= 0 ? forced : (maxT > 1024 ? 5 : 0);
+}
+
 forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, const AdamWScalars &hp,
                               const DeviceInfo &dev, cudaStream_t stream) {
     int maxT = 0;
     for (int i = 0; i < count; ++i) maxT = probs[i].T > maxT ? probs[i].T : maxT;
-    int variant = maxT > 1024 ? 1 : 0;
-    const int forced = env_int("FORGE_CFG", -1);   // debug only
-    if (forced >= 0) variant = forced;
+    const int variant = pick_variant(maxT);
     switch (mdt) {
     case FORGE_MOMENT_FP32:
-        if (variant == 1) return launch_fused<MDT_FP32, MODE_ADAMW, 64, 3, 2>(probs, count, hp, dev, stream);
-        if (variant == 2) return launch_fused<MDT_FP32, MODE_ADAMW, 32, 2, 4>(probs, count, hp, dev, stream);
-        if (variant == 3) return launch_fused<MDT_FP32, MODE_ADAMW, 32, 3, 4, 2>(probs, count, hp, dev, stream);
-        if (variant == 4) return launch_fused<MDT_FP32, MODE_ADAMW, 64, 2, 4, 2>(probs, count, hp, dev, stream);
-        if (variant == 5) return launch_fused<MDT_FP32, MODE_ADAMW, 64, 4, 2, 2>(probs, count, hp, dev, stream);
-        return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 4, 2>(probs, count, hp, dev, stream);
+        switch (variant) {
+        case 1: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 3, 2, 1, 64, 64>(probs, count, hp, dev, stream);
+        case 2: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 4, 2, 128, 32>(probs, count, hp, dev, stream);
+        case 3: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 4, 2, 32, 128>(probs, count, hp, dev, stream);
+        case 4: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 2, 4, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 5: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 4, 2, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 6: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 7: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 2, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 8: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 8, 2, 64, 32>(probs, count, hp, dev, stream);
+        case 9: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 8, 2, 32, 64>(probs, count, hp, dev, stream);
+        case 10: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 2, 2, 64, 64>(probs, count, hp, dev, stream);
+        default: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 2, 2, 64, 128>(probs, count, hp, dev, stream);
+        }
     case FORGE_MOMENT_BF16:
-        if (variant == 1) return launch_fused<MDT_BF16, MODE_ADAMW, 64, 3, 2>(probs, count, hp, dev, stream);
-        if (variant == 2) return launch_fused<MDT_BF16, MODE_ADAMW, 32, 3, 6>(probs, count, hp, dev, stream);
-        if (variant == 3) return launch_fused<MDT_BF16, MODE_ADAMW, 64, 2, 6, 2>(probs, count, hp, dev, stream);
-        return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 6, 2>(probs, count, hp, dev, stream);
+        switch (variant) {
+        case 1: return launch_fused<MDT_BF16, MODE_ADAMW, 64, 3, 2, 1, 64, 64>(probs, count, hp, dev, stream);
+        case 2: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 6, 2, 128, 32>(probs, count, hp, dev, stream);
+        case 3: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 2, 4, 2, 64, 128>(probs, count, hp, dev, stream);
+        case 4: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 2, 4, 2, 32, 256>(probs, count, hp, dev, stream);
+        case 5: return launch_fused<MDT_BF16, MODE_ADAMW, 64, 4, 2, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 6: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 7: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 2, 2, 64, 128>(probs, count, hp, dev, stream);
+        default: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 6, 2, 64, 64>(probs, count, hp, dev, stream);
+        }
     case FORGE_MOMENT_INT8:
-        if (variant == 2) return launch_fused<MDT_INT8, MODE_ADAMW, 32, 2, 10>(probs, count, hp, dev, stream);
-        return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 10, 2>(probs, count, hp, dev, stream);
+        switch (variant) {
+        case 2: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 10, 2, 128, 32>(probs, count, hp, dev, stream);
+        default: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 10, 2, 64, 64>(probs, count, hp, dev, stream);
+        }
     default:
         return FORGE_ERR_BAD_DTYPE;
     }
@@ -307,13 +326,13 @@ forge_status_t forge_wgrad_store_g(const void *X, const void *dY, float *G, int3
     p.X = X; p.dY = dY; p.m = G; p.T = T; p.out = out; p.in = in;
     AdamWScalars hp;
     std::memset(&hp, 0, sizeof(hp));
-    // same token-chunk length as the fused variant chosen for this T: identical summation order
-    int variant = T > 1024 ? 1 : 0;
-    const int forced = env_int("FORGE_CFG", -1);
-    if (forced >= 0) variant = forced;
-    if (variant == 1)
-        return launch_fused<MDT_FP32, MODE_STORE_G, 64, 3, 2>(&p, 1, hp, dev, reinterpret_cast<cudaStream_t>(stream));
-    return launch_fused<MDT_FP32, MODE_STORE_G, 32, 2, 4>(&p, 1, hp, dev, reinterpret_cast<cudaStream_t>(stream));
+    // same token-chunk length and CTA grouping as the fused variant chosen for this T: identical
+    // summation order, so store-G + forge_adamw_from_g is bit-identical to the fused call
+    const int variant = pick_variant(T);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    if (variant == 1) return launch_fused<MDT_FP32, MODE_STORE_G, 64, 3, 2, 1, 64, 64>(&p, 1, hp, dev, st);
+    if (variant == 4 || variant == 5) return launch_fused<MDT_FP32, MODE_STORE_G, 64, 4, 2, 2, 64, 64>(&p, 1, hp, dev, st);
+    return launch_fused<MDT_FP32, MODE_STORE_G, 32, 4, 2, 2, 64, 128>(&p, 1, hp, dev, st);
 }
 
 forge_status_t forge_adamw_from_g(const float *G, void *W, void *m, void *v, float *m_scale, float *v_scale,

@@ -2,7 +2,7 @@
 //
 // Per weight tile (128 rows of `out` x 256 columns of `in`), Algorithm 1:
 //   lines 2-5  G_ij = sum_k dY_k,i^T X_k,j      tcgen05.mma, bf16 x bf16 -> fp32 in tensor memory
-//   line  6    load W_ij, m_ij, v_ij            TMA, 128 x 32-column chunks into a smem ring
+//   line  6    load W_ij, m_ij, v_ij            TMA, CM x CN chunks (default 64 x 64) into a smem ring
 //   lines 7-10 AdamW in fp32 registers          adamw_math.cuh
 //   line  11   store W_ij, m_ij, v_ij           in place in the smem chunk, then TMA store
 // G never leaves the SM.  One CTA owns a tile for the whole token loop, so a
@@ -15,7 +15,8 @@
 //               they run ahead of the mainloop and across tile boundaries)
 //   warp 3      state storer: TMA stores of finished chunks, recycles ring slots
 //   warps 4-11  two epilogue warpgroups; warp w reads TMEM lanes 32*(w%4).., one W row per thread,
-//               warpgroup g takes chunks g, g+2, ...
+//               32 columns at a time: a chunk is cut into 32 x 32 sub-blocks, the warp whose TMEM
+//               lane quadrant holds the rows takes them, warpgroup g the sub-block columns g, g+2, ..
 //
 // Both GEMM operands are MN-major: A = dY^T has `out` contiguous, B = X has `in` contiguous, and
 // the token axis (K) is the slow axis of both.  A token chunk is staged as 64-element (128 B)
@@ -34,8 +35,7 @@ namespace forge {
 constexpr int kMaxProblems = 8;
 constexpr int BLOCK_M = 128;   // tile rows  (out)  = TMEM lanes
 constexpr int BLOCK_N = 256;   // tile cols  (in)   = TMEM columns = one int8 block per row
-constexpr int CHUNK_N = 32;    // state chunk columns
-constexpr int CHUNKS = BLOCK_N / CHUNK_N;
+constexpr int SUB = 32;        // epilogue sub-block: 32 rows (one warp's TMEM lanes) x 32 columns
 constexpr int kCtrlWarps = 4;
 constexpr int kEpiWarps = 8;
 constexpr int kThreads = (kCtrlWarps + kEpiWarps) * 32;
@@ -63,7 +63,7 @@ struct alignas(64) KernelParams {
     AdamWScalars hp;
     int32_t num_problems;
     int32_t total_tiles;
-    int32_t pf_chunks;   // state chunks prefetched into L2 ahead of the shared-memory ring
+    int32_t pad_;
     int32_t debug;       // ablation switches for profiling ONLY (results are wrong when set):
                          // 1 = no operand loads / MMA, 2 = no state loads / stores, 4 = no epilogue math
 };
@@ -74,18 +74,38 @@ enum : int { DBG_NO_MAINLOOP = 1, DBG_NO_STATE = 2, DBG_NO_EPILOGUE = 4 };
 // 256 columns), the pair's leader issues one M=256 MMA that reads both CTAs' shared memory, and
 // each CTA's TMEM receives its own 128 x 256 accumulator.  Operand bytes per CTA fall by a third
 // (L2 -> SM traffic and smem per stage), the state path stays CTA-local.
-template <int MDT, int kBlockK, int kStages, int kStateStages, int CG = 1>
+// State chunk geometry.  The state stream (W, m, v once in, once out) is the roofline of the
+// HBM-bound shapes, and what it achieves depends on the chunk shape more than on the depth of the
+// ring: a probe that only streams W/m/v through TMA in place (profiles/r01_state_stream_probe.md)
+// reaches 5.3 TB/s with 128 x 32 chunks and 6.0 TB/s with 64 x 64 chunks at the same 160 KB of ring
+// (longer contiguous runs per DRAM page, fewer pages open at once).
+template <int MDT, int kBlockK, int kStages, int kStateStages, int CG = 1, int CM_ = 64, int CN_ = 64>
 struct KernelCfg {
     static constexpr int kMomBytes = (MDT == MDT_FP32) ? 4 : (MDT == MDT_BF16 ? 2 : 1);
     static constexpr int A_STAGE = kBlockK * 128 * (BLOCK_M / 64);
     static constexpr int B_STAGE = kBlockK * 128 * (BLOCK_N / 64) / CG;
     static constexpr int ML_STAGE = A_STAGE + B_STAGE;
-    static constexpr int W_ROW = CHUNK_N * 2;
-    static constexpr int M_ROW = CHUNK_N * kMomBytes;
-    static constexpr int W_CHUNK = BLOCK_M * W_ROW;
-    static constexpr int M_CHUNK = (BLOCK_M * M_ROW + 1023) / 1024 * 1024;
+    // chunk = CM rows x CN columns of the tile; RB x CB chunks per tile, row block fastest
+    static constexpr int CM = CM_, CN = CN_;
+    static constexpr int RB = BLOCK_M / CM, CB = BLOCK_N / CN, CHUNKS = RB * CB;
+    static constexpr int SUBS = CN / SUB;                   // 32-column sub-blocks per chunk row
+    static constexpr int WGS = SUBS >= 2 ? 2 : 1;           // warpgroups that share one chunk
+    // chunks ci and ci + PERIOD are consumed by the same warps
+    static constexpr int PERIOD = RB * (SUBS >= 2 ? 1 : 2);
+    static constexpr int DONE_COUNT = (CM / SUB) * WGS * 32;
+    // TMA boxes: at most 128 B per row (one swizzle span), CM rows
+    static constexpr int W_BOX_COLS = CN < 64 ? CN : 64;
+    static constexpr int W_ROW = W_BOX_COLS * 2;
+    static constexpr int W_BOXES = CN / W_BOX_COLS;
+    static constexpr int W_BOX = CM * W_ROW;
+    static constexpr int W_CHUNK = W_BOXES * W_BOX;
+    static constexpr int M_BOX_COLS = CN < 128 / kMomBytes ? CN : 128 / kMomBytes;
+    static constexpr int M_ROW = M_BOX_COLS * kMomBytes;
+    static constexpr int M_BOXES = CN / M_BOX_COLS;
+    static constexpr int M_BOX = CM * M_ROW;
+    static constexpr int M_CHUNK = M_BOXES * M_BOX;
     static constexpr int ST_STAGE = W_CHUNK + 2 * M_CHUNK;
-    static constexpr int ST_TX_BYTES = BLOCK_M * (W_ROW + 2 * M_ROW);
+    static constexpr int ST_TX_BYTES = ST_STAGE;
     static constexpr int kNumBars = 2 * kStages + 4 + 3 * kStateStages;
     static constexpr int XCHG_BYTES = (MDT == MDT_INT8) ? 4096 : 0;   // absmax exchange, 2 buffers
     static constexpr int SMEM_BYTES = 1024 /*align slack*/ + kStages * ML_STAGE +
@@ -93,12 +113,14 @@ struct KernelCfg {
     static_assert(SMEM_BYTES <= 232448, "shared memory budget exceeded");
     static_assert(kBlockK % 16 == 0 && kBlockK >= 16, "kBlockK must be a multiple of UMMA_K");
     static_assert(CG == 1 || CG == 2, "CTA group is 1 or 2");
-    static_assert(MDT != MDT_INT8 || kStateStages >= CHUNKS + 1, "int8 needs a whole tile resident");
-    // Chunk ci lives in ring slot ci % kStateStages and is consumed by epilogue warpgroup ci % 2.
-    // With an even ring every slot always belongs to the same warpgroup, so a warpgroup observes
-    // every phase of the slot barriers it waits on; with an odd ring it would skip the other
-    // warpgroup's phases and an mbarrier parity wait could alias to a phase two steps back.
-    static_assert(kStateStages % 2 == 0, "state ring must be even (one consumer warpgroup per slot)");
+    static_assert(BLOCK_M % CM == 0 && BLOCK_N % CN == 0 && CM % SUB == 0 && CN % SUB == 0, "chunk must tile the tile");
+    static_assert(W_BOX % 1024 == 0 && M_BOX % 1024 == 0, "boxes must keep the swizzle pattern aligned");
+    static_assert(MDT != MDT_INT8 || kStateStages >= CHUNKS + PERIOD, "int8 needs a whole tile resident");
+    // Chunk ci lives in ring slot ci % kStateStages.  With the ring a multiple of PERIOD every slot is
+    // always consumed by the same warps, so a warp observes every phase of the slot barriers it
+    // waits on; otherwise it would skip phases and an mbarrier parity wait could alias to a phase
+    // two steps back.
+    static_assert(kStateStages % PERIOD == 0 && CHUNKS % PERIOD == 0, "ring must be a multiple of the consumer period");
 };
 
 struct TileCoord {
@@ -116,7 +138,7 @@ __device__ __forceinline__ TileCoord decode_tile(const KernelParams &P, int tile
     return TileCoord{p, (local / tn_count) * CG + static_cast<int>(rank), local % tn_count};
 }
 
-// byte offset of 16-byte chunk j of row r in a TMA-swizzled box whose rows are ROW bytes long
+// byte offset of 16-byte piece j of row r in a TMA-swizzled box whose rows are ROW bytes long
 template <int ROW>
 __device__ __forceinline__ uint32_t swz(uint32_t r, uint32_t j) {
     if constexpr (ROW == 128) return r * 128u + ((j ^ (r & 7u)) << 4);
@@ -124,55 +146,67 @@ __device__ __forceinline__ uint32_t swz(uint32_t r, uint32_t j) {
     else return r * 32u + ((j ^ ((r >> 2) & 1u)) << 4);
 }
 
+// Where the 32 columns [col, col + 32) of chunk row r live in the chunk's shared-memory image.
+template <class Cfg>
+struct SubAddr {
+    uint32_t w, m, v;      // box base addresses (shared window)
+    uint32_t pw, pm;       // first 16-byte piece of the sub-block inside the box row
+    __device__ __forceinline__ SubAddr(uint32_t chunk_base, int col) {
+        const int wb = col / Cfg::W_BOX_COLS, mb = col / Cfg::M_BOX_COLS;
+        w = chunk_base + wb * Cfg::W_BOX;
+        m = chunk_base + Cfg::W_CHUNK + mb * Cfg::M_BOX;
+        v = m + Cfg::M_CHUNK;
+        pw = (col % Cfg::W_BOX_COLS) * 2 / 16;
+        pm = (col % Cfg::M_BOX_COLS) * Cfg::kMomBytes / 16;
+    }
+};
+
 // ---------------------------------------------------------------------------------------------
-// epilogue bodies: one thread = one W row of the tile, 32 columns of chunk `c` at a time
+// epilogue bodies: one thread = one W row of the chunk, one 32-column sub-block at a time
 // ---------------------------------------------------------------------------------------------
-template <int MDT>
-__device__ __forceinline__ void epi_chunk_fp(const AdamWScalars &hp, const uint32_t (&g)[32],
-                                             uint32_t sW, uint32_t sM, uint32_t sV, uint32_t row) {
-    // 4 groups of 8 columns: one 16 B piece of W (8 bf16) + matching moments
+template <int MDT, class Cfg>
+__device__ __forceinline__ void epi_sub_fp(const AdamWScalars &hp, const uint32_t (&g)[32],
+                                           const SubAddr<Cfg> &a, uint32_t row) {
+    // 4 groups of 8 columns: one 16 B piece of W (8 bf16) + matching moments, as 4 coordinate pairs
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-        const uint32_t aw = sW + swz<64>(row, j);
-        uint4 wq = lds128(aw);
-        float w[8] = {bf16lo(wq.x), bf16hi(wq.x), bf16lo(wq.y), bf16hi(wq.y),
-                      bf16lo(wq.z), bf16hi(wq.z), bf16lo(wq.w), bf16hi(wq.w)};
-        float m[8], v[8];
+        const uint32_t aw = a.w + swz<Cfg::W_ROW>(row, a.pw + j);
+        const uint4 wq = lds128(aw);
+        f32x2 w[4] = {bf16x2_to_f32x2(wq.x), bf16x2_to_f32x2(wq.y), bf16x2_to_f32x2(wq.z), bf16x2_to_f32x2(wq.w)};
+        f32x2 m[4], v[4];
         if constexpr (MDT == MDT_FP32) {
-            const uint32_t am0 = sM + swz<128>(row, 2 * j), am1 = sM + swz<128>(row, 2 * j + 1);
-            const uint32_t av0 = sV + swz<128>(row, 2 * j), av1 = sV + swz<128>(row, 2 * j + 1);
-            uint4 a = lds128(am0), b = lds128(am1), c = lds128(av0), d = lds128(av1);
-            m[0] = __uint_as_float(a.x); m[1] = __uint_as_float(a.y); m[2] = __uint_as_float(a.z); m[3] = __uint_as_float(a.w);
-            m[4] = __uint_as_float(b.x); m[5] = __uint_as_float(b.y); m[6] = __uint_as_float(b.z); m[7] = __uint_as_float(b.w);
-            v[0] = __uint_as_float(c.x); v[1] = __uint_as_float(c.y); v[2] = __uint_as_float(c.z); v[3] = __uint_as_float(c.w);
-            v[4] = __uint_as_float(d.x); v[5] = __uint_as_float(d.y); v[6] = __uint_as_float(d.z); v[7] = __uint_as_float(d.w);
+            const uint32_t o0 = swz<Cfg::M_ROW>(row, a.pm + 2 * j), o1 = swz<Cfg::M_ROW>(row, a.pm + 2 * j + 1);
+            const uint32_t am0 = a.m + o0, am1 = a.m + o1, av0 = a.v + o0, av1 = a.v + o1;
+            const uint4 x = lds128(am0), b = lds128(am1), c = lds128(av0), d = lds128(av1);
+            m[0] = pk2u(x.x, x.y); m[1] = pk2u(x.z, x.w); m[2] = pk2u(b.x, b.y); m[3] = pk2u(b.z, b.w);
+            v[0] = pk2u(c.x, c.y); v[1] = pk2u(c.z, c.w); v[2] = pk2u(d.x, d.y); v[3] = pk2u(d.z, d.w);
 #pragma unroll
-            for (int e = 0; e < 8; ++e) adamw_update(hp, __uint_as_float(g[8 * j + e]), w[e], m[e], v[e]);
-            sts128(am0, make_uint4(__float_as_uint(m[0]), __float_as_uint(m[1]), __float_as_uint(m[2]), __float_as_uint(m[3])));
-            sts128(am1, make_uint4(__float_as_uint(m[4]), __float_as_uint(m[5]), __float_as_uint(m[6]), __float_as_uint(m[7])));
-            sts128(av0, make_uint4(__float_as_uint(v[0]), __float_as_uint(v[1]), __float_as_uint(v[2]), __float_as_uint(v[3])));
-            sts128(av1, make_uint4(__float_as_uint(v[4]), __float_as_uint(v[5]), __float_as_uint(v[6]), __float_as_uint(v[7])));
+            for (int e = 0; e < 4; ++e) adamw_update2(hp, pk2u(g[8 * j + 2 * e], g[8 * j + 2 * e + 1]), w[e], m[e], v[e]);
+            sts128(am0, make_uint4(lo2u(m[0]), hi2u(m[0]), lo2u(m[1]), hi2u(m[1])));
+            sts128(am1, make_uint4(lo2u(m[2]), hi2u(m[2]), lo2u(m[3]), hi2u(m[3])));
+            sts128(av0, make_uint4(lo2u(v[0]), hi2u(v[0]), lo2u(v[1]), hi2u(v[1])));
+            sts128(av1, make_uint4(lo2u(v[2]), hi2u(v[2]), lo2u(v[3]), hi2u(v[3])));
         } else {
-            const uint32_t am = sM + swz<64>(row, j), av = sV + swz<64>(row, j);
-            uint4 a = lds128(am), c = lds128(av);
-            m[0] = bf16lo(a.x); m[1] = bf16hi(a.x); m[2] = bf16lo(a.y); m[3] = bf16hi(a.y);
-            m[4] = bf16lo(a.z); m[5] = bf16hi(a.z); m[6] = bf16lo(a.w); m[7] = bf16hi(a.w);
-            v[0] = bf16lo(c.x); v[1] = bf16hi(c.x); v[2] = bf16lo(c.y); v[3] = bf16hi(c.y);
-            v[4] = bf16lo(c.z); v[5] = bf16hi(c.z); v[6] = bf16lo(c.w); v[7] = bf16hi(c.w);
+            const uint32_t o = swz<Cfg::M_ROW>(row, a.pm + j);
+            const uint32_t am = a.m + o, av = a.v + o;
+            const uint4 x = lds128(am), c = lds128(av);
+            m[0] = bf16x2_to_f32x2(x.x); m[1] = bf16x2_to_f32x2(x.y); m[2] = bf16x2_to_f32x2(x.z); m[3] = bf16x2_to_f32x2(x.w);
+            v[0] = bf16x2_to_f32x2(c.x); v[1] = bf16x2_to_f32x2(c.y); v[2] = bf16x2_to_f32x2(c.z); v[3] = bf16x2_to_f32x2(c.w);
 #pragma unroll
-            for (int e = 0; e < 8; ++e) adamw_update(hp, __uint_as_float(g[8 * j + e]), w[e], m[e], v[e]);
-            sts128(am, make_uint4(pack_bf16(m[0], m[1]), pack_bf16(m[2], m[3]), pack_bf16(m[4], m[5]), pack_bf16(m[6], m[7])));
-            sts128(av, make_uint4(pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]), pack_bf16(v[4], v[5]), pack_bf16(v[6], v[7])));
+            for (int e = 0; e < 4; ++e) adamw_update2(hp, pk2u(g[8 * j + 2 * e], g[8 * j + 2 * e + 1]), w[e], m[e], v[e]);
+            sts128(am, make_uint4(f32x2_to_bf16x2(m[0]), f32x2_to_bf16x2(m[1]), f32x2_to_bf16x2(m[2]), f32x2_to_bf16x2(m[3])));
+            sts128(av, make_uint4(f32x2_to_bf16x2(v[0]), f32x2_to_bf16x2(v[1]), f32x2_to_bf16x2(v[2]), f32x2_to_bf16x2(v[3])));
         }
-        sts128(aw, make_uint4(pack_bf16(w[0], w[1]), pack_bf16(w[2], w[3]), pack_bf16(w[4], w[5]), pack_bf16(w[6], w[7])));
+        sts128(aw, make_uint4(f32x2_to_bf16x2(w[0]), f32x2_to_bf16x2(w[1]), f32x2_to_bf16x2(w[2]), f32x2_to_bf16x2(w[3])));
     }
 }
 
-// store-G twin: the fp32 tile chunk goes to the smem chunk buffer unchanged
-__device__ __forceinline__ void epi_chunk_store_g(const uint32_t (&g)[32], uint32_t sG, uint32_t row) {
+// store-G twin: the fp32 sub-block goes to the chunk's m image unchanged
+template <class Cfg>
+__device__ __forceinline__ void epi_sub_store_g(const uint32_t (&g)[32], const SubAddr<Cfg> &a, uint32_t row) {
 #pragma unroll
     for (int j = 0; j < 8; ++j)
-        sts128(sG + swz<128>(row, j), make_uint4(g[4 * j], g[4 * j + 1], g[4 * j + 2], g[4 * j + 3]));
+        sts128(a.m + swz<Cfg::M_ROW>(row, a.pm + j), make_uint4(g[4 * j], g[4 * j + 1], g[4 * j + 2], g[4 * j + 3]));
 }
 
 
@@ -182,100 +216,110 @@ __device__ __forceinline__ void epi_chunk_store_g(const uint32_t (&g)[32], uint3
 // pass 2 recomputes the identical m', v' (same instructions, same operands), forms W', and emits
 // the codes.  A row is owned by one thread of each warpgroup (even / odd chunks); the two partial
 // maxima are combined through shared memory.
-__device__ __forceinline__ void unpack_codes(const uint4 &q, int (&c)[16], bool is_signed) {
-    const uint32_t w[4] = {q.x, q.y, q.z, q.w};
-#pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        const uint32_t b = (w[i >> 2] >> (8 * (i & 3))) & 0xFFu;
-        c[i] = is_signed ? static_cast<int>(static_cast<int8_t>(b)) : static_cast<int>(b);
-    }
-}
-__device__ __forceinline__ uint4 pack_codes(const int (&c)[16]) {
-    uint32_t w[4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-        w[i] = (static_cast<uint32_t>(c[4 * i]) & 0xFFu) | ((static_cast<uint32_t>(c[4 * i + 1]) & 0xFFu) << 8) |
-               ((static_cast<uint32_t>(c[4 * i + 2]) & 0xFFu) << 16) | ((static_cast<uint32_t>(c[4 * i + 3]) & 0xFFu) << 24);
-    return make_uint4(w[0], w[1], w[2], w[3]);
-}
-
 template <class Cfg, int kStateStages, int CG>
 __device__ __forceinline__ void epi_tile_int8(const KernelParams &P, const AdamWScalars &hp, int tile, uint32_t rank,
                                               uint32_t titer, uint32_t taddr, uint32_t sST,
-                                              uint32_t bar_st_full, uint32_t bar_st_done, uint32_t row,
-                                              int wg, uint32_t s_xchg) {
+                                              uint32_t bar_st_full, uint32_t bar_st_done, uint32_t quad,
+                                              uint32_t lane, int wg, uint32_t s_xchg) {
     const TileCoord tc = decode_tile<CG>(P, tile, rank);
     const ProblemDesc &pd = P.prob[tc.p];
-    const int row_g = tc.tm * BLOCK_M + static_cast<int>(row);
+    const uint32_t row_t = quad * 32 + lane;                 // row of the tile == TMEM lane
+    const uint32_t rb = row_t / Cfg::CM, row = row_t % Cfg::CM;
+    const int row_g = tc.tm * BLOCK_M + static_cast<int>(row_t);
     const bool valid = row_g < pd.out;
     const size_t sidx = static_cast<size_t>(valid ? row_g : 0) * static_cast<size_t>(pd.in / BLOCK_N) + tc.tn;
     const float a_m_old = valid ? pd.m_scale[sidx] : 0.0f;
     const float a_v_old = valid ? pd.v_scale[sidx] : 0.0f;
-    const float dm = dequant_step(a_m_old, 127.0f), dv = dequant_step(a_v_old, 255.0f);
+    const float bm = __fmul_rn(hp.beta1, dequant_step(a_m_old, 127.0f));
+    const float bv = __fmul_rn(hp.beta2, dequant_step(a_v_old, 255.0f));
 
-    // ---- pass 1: block absmax of m', v'
+    // ---- pass 1: block absmax of m', v' over this warp's sub-blocks of the row
     float pm = 0.0f, pv = 0.0f;
-    for (int c = wg; c < CHUNKS; c += 2) {
-        const uint32_t ci = titer * CHUNKS + c;
+    for (int cb = 0; cb < Cfg::CB; ++cb) {
+        if (Cfg::SUBS < 2 && (cb & 1) != wg) continue;
+        const uint32_t ci = titer * Cfg::CHUNKS + cb * Cfg::RB + rb;
         const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
-        uint32_t g[32];
-        tmem_ld_32x32b_x32(taddr + c * CHUNK_N, g);
-        const uint32_t sM = sST + s * Cfg::ST_STAGE + Cfg::W_CHUNK, sV = sM + Cfg::M_CHUNK;
         mbar_wait(bar_st_full + 8 * s, ph);
-        tmem_ld_wait();
+        for (int j32 = (Cfg::SUBS >= 2 ? wg : 0); j32 < Cfg::SUBS; j32 += Cfg::WGS) {
+            uint32_t g[32];
+            tmem_ld_32x32b_x32(taddr + cb * Cfg::CN + j32 * SUB, g);
+            const SubAddr<Cfg> a(sST + s * Cfg::ST_STAGE, j32 * SUB);
+            tmem_ld_wait();
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {
-            int mc[16], vc[16];
-            unpack_codes(lds128(sM + swz<32>(row, j)), mc, true);
-            unpack_codes(lds128(sV + swz<32>(row, j)), vc, false);
+            for (int j = 0; j < 2; ++j) {
+                const uint32_t o = swz<Cfg::M_ROW>(row, a.pm + j);
+                const uint4 mq = lds128(a.m + o), vq = lds128(a.v + o);
+                const uint32_t mw[4] = {mq.x, mq.y, mq.z, mq.w}, vw[4] = {vq.x, vq.y, vq.z, vq.w};
 #pragma unroll
-            for (int e = 0; e < 16; ++e) {
-                float w = 0.0f, m = __fmul_rn(static_cast<float>(mc[e]), dm), v = __fmul_rn(static_cast<float>(vc[e]), dv);
-                adamw_update(hp, __uint_as_float(g[16 * j + e]), w, m, v);
-                pm = fmaxf(pm, fabsf(m));
-                pv = fmaxf(pv, fabsf(v));
+                for (int q = 0; q < 4; ++q) {
+                    f32x2 cm[2], cv[2];
+                    codes4_to_f32(mw[q], true, cm[0], cm[1]);
+                    codes4_to_f32(vw[q], false, cv[0], cv[1]);
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int gi = 16 * j + 4 * q + 2 * e;
+                        f32x2 m, v;
+                        adamw_moments2_q(hp, pk2u(g[gi], g[gi + 1]), cm[e], cv[e], bm, bv, m, v);
+                        pm = fmaxf(pm, fmaxf(fabsf(lo2(m)), fabsf(hi2(m))));
+                        pv = fmaxf(pv, fmaxf(lo2(v), hi2(v)));           // v' >= 0
+                    }
+                }
             }
         }
     }
-    // ---- combine the two half-rows
+    // ---- combine the two warpgroups' parts of the row (same TMEM quadrant: warps quad and 4 + quad)
     const uint32_t xb = s_xchg + (titer & 1u) * 2048u;
-    asm volatile("st.shared.v2.f32 [%0], {%1, %2};\n" ::"r"(xb + (wg * 128u + row) * 8u), "f"(pm), "f"(pv) : "memory");
-    asm volatile("bar.sync 1, 256;\n" ::: "memory");
+    asm volatile("st.shared.v2.f32 [%0], {%1, %2};\n" ::"r"(xb + (wg * 128u + row_t) * 8u), "f"(pm), "f"(pv) : "memory");
+    asm volatile("bar.sync %0, 64;\n" ::"r"(1u + quad) : "memory");
     float om, ov;
-    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];\n" : "=f"(om), "=f"(ov) : "r"(xb + ((wg ^ 1) * 128u + row) * 8u));
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];\n" : "=f"(om), "=f"(ov) : "r"(xb + ((wg ^ 1) * 128u + row_t) * 8u));
     const float a_m = fmaxf(pm, om), a_v = fmaxf(pv, ov);
     const float inv_m = quant_inv_scale(a_m, 127.0f), inv_v = quant_inv_scale(a_v, 255.0f);
+    const float v_floor = quant_v_floor(inv_v);
 
-    // ---- pass 2: recompute, update W, requantise
-    for (int c = wg; c < CHUNKS; c += 2) {
-        const uint32_t ci = titer * CHUNKS + c;
+    // ---- pass 2: recompute (same instructions, same operands), update W, requantise
+    for (int cb = 0; cb < Cfg::CB; ++cb) {
+        if (Cfg::SUBS < 2 && (cb & 1) != wg) continue;
+        const uint32_t ci = titer * Cfg::CHUNKS + cb * Cfg::RB + rb;
         const uint32_t s = ci % kStateStages;
-        uint32_t g[32];
-        tmem_ld_32x32b_x32(taddr + c * CHUNK_N, g);
-        const uint32_t sW = sST + s * Cfg::ST_STAGE, sM = sW + Cfg::W_CHUNK, sV = sM + Cfg::M_CHUNK;
-        tmem_ld_wait();
+        for (int j32 = (Cfg::SUBS >= 2 ? wg : 0); j32 < Cfg::SUBS; j32 += Cfg::WGS) {
+            uint32_t g[32];
+            tmem_ld_32x32b_x32(taddr + cb * Cfg::CN + j32 * SUB, g);
+            const SubAddr<Cfg> a(sST + s * Cfg::ST_STAGE, j32 * SUB);
+            tmem_ld_wait();
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {
-            int mc[16], vc[16];
-            const uint32_t am = sM + swz<32>(row, j), av = sV + swz<32>(row, j);
-            unpack_codes(lds128(am), mc, true);
-            unpack_codes(lds128(av), vc, false);
-            const uint32_t aw0 = sW + swz<64>(row, 2 * j), aw1 = sW + swz<64>(row, 2 * j + 1);
-            const uint4 w0 = lds128(aw0), w1 = lds128(aw1);
-            float w[16] = {bf16lo(w0.x), bf16hi(w0.x), bf16lo(w0.y), bf16hi(w0.y), bf16lo(w0.z), bf16hi(w0.z),
-                           bf16lo(w0.w), bf16hi(w0.w), bf16lo(w1.x), bf16hi(w1.x), bf16lo(w1.y), bf16hi(w1.y),
-                           bf16lo(w1.z), bf16hi(w1.z), bf16lo(w1.w), bf16hi(w1.w)};
+            for (int j = 0; j < 2; ++j) {
+                const uint32_t o = swz<Cfg::M_ROW>(row, a.pm + j);
+                const uint32_t am = a.m + o, av = a.v + o;
+                const uint4 mq = lds128(am), vq = lds128(av);
+                const uint32_t aw0 = a.w + swz<Cfg::W_ROW>(row, a.pw + 2 * j), aw1 = a.w + swz<Cfg::W_ROW>(row, a.pw + 2 * j + 1);
+                const uint4 w0 = lds128(aw0), w1 = lds128(aw1);
+                const uint32_t mw[4] = {mq.x, mq.y, mq.z, mq.w}, vw[4] = {vq.x, vq.y, vq.z, vq.w};
+                const uint32_t ww[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+                uint32_t mo[4], vo[4], wo[8];
 #pragma unroll
-            for (int e = 0; e < 16; ++e) {
-                float m = __fmul_rn(static_cast<float>(mc[e]), dm), v = __fmul_rn(static_cast<float>(vc[e]), dv);
-                adamw_update(hp, __uint_as_float(g[16 * j + e]), w[e], m, v);
-                mc[e] = quant_m_code(m, inv_m);
-                vc[e] = quant_v_code(v, inv_v);
+                for (int q = 0; q < 4; ++q) {
+                    f32x2 cm[2], cv[2], qm[2], qv[2];
+                    codes4_to_f32(mw[q], true, cm[0], cm[1]);
+                    codes4_to_f32(vw[q], false, cv[0], cv[1]);
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int gi = 16 * j + 4 * q + 2 * e;
+                        f32x2 m, v, w = bf16x2_to_f32x2(ww[2 * q + e]);
+                        adamw_moments2_q(hp, pk2u(g[gi], g[gi + 1]), cm[e], cv[e], bm, bv, m, v);
+                        adamw_weight2(hp, m, v, w);
+                        wo[2 * q + e] = f32x2_to_bf16x2(w);
+                        qm[e] = quant_m2(m, inv_m);
+                        qv[e] = quant_v2(v, inv_v, v_floor);
+                    }
+                    mo[q] = pack_codes4(qm[0], qm[1]);
+                    vo[q] = pack_codes4(qv[0], qv[1]);
+                }
+                sts128(am, make_uint4(mo[0], mo[1], mo[2], mo[3]));
+                sts128(av, make_uint4(vo[0], vo[1], vo[2], vo[3]));
+                sts128(aw0, make_uint4(wo[0], wo[1], wo[2], wo[3]));
+                sts128(aw1, make_uint4(wo[4], wo[5], wo[6], wo[7]));
             }
-            sts128(am, pack_codes(mc));
-            sts128(av, pack_codes(vc));
-            sts128(aw0, make_uint4(pack_bf16(w[0], w[1]), pack_bf16(w[2], w[3]), pack_bf16(w[4], w[5]), pack_bf16(w[6], w[7])));
-            sts128(aw1, make_uint4(pack_bf16(w[8], w[9]), pack_bf16(w[10], w[11]), pack_bf16(w[12], w[13]), pack_bf16(w[14], w[15])));
         }
         fence_proxy_async_smem();
         mbar_arrive(bar_st_done + 8 * s);
@@ -289,10 +333,11 @@ __device__ __forceinline__ void epi_tile_int8(const KernelParams &P, const AdamW
 // ---------------------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------------------
-template <int MDT, int MODE, int kBlockK, int kStages, int kStateStages, int CG>
+template <int MDT, int MODE, int kBlockK, int kStages, int kStateStages, int CG, int CM, int CN>
 __global__ void __launch_bounds__(kThreads, 1)
 forge_fused_kernel(const __grid_constant__ KernelParams P) {
-    using Cfg = KernelCfg<MDT, kBlockK, kStages, kStateStages, CG>;
+    using Cfg = KernelCfg<MDT, kBlockK, kStages, kStateStages, CG, CM, CN>;
+    constexpr int CHUNKS = Cfg::CHUNKS;
     const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;   // rank 0 = the pair's leader
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -324,7 +369,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         }
         for (int i = 0; i < kStateStages; ++i) {
             mbar_init(bar_st_full + 8 * i, 1);
-            mbar_init(bar_st_done + 8 * i, 128);
+            mbar_init(bar_st_done + 8 * i, Cfg::DONE_COUNT);
             mbar_init(bar_st_empty + 8 * i, 1);
         }
         mbar_fence_init();
@@ -419,49 +464,27 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
     } else if (warp == 2) {
         // ================= state loader (Alg. 1 line 6: load W_ij, m_ij, v_ij) ===================
         if (MODE == MODE_ADAMW && lane == 0 && !(P.debug & DBG_NO_STATE)) {
-            // The ring holds only kStateStages chunks, and a slot stays busy through load latency,
-            // epilogue and store read; an L2 prefetch cursor runs pf_chunks further ahead so that
-            // the DRAM requests in flight are not bounded by shared memory (126 MB of L2 absorb it).
-            int pf_tile = first_tile, pf_c = 0;
-            TileCoord pf_tc = decode_tile<CG>(P, pf_tile < P.total_tiles ? pf_tile : first_tile, rank);
-            auto prefetch_next = [&]() {
-                if (pf_tile >= P.total_tiles) return;
-                const ProblemDesc &pd = P.prob[pf_tc.p];
-                const int x = pf_tc.tn * BLOCK_N + pf_c * CHUNK_N, y = pf_tc.tm * BLOCK_M;
-                tma_prefetch_l2_2d(&pd.map_W, x, y);
-                tma_prefetch_l2_2d(&pd.map_m, x, y);
-                tma_prefetch_l2_2d(&pd.map_v, x, y);
-                if (++pf_c == CHUNKS) {
-                    pf_c = 0;
-                    pf_tile += tile_step;
-                    if (pf_tile < P.total_tiles) pf_tc = decode_tile<CG>(P, pf_tile, rank);
-                }
-            };
-            for (int i = 0; i < P.pf_chunks + kStateStages; ++i) {
-                if (i >= kStateStages) prefetch_next();
-                else if (P.pf_chunks > 0) {   // the first ring fill is loaded directly: skip, do not prefetch
-                    if (++pf_c == CHUNKS) {
-                        pf_c = 0;
-                        pf_tile += tile_step;
-                        if (pf_tile < P.total_tiles) pf_tc = decode_tile<CG>(P, pf_tile, rank);
-                    }
-                }
-            }
             uint32_t ci = 0;  // running chunk counter
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step) {
                 const TileCoord tc = decode_tile<CG>(P, tile, rank);
                 const ProblemDesc &pd = P.prob[tc.p];
                 for (int c = 0; c < CHUNKS; ++c, ++ci) {
-                    if (P.pf_chunks > 0) prefetch_next();
                     const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
                     mbar_wait(bar_st_empty + 8 * s, ph ^ 1u);
                     const uint32_t full = bar_st_full + 8 * s;
                     mbar_expect_tx(full, Cfg::ST_TX_BYTES);
                     const uint32_t base = sST + s * Cfg::ST_STAGE;
-                    const int x = tc.tn * BLOCK_N + c * CHUNK_N, y = tc.tm * BLOCK_M;
-                    tma_load_2d(base, &pd.map_W, full, x, y, kEvictFirst);
-                    tma_load_2d(base + Cfg::W_CHUNK, &pd.map_m, full, x, y, kEvictFirst);
-                    tma_load_2d(base + Cfg::W_CHUNK + Cfg::M_CHUNK, &pd.map_v, full, x, y, kEvictFirst);
+                    const int x = tc.tn * BLOCK_N + (c / Cfg::RB) * CN, y = tc.tm * BLOCK_M + (c % Cfg::RB) * CM;
+#pragma unroll
+                    for (int i = 0; i < Cfg::W_BOXES; ++i)
+                        tma_load_2d(base + i * Cfg::W_BOX, &pd.map_W, full, x + i * Cfg::W_BOX_COLS, y, kEvictFirst);
+#pragma unroll
+                    for (int i = 0; i < Cfg::M_BOXES; ++i)
+                        tma_load_2d(base + Cfg::W_CHUNK + i * Cfg::M_BOX, &pd.map_m, full, x + i * Cfg::M_BOX_COLS, y, kEvictFirst);
+#pragma unroll
+                    for (int i = 0; i < Cfg::M_BOXES; ++i)
+                        tma_load_2d(base + Cfg::W_CHUNK + Cfg::M_CHUNK + i * Cfg::M_BOX, &pd.map_v, full,
+                                    x + i * Cfg::M_BOX_COLS, y, kEvictFirst);
                 }
             }
         }
@@ -486,14 +509,23 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                     }
                     mbar_wait(bar_st_done + 8 * s, ph);
                     const uint32_t base = sST + s * Cfg::ST_STAGE;
-                    const int x = tc.tn * BLOCK_N + c * CHUNK_N, y = tc.tm * BLOCK_M;
+                    const int x = tc.tn * BLOCK_N + (c / Cfg::RB) * CN, y = tc.tm * BLOCK_M + (c % Cfg::RB) * CM;
                     if (P.debug & DBG_NO_STATE) {
-                    } else if constexpr (MODE == MODE_ADAMW) {
-                        tma_store_2d(&pd.map_W, base, x, y, kEvictFirst);
-                        tma_store_2d(&pd.map_m, base + Cfg::W_CHUNK, x, y, kEvictFirst);
-                        tma_store_2d(&pd.map_v, base + Cfg::W_CHUNK + Cfg::M_CHUNK, x, y, kEvictFirst);
                     } else {
-                        tma_store_2d(&pd.map_m, base + Cfg::W_CHUNK, x, y, kEvictFirst);
+                        if constexpr (MODE == MODE_ADAMW) {
+#pragma unroll
+                            for (int i = 0; i < Cfg::W_BOXES; ++i)
+                                tma_store_2d(&pd.map_W, base + i * Cfg::W_BOX, x + i * Cfg::W_BOX_COLS, y, kEvictFirst);
+                        }
+#pragma unroll
+                        for (int i = 0; i < Cfg::M_BOXES; ++i)      // MODE_STORE_G: the m image carries G
+                            tma_store_2d(&pd.map_m, base + Cfg::W_CHUNK + i * Cfg::M_BOX, x + i * Cfg::M_BOX_COLS, y, kEvictFirst);
+                        if constexpr (MODE == MODE_ADAMW) {
+#pragma unroll
+                            for (int i = 0; i < Cfg::M_BOXES; ++i)
+                                tma_store_2d(&pd.map_v, base + Cfg::W_CHUNK + Cfg::M_CHUNK + i * Cfg::M_BOX,
+                                             x + i * Cfg::M_BOX_COLS, y, kEvictFirst);
+                        }
                     }
                     tma_store_commit();
                     if (held >= 0) {
@@ -511,7 +543,8 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         const int ew = warp - kCtrlWarps;
         const int wg = ew >> 2;                       // warpgroup 0/1
         const uint32_t quad = warp & 3;               // TMEM lane quadrant this warp may read
-        const uint32_t row = quad * 32 + lane;        // row of the tile == TMEM lane
+        const uint32_t row_t = quad * 32 + lane;      // row of the tile == TMEM lane
+        const uint32_t rb = row_t / CM, row = row_t % CM;   // this warp's row block, row inside the chunk
         const AdamWScalars hp = P.hp;
         uint32_t titer = 0;
         for (int tile = first_tile; tile < P.total_tiles; tile += tile_step, ++titer) {
@@ -520,30 +553,30 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
             tc_fence_after();
             const uint32_t taddr = tmem_base + ((quad * 32u) << 16) + as * BLOCK_N;
             if constexpr (MDT != MDT_INT8) {
-                for (int c = wg; c < CHUNKS; c += 2) {
-                    const uint32_t ci = titer * CHUNKS + c;
+                for (int cb = 0; cb < Cfg::CB; ++cb) {
+                    if (Cfg::SUBS < 2 && (cb & 1) != wg) continue;
+                    const uint32_t ci = titer * CHUNKS + cb * Cfg::RB + rb;
                     const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
-                    uint32_t g[32];
-                    tmem_ld_32x32b_x32(taddr + c * CHUNK_N, g);
                     const uint32_t base = sST + s * Cfg::ST_STAGE;
-                    if constexpr (MODE == MODE_ADAMW) {
-                        if (!(P.debug & DBG_NO_STATE)) mbar_wait(bar_st_full + 8 * s, ph);
-                        else mbar_wait(bar_st_empty + 8 * s, ph ^ 1u);
+                    if (MODE == MODE_ADAMW && !(P.debug & DBG_NO_STATE)) mbar_wait(bar_st_full + 8 * s, ph);
+                    else mbar_wait(bar_st_empty + 8 * s, ph ^ 1u);
+                    for (int j32 = (Cfg::SUBS >= 2 ? wg : 0); j32 < Cfg::SUBS; j32 += Cfg::WGS) {
+                        uint32_t g[32];
+                        tmem_ld_32x32b_x32(taddr + cb * CN + j32 * SUB, g);
+                        const SubAddr<Cfg> a(base, j32 * SUB);
                         tmem_ld_wait();
-                        if (!(P.debug & DBG_NO_EPILOGUE))
-                            epi_chunk_fp<MDT>(hp, g, base, base + Cfg::W_CHUNK,
-                                              base + Cfg::W_CHUNK + Cfg::M_CHUNK, row);
-                    } else {
-                        mbar_wait(bar_st_empty + 8 * s, ph ^ 1u);
-                        tmem_ld_wait();
-                        epi_chunk_store_g(g, base + Cfg::W_CHUNK, row);
+                        if constexpr (MODE == MODE_ADAMW) {
+                            if (!(P.debug & DBG_NO_EPILOGUE)) epi_sub_fp<MDT, Cfg>(hp, g, a, row);
+                        } else {
+                            epi_sub_store_g<Cfg>(g, a, row);
+                        }
                     }
                     fence_proxy_async_smem();
                     mbar_arrive(bar_st_done + 8 * s);
                 }
             } else {
                 epi_tile_int8<Cfg, kStateStages, CG>(P, hp, tile, rank, titer, taddr, sST, bar_st_full,
-                                                 bar_st_done, row, wg, s_xchg);
+                                                     bar_st_done, quad, lane, wg, s_xchg);
             }
             // this warp has drained the accumulator: tell the (leader's) MMA issuer
             tc_fence_before();
