@@ -180,6 +180,10 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
                             swizzle_for_row_bytes(Cfg::M_ROW));
             ok &= encode_2d(&d.map_v, mom_dt, Cfg::kMomBytes, p.v, p.out, p.in, Cfg::M_BOX_COLS, CM,
                             swizzle_for_row_bytes(Cfg::M_ROW));
+            if (MDT == MDT_INT8) {   // first-pass view of the same codes: 128 rows x 128 columns per box
+                ok &= encode_2d(&d.map_m1, mom_dt, 1, p.m, p.out, p.in, 128, 128, CU_TENSOR_MAP_SWIZZLE_128B);
+                ok &= encode_2d(&d.map_v1, mom_dt, 1, p.v, p.out, p.in, 128, 128, CU_TENSOR_MAP_SWIZZLE_128B);
+            }
         } else {  // store-G twin: p.m carries the fp32 G output
             ok &= encode_2d(&d.map_m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, p.m, p.out, p.in, Cfg::M_BOX_COLS, CM,
                             swizzle_for_row_bytes(Cfg::M_ROW));
@@ -202,7 +206,7 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
     if (grid > tiles) grid = tiles;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(grid * CG));
-    cfg.blockDim = dim3(kThreads);
+    cfg.blockDim = dim3(block_threads(MDT));
     cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
@@ -263,8 +267,11 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
         }
     case FORGE_MOMENT_INT8:
         switch (variant) {
-        case 2: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 10, 2, 128, 32>(probs, count, hp, dev, stream);
-        default: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 10, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 1: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 2, 3, 1, 128, 64>(probs, count, hp, dev, stream);
+        case 2: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 2, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 3: return launch_fused<MDT_INT8, MODE_ADAMW, 16, 3, 4, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 5: return launch_fused<MDT_INT8, MODE_ADAMW, 64, 2, 2, 2, 128, 64>(probs, count, hp, dev, stream);
+        default: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 3, 2, 128, 64>(probs, count, hp, dev, stream);
         }
     default:
         return FORGE_ERR_BAD_DTYPE;

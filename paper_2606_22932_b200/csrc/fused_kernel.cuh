@@ -8,7 +8,7 @@
 // G never leaves the SM.  One CTA owns a tile for the whole token loop, so a
 // partial-K update can never be applied.
 //
-// Warp roles (384 threads, one CTA per SM, persistent over a static tile list):
+// Warp roles (384 threads -- 512 with int8 moments --, one CTA per SM, persistent over a static tile list):
 //   warp 0      operand producer: TMA loads of dY / X token chunks into the mainloop ring
 //   warp 1      MMA issuer: one thread issues tcgen05.mma; accumulators double-buffered in TMEM
 //   warp 2      TMEM allocator + state loader: TMA loads of W/m/v chunks (independent of G, so
@@ -37,8 +37,8 @@ constexpr int BLOCK_M = 128;   // tile rows  (out)  = TMEM lanes
 constexpr int BLOCK_N = 256;   // tile cols  (in)   = TMEM columns = one int8 block per row
 constexpr int SUB = 32;        // epilogue sub-block: 32 rows (one warp's TMEM lanes) x 32 columns
 constexpr int kCtrlWarps = 4;
-constexpr int kEpiWarps = 8;
-constexpr int kThreads = (kCtrlWarps + kEpiWarps) * 32;
+__host__ __device__ constexpr int epi_warps(int) { return 8; }
+__host__ __device__ constexpr int block_threads(int mdt) { return (kCtrlWarps + epi_warps(mdt)) * 32; }
 constexpr int kTmemCols = 512;  // 2 accumulator buffers x 256 fp32 columns
 
 enum : int { MDT_FP32 = 0, MDT_BF16 = 1, MDT_INT8 = 2 };
@@ -50,6 +50,8 @@ struct alignas(64) ProblemDesc {
     CUtensorMap map_W;   // [out, in] bf16, box {32, 128}, SWIZZLE_64B
     CUtensorMap map_m;   // [out, in] moment dtype, box {32, 128}, swizzle = row bytes
     CUtensorMap map_v;   //   (MODE_STORE_G: map_m is the fp32 G output)
+    CUtensorMap map_m1;  // INT8 only: the same m / v codes with box {128, 64}, SWIZZLE_128B, for the
+    CUtensorMap map_v1;  //   absmax pass that reads whole 256-column rows
     float *m_scale;      // INT8 only: [out, in/256]
     float *v_scale;
     int32_t T, out, in;
@@ -106,16 +108,21 @@ struct KernelCfg {
     static constexpr int M_CHUNK = M_BOXES * M_BOX;
     static constexpr int ST_STAGE = W_CHUNK + 2 * M_CHUNK;
     static constexpr int ST_TX_BYTES = ST_STAGE;
-    static constexpr int kNumBars = 2 * kStages + 4 + 3 * kStateStages;
-    static constexpr int XCHG_BYTES = (MDT == MDT_INT8) ? 4096 : 0;   // absmax exchange, 2 buffers
-    static constexpr int SMEM_BYTES = 1024 /*align slack*/ + kStages * ML_STAGE +
-                                      kStateStages * ST_STAGE + kNumBars * 8 + 16 + XCHG_BYTES;
+    // INT8: a second, read-only ring feeds the absmax pass: chunks of 128 rows x 128 columns of m and
+    // of v codes (one 128 x 128 B box each), two slots = one tile
+    static constexpr int P1_STAGES = (MDT == MDT_INT8) ? 2 : 0;
+    static constexpr int P1_BOX = 128 * 128;
+    static constexpr int P1_STAGE = 2 * P1_BOX;
+    static constexpr int kNumBars = 2 * kStages + 4 + 3 * kStateStages + 2 * P1_STAGES;
+    static constexpr int XCHG_BYTES = (MDT == MDT_INT8) ? 4096 : 0;   // partial row maxima of the two warpgroups, 2 buffers
+    static constexpr int SMEM_BYTES = 1024 /*align slack*/ + kStages * ML_STAGE + kStateStages * ST_STAGE +
+                                      P1_STAGES * P1_STAGE + kNumBars * 8 + 16 + XCHG_BYTES;
     static_assert(SMEM_BYTES <= 232448, "shared memory budget exceeded");
     static_assert(kBlockK % 16 == 0 && kBlockK >= 16, "kBlockK must be a multiple of UMMA_K");
     static_assert(CG == 1 || CG == 2, "CTA group is 1 or 2");
     static_assert(BLOCK_M % CM == 0 && BLOCK_N % CN == 0 && CM % SUB == 0 && CN % SUB == 0, "chunk must tile the tile");
     static_assert(W_BOX % 1024 == 0 && M_BOX % 1024 == 0, "boxes must keep the swizzle pattern aligned");
-    static_assert(MDT != MDT_INT8 || kStateStages >= CHUNKS + PERIOD, "int8 needs a whole tile resident");
+    static_assert(MDT != MDT_INT8 || (CM == 128 && CN == 64), "the int8 path is written for 128 x 64 chunks (one 32-column half per warpgroup)");
     // Chunk ci lives in ring slot ci % kStateStages.  With the ring a multiple of PERIOD every slot is
     // always consumed by the same warps, so a warp observes every phase of the slot barriers it
     // waits on; otherwise it would skip phases and an mbarrier parity wait could alias to a phase
@@ -211,45 +218,48 @@ __device__ __forceinline__ void epi_sub_store_g(const uint32_t (&g)[32], const S
 
 
 // int8 blockwise moments (App. B; 256-element blocks along `in` == one block per tile
-// row).  The new block absmax is only known once all 256 m', v' of the row exist, so the tile is
-// walked twice over the TMEM accumulator and the smem-resident codes: pass 1 finds max|m'|, max v',
-// pass 2 recomputes the identical m', v' (same instructions, same operands), forms W', and emits
-// the codes.  A row is owned by one thread of each warpgroup (even / odd chunks); the two partial
-// maxima are combined through shared memory.
-template <class Cfg, int kStateStages, int CG>
-__device__ __forceinline__ void epi_tile_int8(const KernelParams &P, const AdamWScalars &hp, int tile, uint32_t rank,
-                                              uint32_t titer, uint32_t taddr, uint32_t sST,
-                                              uint32_t bar_st_full, uint32_t bar_st_done, uint32_t quad,
-                                              uint32_t lane, int wg, uint32_t s_xchg) {
-    const TileCoord tc = decode_tile<CG>(P, tile, rank);
-    const ProblemDesc &pd = P.prob[tc.p];
-    const uint32_t row_t = quad * 32 + lane;                 // row of the tile == TMEM lane
-    const uint32_t rb = row_t / Cfg::CM, row = row_t % Cfg::CM;
-    const int row_g = tc.tm * BLOCK_M + static_cast<int>(row_t);
-    const bool valid = row_g < pd.out;
-    const size_t sidx = static_cast<size_t>(valid ? row_g : 0) * static_cast<size_t>(pd.in / BLOCK_N) + tc.tn;
-    const float a_m_old = valid ? pd.m_scale[sidx] : 0.0f;
-    const float a_v_old = valid ? pd.v_scale[sidx] : 0.0f;
-    const float bm = __fmul_rn(hp.beta1, dequant_step(a_m_old, 127.0f));
-    const float bv = __fmul_rn(hp.beta2, dequant_step(a_v_old, 255.0f));
+// row).  The new block absmax is only known once all 256 m', v' of the row exist, and a tile's state
+// (128 KB) cannot be double-buffered in shared memory, so the tile is walked twice over the TMEM
+// accumulator with the state STREAMED both times:
+//   pass 1: the m / v codes of the tile come through a small read-only ring (128 rows x 128 columns
+//       per chunk); m', v' are formed from the accumulator and only the row maxima are kept;
+//   pass 2: W and the codes come through the in-place ring (the codes again: an L2 hit, they were
+//       read microseconds ago); the identical m', v' are recomputed (same instructions, same
+//       operands), W' formed, the state requantised with the new scales and stored in place.
+// A row is owned by one thread of each warpgroup (each takes half of the columns); the two partial
+// maxima are combined through shared memory.  DRAM traffic is unchanged (8.06 B / element);
+// L2 -> SM traffic grows by the 2 B / element of the second code read.
+struct Int8Smem {
+    uint32_t p1, bar_p1_full, bar_p1_empty, xchg;
+};
+struct Int8Row {           // per-thread view of its row's 256-block in the current tile
+    size_t sidx;
+    float bm, bv;          // beta * (old absmax / levels): dequantisation folded into the moment update
+    bool valid;
+};
 
-    // ---- pass 1: block absmax of m', v' over this warp's sub-blocks of the row
-    float pm = 0.0f, pv = 0.0f;
-    for (int cb = 0; cb < Cfg::CB; ++cb) {
-        if (Cfg::SUBS < 2 && (cb & 1) != wg) continue;
-        const uint32_t ci = titer * Cfg::CHUNKS + cb * Cfg::RB + rb;
-        const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
-        mbar_wait(bar_st_full + 8 * s, ph);
-        for (int j32 = (Cfg::SUBS >= 2 ? wg : 0); j32 < Cfg::SUBS; j32 += Cfg::WGS) {
+// pass 1: row maxima of m', v' ("absmax") over this warp's half of the columns
+template <class Cfg>
+__device__ __forceinline__ void int8_pass1(const AdamWScalars &hp, const Int8Row &R, uint32_t titer, uint32_t taddr,
+                                           const Int8Smem &S, uint32_t row_t, int wg, float &pm, float &pv) {
+    pm = 0.0f;
+    pv = 0.0f;
+#pragma unroll 1
+    for (int c1 = 0; c1 < 2; ++c1) {
+        const uint32_t i1 = titer * 2 + c1, s = i1 % Cfg::P1_STAGES, ph = (i1 / Cfg::P1_STAGES) & 1u;
+        const uint32_t am = S.p1 + s * Cfg::P1_STAGE, av = am + Cfg::P1_BOX;
+        mbar_wait(S.bar_p1_full + 8 * s, ph);
+#pragma unroll 1
+        for (int i = 0; i < 2; ++i) {
+            const int j32 = 2 * wg + i;                    // 32-column sub-block of the 128-column chunk
             uint32_t g[32];
-            tmem_ld_32x32b_x32(taddr + cb * Cfg::CN + j32 * SUB, g);
-            const SubAddr<Cfg> a(sST + s * Cfg::ST_STAGE, j32 * SUB);
+            tmem_ld_32x32b_x32(taddr + c1 * 128 + j32 * SUB, g);
+            const uint32_t o0 = swz<128>(row_t, 2 * j32), o1 = swz<128>(row_t, 2 * j32 + 1);
+            const uint4 mq[2] = {lds128(am + o0), lds128(am + o1)}, vq[2] = {lds128(av + o0), lds128(av + o1)};
             tmem_ld_wait();
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
-                const uint32_t o = swz<Cfg::M_ROW>(row, a.pm + j);
-                const uint4 mq = lds128(a.m + o), vq = lds128(a.v + o);
-                const uint32_t mw[4] = {mq.x, mq.y, mq.z, mq.w}, vw[4] = {vq.x, vq.y, vq.z, vq.w};
+                const uint32_t mw[4] = {mq[j].x, mq[j].y, mq[j].z, mq[j].w}, vw[4] = {vq[j].x, vq[j].y, vq[j].z, vq[j].w};
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
                     f32x2 cm[2], cv[2];
@@ -259,74 +269,126 @@ __device__ __forceinline__ void epi_tile_int8(const KernelParams &P, const AdamW
                     for (int e = 0; e < 2; ++e) {
                         const int gi = 16 * j + 4 * q + 2 * e;
                         f32x2 m, v;
-                        adamw_moments2_q(hp, pk2u(g[gi], g[gi + 1]), cm[e], cv[e], bm, bv, m, v);
+                        adamw_moments2_q(hp, pk2u(g[gi], g[gi + 1]), cm[e], cv[e], R.bm, R.bv, m, v);
                         pm = fmaxf(pm, fmaxf(fabsf(lo2(m)), fabsf(hi2(m))));
                         pv = fmaxf(pv, fmaxf(lo2(v), hi2(v)));           // v' >= 0
                     }
                 }
             }
         }
+        mbar_arrive(S.bar_p1_empty + 8 * s);              // the codes have been read: slot reusable
     }
-    // ---- combine the two warpgroups' parts of the row (same TMEM quadrant: warps quad and 4 + quad)
-    const uint32_t xb = s_xchg + (titer & 1u) * 2048u;
-    asm volatile("st.shared.v2.f32 [%0], {%1, %2};\n" ::"r"(xb + (wg * 128u + row_t) * 8u), "f"(pm), "f"(pv) : "memory");
-    asm volatile("bar.sync %0, 64;\n" ::"r"(1u + quad) : "memory");
-    float om, ov;
-    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];\n" : "=f"(om), "=f"(ov) : "r"(xb + ((wg ^ 1) * 128u + row_t) * 8u));
-    const float a_m = fmaxf(pm, om), a_v = fmaxf(pv, ov);
+}
+
+// pass 2: W' and the requantised state for this warp's 32-column half of every chunk
+template <class Cfg, int kStateStages>
+__device__ __forceinline__ void int8_pass2(const AdamWScalars &hp, const Int8Row &R, float a_m, float a_v,
+                                           uint32_t titer, uint32_t taddr, uint32_t sST, uint32_t bar_st_full,
+                                           uint32_t bar_st_done, uint32_t row_t, int half) {
+    const uint32_t rb = row_t / Cfg::CM, row = row_t % Cfg::CM;
+    const float bm = R.bm, bv = R.bv;
     const float inv_m = quant_inv_scale(a_m, 127.0f), inv_v = quant_inv_scale(a_v, 255.0f);
     const float v_floor = quant_v_floor(inv_v);
-
-    // ---- pass 2: recompute (same instructions, same operands), update W, requantise
+#pragma unroll 1
     for (int cb = 0; cb < Cfg::CB; ++cb) {
-        if (Cfg::SUBS < 2 && (cb & 1) != wg) continue;
         const uint32_t ci = titer * Cfg::CHUNKS + cb * Cfg::RB + rb;
-        const uint32_t s = ci % kStateStages;
-        for (int j32 = (Cfg::SUBS >= 2 ? wg : 0); j32 < Cfg::SUBS; j32 += Cfg::WGS) {
-            uint32_t g[32];
-            tmem_ld_32x32b_x32(taddr + cb * Cfg::CN + j32 * SUB, g);
-            const SubAddr<Cfg> a(sST + s * Cfg::ST_STAGE, j32 * SUB);
-            tmem_ld_wait();
+        const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
+        uint32_t g[32];
+        tmem_ld_32x32b_x32(taddr + cb * Cfg::CN + half * SUB, g);
+        const SubAddr<Cfg> a(sST + s * Cfg::ST_STAGE, half * SUB);
+        mbar_wait(bar_st_full + 8 * s, ph);
+        tmem_ld_wait();
 #pragma unroll
-            for (int j = 0; j < 2; ++j) {
-                const uint32_t o = swz<Cfg::M_ROW>(row, a.pm + j);
-                const uint32_t am = a.m + o, av = a.v + o;
-                const uint4 mq = lds128(am), vq = lds128(av);
-                const uint32_t aw0 = a.w + swz<Cfg::W_ROW>(row, a.pw + 2 * j), aw1 = a.w + swz<Cfg::W_ROW>(row, a.pw + 2 * j + 1);
-                const uint4 w0 = lds128(aw0), w1 = lds128(aw1);
-                const uint32_t mw[4] = {mq.x, mq.y, mq.z, mq.w}, vw[4] = {vq.x, vq.y, vq.z, vq.w};
-                const uint32_t ww[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
-                uint32_t mo[4], vo[4], wo[8];
+        for (int j = 0; j < 2; ++j) {
+            const uint32_t o = swz<Cfg::M_ROW>(row, a.pm + j);
+            const uint32_t am = a.m + o, av = a.v + o;
+            const uint4 mq = lds128(am), vq = lds128(av);
+            const uint32_t aw0 = a.w + swz<Cfg::W_ROW>(row, a.pw + 2 * j), aw1 = a.w + swz<Cfg::W_ROW>(row, a.pw + 2 * j + 1);
+            const uint4 w0 = lds128(aw0), w1 = lds128(aw1);
+            const uint32_t mw[4] = {mq.x, mq.y, mq.z, mq.w}, vw[4] = {vq.x, vq.y, vq.z, vq.w};
+            const uint32_t ww[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+            uint32_t mo[4], vo[4], wo[8];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    f32x2 cm[2], cv[2], qm[2], qv[2];
-                    codes4_to_f32(mw[q], true, cm[0], cm[1]);
-                    codes4_to_f32(vw[q], false, cv[0], cv[1]);
+            for (int q = 0; q < 4; ++q) {
+                f32x2 cm[2], cv[2], qm[2], qv[2];
+                codes4_to_f32(mw[q], true, cm[0], cm[1]);
+                codes4_to_f32(vw[q], false, cv[0], cv[1]);
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        const int gi = 16 * j + 4 * q + 2 * e;
-                        f32x2 m, v, w = bf16x2_to_f32x2(ww[2 * q + e]);
-                        adamw_moments2_q(hp, pk2u(g[gi], g[gi + 1]), cm[e], cv[e], bm, bv, m, v);
-                        adamw_weight2(hp, m, v, w);
-                        wo[2 * q + e] = f32x2_to_bf16x2(w);
-                        qm[e] = quant_m2(m, inv_m);
-                        qv[e] = quant_v2(v, inv_v, v_floor);
-                    }
-                    mo[q] = pack_codes4(qm[0], qm[1]);
-                    vo[q] = pack_codes4(qv[0], qv[1]);
+                for (int e = 0; e < 2; ++e) {
+                    const int gi = 16 * j + 4 * q + 2 * e;
+                    f32x2 m, v, w = bf16x2_to_f32x2(ww[2 * q + e]);
+                    adamw_moments2_q(hp, pk2u(g[gi], g[gi + 1]), cm[e], cv[e], bm, bv, m, v);
+                    adamw_weight2(hp, m, v, w);
+                    wo[2 * q + e] = f32x2_to_bf16x2(w);
+                    qm[e] = quant_m2(m, inv_m);
+                    qv[e] = quant_v2(v, inv_v, v_floor);
                 }
-                sts128(am, make_uint4(mo[0], mo[1], mo[2], mo[3]));
-                sts128(av, make_uint4(vo[0], vo[1], vo[2], vo[3]));
-                sts128(aw0, make_uint4(wo[0], wo[1], wo[2], wo[3]));
-                sts128(aw1, make_uint4(wo[4], wo[5], wo[6], wo[7]));
+                mo[q] = pack_codes4(qm[0], qm[1]);
+                vo[q] = pack_codes4(qv[0], qv[1]);
             }
+            sts128(am, make_uint4(mo[0], mo[1], mo[2], mo[3]));
+            sts128(av, make_uint4(vo[0], vo[1], vo[2], vo[3]));
+            sts128(aw0, make_uint4(wo[0], wo[1], wo[2], wo[3]));
+            sts128(aw1, make_uint4(wo[4], wo[5], wo[6], wo[7]));
         }
         fence_proxy_async_smem();
         mbar_arrive(bar_st_done + 8 * s);
     }
-    if (wg == 0 && valid) {
-        pd.m_scale[sidx] = a_m;
-        pd.v_scale[sidx] = a_v;
+}
+
+template <int CG>
+__device__ __forceinline__ Int8Row int8_row(const KernelParams &P, const AdamWScalars &hp, int tile, uint32_t rank,
+                                            uint32_t row_t) {
+    const TileCoord tc = decode_tile<CG>(P, tile, rank);
+    const ProblemDesc &pd = P.prob[tc.p];
+    const int row_g = tc.tm * BLOCK_M + static_cast<int>(row_t);
+    Int8Row R;
+    R.valid = row_g < pd.out;
+    R.sidx = static_cast<size_t>(R.valid ? row_g : 0) * static_cast<size_t>(pd.in / BLOCK_N) + tc.tn;
+    R.bm = __fmul_rn(hp.beta1, dequant_step(R.valid ? pd.m_scale[R.sidx] : 0.0f, 127.0f));
+    R.bv = __fmul_rn(hp.beta2, dequant_step(R.valid ? pd.v_scale[R.sidx] : 0.0f, 255.0f));
+    return R;
+}
+
+// int8 state loader: one thread feeds both rings, polling whichever has a free slot
+template <class Cfg, int kStateStages, int CG>
+__device__ __forceinline__ void int8_loader(const KernelParams &P, uint32_t rank, int first_tile, int tile_step,
+                                            uint32_t sST, uint32_t bar_st_full, uint32_t bar_st_empty,
+                                            const Int8Smem &S) {
+    if (first_tile >= P.total_tiles) return;
+    const uint32_t my_tiles = (P.total_tiles - first_tile + tile_step - 1) / tile_step;
+    const uint32_t n1 = my_tiles * 2, n2 = my_tiles * Cfg::CHUNKS;
+    uint32_t i1 = 0, i2 = 0;
+    TileCoord tc1 = decode_tile<CG>(P, first_tile, rank), tc2 = tc1;
+    while (i1 < n1 || i2 < n2) {
+        if (i1 < n1) {
+            const uint32_t s = i1 % Cfg::P1_STAGES, ph = (i1 / Cfg::P1_STAGES) & 1u;
+            if (mbar_test_wait(S.bar_p1_empty + 8 * s, ph ^ 1u)) {
+                if ((i1 % 2) == 0 && i1 > 0) tc1 = decode_tile<CG>(P, first_tile + (i1 / 2) * tile_step, rank);
+                const ProblemDesc &pd = P.prob[tc1.p];
+                const uint32_t full = S.bar_p1_full + 8 * s, base = S.p1 + s * Cfg::P1_STAGE;
+                mbar_expect_tx(full, Cfg::P1_STAGE);
+                const int x = tc1.tn * BLOCK_N + (i1 % 2) * 128, y = tc1.tm * BLOCK_M;
+                tma_load_2d(base, &pd.map_m1, full, x, y, kEvictNormal);
+                tma_load_2d(base + Cfg::P1_BOX, &pd.map_v1, full, x, y, kEvictNormal);
+                ++i1;
+            }
+        }
+        if (i2 < n2) {
+            const uint32_t s = i2 % kStateStages, ph = (i2 / kStateStages) & 1u;
+            if (mbar_test_wait(bar_st_empty + 8 * s, ph ^ 1u)) {
+                const uint32_t c = i2 % Cfg::CHUNKS;
+                if (c == 0 && i2 > 0) tc2 = decode_tile<CG>(P, first_tile + (i2 / Cfg::CHUNKS) * tile_step, rank);
+                const ProblemDesc &pd = P.prob[tc2.p];
+                const uint32_t full = bar_st_full + 8 * s, base = sST + s * Cfg::ST_STAGE;
+                mbar_expect_tx(full, Cfg::ST_TX_BYTES);
+                const int x = tc2.tn * BLOCK_N + (c / Cfg::RB) * Cfg::CN, y = tc2.tm * BLOCK_M + (c % Cfg::RB) * Cfg::CM;
+                tma_load_2d(base, &pd.map_W, full, x, y, kEvictFirst);
+                tma_load_2d(base + Cfg::W_CHUNK, &pd.map_m, full, x, y, kEvictFirst);
+                tma_load_2d(base + Cfg::W_CHUNK + Cfg::M_CHUNK, &pd.map_v, full, x, y, kEvictFirst);
+                ++i2;
+            }
+        }
     }
 }
 
@@ -334,7 +396,7 @@ __device__ __forceinline__ void epi_tile_int8(const KernelParams &P, const AdamW
 // the kernel
 // ---------------------------------------------------------------------------------------------
 template <int MDT, int MODE, int kBlockK, int kStages, int kStateStages, int CG, int CM, int CN>
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __launch_bounds__(block_threads(MDT), 1)
 forge_fused_kernel(const __grid_constant__ KernelParams P) {
     using Cfg = KernelCfg<MDT, kBlockK, kStages, kStateStages, CG, CM, CN>;
     constexpr int CHUNKS = Cfg::CHUNKS;
@@ -343,7 +405,8 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t sML = smem_base;                                   // mainloop ring
     const uint32_t sST = sML + kStages * Cfg::ML_STAGE;               // state ring
-    const uint32_t sBAR = sST + kStateStages * Cfg::ST_STAGE;         // mbarriers
+    const uint32_t sP1 = sST + kStateStages * Cfg::ST_STAGE;          // INT8: first-pass code ring
+    const uint32_t sBAR = sP1 + Cfg::P1_STAGES * Cfg::P1_STAGE;       // mbarriers
     // barrier map
     const uint32_t bar_ml_full = sBAR;
     const uint32_t bar_ml_empty = bar_ml_full + 8 * kStages;
@@ -352,8 +415,10 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
     const uint32_t bar_st_full = bar_tm_empty + 16;
     const uint32_t bar_st_done = bar_st_full + 8 * kStateStages;
     const uint32_t bar_st_empty = bar_st_done + 8 * kStateStages;
-    const uint32_t s_tmem_ptr = bar_st_empty + 8 * kStateStages;
-    const uint32_t s_xchg = s_tmem_ptr + 16;
+    const uint32_t bar_p1_full = bar_st_empty + 8 * kStateStages;     // INT8 only [P1_STAGES]
+    const uint32_t bar_p1_empty = bar_p1_full + 8 * Cfg::P1_STAGES;
+    const uint32_t s_tmem_ptr = bar_p1_empty + 8 * Cfg::P1_STAGES;
+    const Int8Smem i8{sP1, bar_p1_full, bar_p1_empty, s_tmem_ptr + 16};
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -365,12 +430,16 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         }
         for (int i = 0; i < 2; ++i) {
             mbar_init(bar_tm_full + 8 * i, 1);
-            mbar_init(bar_tm_empty + 8 * i, kEpiWarps * CG);   // one arrival per epilogue warp of the pair
+            mbar_init(bar_tm_empty + 8 * i, epi_warps(MDT) * CG);   // one arrival per epilogue warp of the pair
         }
         for (int i = 0; i < kStateStages; ++i) {
             mbar_init(bar_st_full + 8 * i, 1);
             mbar_init(bar_st_done + 8 * i, Cfg::DONE_COUNT);
             mbar_init(bar_st_empty + 8 * i, 1);
+        }
+        for (int i = 0; i < Cfg::P1_STAGES; ++i) {
+            mbar_init(bar_p1_full + 8 * i, 1);
+            mbar_init(bar_p1_empty + 8 * i, 256);     // every epilogue thread reads its part of the chunk
         }
         mbar_fence_init();
     }
@@ -463,7 +532,9 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         }
     } else if (warp == 2) {
         // ================= state loader (Alg. 1 line 6: load W_ij, m_ij, v_ij) ===================
-        if (MODE == MODE_ADAMW && lane == 0 && !(P.debug & DBG_NO_STATE)) {
+        if constexpr (MDT == MDT_INT8) {
+            if (lane == 0) int8_loader<Cfg, kStateStages, CG>(P, rank, first_tile, tile_step, sST, bar_st_full, bar_st_empty, i8);
+        } else if (MODE == MODE_ADAMW && lane == 0 && !(P.debug & DBG_NO_STATE)) {
             uint32_t ci = 0;  // running chunk counter
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step) {
                 const TileCoord tc = decode_tile<CG>(P, tile, rank);
@@ -546,6 +617,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         const uint32_t row_t = quad * 32 + lane;      // row of the tile == TMEM lane
         const uint32_t rb = row_t / CM, row = row_t % CM;   // this warp's row block, row inside the chunk
         const AdamWScalars hp = P.hp;
+        Int8Row i8row{};
         uint32_t titer = 0;
         for (int tile = first_tile; tile < P.total_tiles; tile += tile_step, ++titer) {
             const uint32_t as = titer & 1u, aph = (titer >> 1) & 1u;
@@ -575,8 +647,25 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                     mbar_arrive(bar_st_done + 8 * s);
                 }
             } else {
-                epi_tile_int8<Cfg, kStateStages, CG>(P, hp, tile, rank, titer, taddr, sST, bar_st_full,
-                                                     bar_st_done, quad, lane, wg, s_xchg);
+                // old block scales of this row: loaded one tile ahead (global latency off the critical path)
+                if (titer == 0) i8row = int8_row<CG>(P, hp, tile, rank, row_t);
+                const Int8Row R = i8row;
+                if (tile + tile_step < P.total_tiles) i8row = int8_row<CG>(P, hp, tile + tile_step, rank, row_t);
+                float pm, pv;
+                int8_pass1<Cfg>(hp, R, titer, taddr, i8, row_t, wg, pm, pv);
+                // combine the two warpgroups' halves of the row (same TMEM quadrant: warps quad and 4 + quad)
+                const uint32_t xb = i8.xchg + (titer & 1u) * 2048u;
+                asm volatile("st.shared.v2.f32 [%0], {%1, %2};\n" ::"r"(xb + (wg * 128u + row_t) * 8u), "f"(pm), "f"(pv) : "memory");
+                asm volatile("bar.sync %0, 64;\n" ::"r"(1u + quad) : "memory");
+                float om, ov;
+                asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];\n" : "=f"(om), "=f"(ov) : "r"(xb + ((wg ^ 1) * 128u + row_t) * 8u));
+                const float a_m = fmaxf(pm, om), a_v = fmaxf(pv, ov);
+                int8_pass2<Cfg, kStateStages>(hp, R, a_m, a_v, titer, taddr, sST, bar_st_full, bar_st_done, row_t, wg);
+                if (wg == 0 && R.valid) {
+                    const ProblemDesc &pd = P.prob[decode_tile<CG>(P, tile, rank).p];
+                    pd.m_scale[R.sidx] = a_m;
+                    pd.v_scale[R.sidx] = a_v;
+                }
             }
             // this warp has drained the accumulator: tell the (leader's) MMA issuer
             tc_fence_before();

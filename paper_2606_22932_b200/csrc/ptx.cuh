@@ -212,8 +212,11 @@ __device__ __forceinline__ uint32_t mapa_shared(uint32_t addr, uint32_t rank) {
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;\n" : "=r"(r) : "r"(addr), "r"(rank));
     return r;
 }
+// Default semantics (release at CTA scope): what is handed over with this arrive is the TMEM
+// accumulator, ordered by tcgen05.fence::before_thread_sync; a cluster-scope release would add a
+// MEMBAR.ALL.CTA + ERRBAR that waits for every outstanding shared-memory store of the warp.
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];\n" ::"r"(cluster_addr) : "memory");
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];\n" ::"r"(cluster_addr) : "memory");
 }
 // CTA-pair TMA load: data lands in this CTA's smem, the transaction bytes are signalled on the
 // (possibly remote) mbarrier `bar_cluster` of the pair's leader CTA.
