@@ -33,7 +33,7 @@ MOMENT_ENUM = {"fp32": 0, "bf16": 1, "int8": 2}
 T_TOKENS = 512
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed
 # ncu --set full capture (profiles/); None until a capture of the current kernel exists.
-NCU_TRAFFIC_BYTES = {"fp32": 4530391000, "bf16": None, "int8": None}
+NCU_TRAFFIC_BYTES = {"fp32": 4376165000, "bf16": 2747416000, "int8": 1868895000}
 
 
 def measured_peaks():
@@ -172,8 +172,8 @@ def oracle_time_sample(frac_den: int, seed: int):
 def cpu_baseline(seed: int):
     den = 16
     dt, desc, threads = oracle_time_sample(den, seed)
-    if dt * 4 < 20.0:                      # aim at ~10-30 s of CPU work
-        den = 4
+    while den > 1 and dt * 4 < 30.0:       # aim at ~10-30 s of CPU work: 1/16, 1/4, then the whole layer
+        den //= 4
         dt, desc, threads = oracle_time_sample(den, seed)
     return {"value": dt * den * 1e6, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
             "sample_seconds": round(dt, 3)}

@@ -147,11 +147,11 @@ int env_int(const char *name, int dflt) {
 // ---------------------------------------------------------------------------------------------
 // launch of one fused-kernel instantiation over <= kMaxProblems problems
 // ---------------------------------------------------------------------------------------------
-template <int MDT, int MODE, int BK, int ST, int SS, int CG = 1, int CM = 64, int CN = 64>
+template <int MDT, int MODE, int BK, int ST, int SS, int CG = 1, int CM = 64, int CN = 64, int P1C = 128, int P1S = 2>
 forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamWScalars &hp,
                             const DeviceInfo &dev, cudaStream_t stream) {
-    using Cfg = KernelCfg<MDT, BK, ST, SS, CG, CM, CN>;
-    auto kernel = forge_fused_kernel<MDT, MODE, BK, ST, SS, CG, CM, CN>;
+    using Cfg = KernelCfg<MDT, BK, ST, SS, CG, CM, CN, P1C, P1S>;
+    auto kernel = forge_fused_kernel<MDT, MODE, BK, ST, SS, CG, CM, CN, P1C, P1S>;
     static std::once_flag once;
     static cudaError_t attr_err = cudaSuccess;
     std::call_once(once, [&] {
@@ -181,8 +181,8 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
             ok &= encode_2d(&d.map_v, mom_dt, Cfg::kMomBytes, p.v, p.out, p.in, Cfg::M_BOX_COLS, CM,
                             swizzle_for_row_bytes(Cfg::M_ROW));
             if (MDT == MDT_INT8) {   // first-pass view of the same codes: 128 rows x 128 columns per box
-                ok &= encode_2d(&d.map_m1, mom_dt, 1, p.m, p.out, p.in, 128, 128, CU_TENSOR_MAP_SWIZZLE_128B);
-                ok &= encode_2d(&d.map_v1, mom_dt, 1, p.v, p.out, p.in, 128, 128, CU_TENSOR_MAP_SWIZZLE_128B);
+                ok &= encode_2d(&d.map_m1, mom_dt, 1, p.m, p.out, p.in, P1C, 128, swizzle_for_row_bytes(P1C));
+                ok &= encode_2d(&d.map_v1, mom_dt, 1, p.v, p.out, p.in, P1C, 128, swizzle_for_row_bytes(P1C));
             }
         } else {  // store-G twin: p.m carries the fp32 G output
             ok &= encode_2d(&d.map_m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, p.m, p.out, p.in, Cfg::M_BOX_COLS, CM,
@@ -261,17 +261,20 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
         case 3: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 2, 4, 2, 64, 128>(probs, count, hp, dev, stream);
         case 4: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 2, 4, 2, 32, 256>(probs, count, hp, dev, stream);
         case 5: return launch_fused<MDT_BF16, MODE_ADAMW, 64, 4, 2, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 6: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 6: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 6, 2, 64, 64>(probs, count, hp, dev, stream);
         case 7: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 2, 2, 64, 128>(probs, count, hp, dev, stream);
-        default: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 6, 2, 64, 64>(probs, count, hp, dev, stream);
+        default: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
         }
     case FORGE_MOMENT_INT8:
         switch (variant) {
-        case 1: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 2, 3, 1, 128, 64>(probs, count, hp, dev, stream);
-        case 2: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 2, 2, 128, 64>(probs, count, hp, dev, stream);
-        case 3: return launch_fused<MDT_INT8, MODE_ADAMW, 16, 3, 4, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 1: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 2, 2, 1, 128, 64>(probs, count, hp, dev, stream);
+        case 2: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 3, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 3: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 4, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
+        case 4: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 2, 4, 2, 128, 64, 64, 3>(probs, count, hp, dev, stream);
         case 5: return launch_fused<MDT_INT8, MODE_ADAMW, 64, 2, 2, 2, 128, 64>(probs, count, hp, dev, stream);
-        default: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 3, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 6: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 2, 2, 128, 64, 64, 4>(probs, count, hp, dev, stream);
+        case 7: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 4, 2, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
+        default: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 2, 2, 128, 64>(probs, count, hp, dev, stream);
         }
     default:
         return FORGE_ERR_BAD_DTYPE;

@@ -37,7 +37,12 @@ constexpr int BLOCK_M = 128;   // tile rows  (out)  = TMEM lanes
 constexpr int BLOCK_N = 256;   // tile cols  (in)   = TMEM columns = one int8 block per row
 constexpr int SUB = 32;        // epilogue sub-block: 32 rows (one warp's TMEM lanes) x 32 columns
 constexpr int kCtrlWarps = 4;
-__host__ __device__ constexpr int epi_warps(int) { return 8; }
+#ifndef FORGE_INT8_WARPS_PER_QUAD
+#define FORGE_INT8_WARPS_PER_QUAD 2
+#endif
+// int8: warps per TMEM quadrant sharing a row (2 = the two warpgroups; 3 measured slower: 485 vs 461 us/layer)
+constexpr int kI8W = FORGE_INT8_WARPS_PER_QUAD;
+__host__ __device__ constexpr int epi_warps(int mdt) { return mdt == 2 /*MDT_INT8*/ ? 4 * kI8W : 8; }
 __host__ __device__ constexpr int block_threads(int mdt) { return (kCtrlWarps + epi_warps(mdt)) * 32; }
 constexpr int kTmemCols = 512;  // 2 accumulator buffers x 256 fp32 columns
 
@@ -78,10 +83,10 @@ enum : int { DBG_NO_MAINLOOP = 1, DBG_NO_STATE = 2, DBG_NO_EPILOGUE = 4 };
 // (L2 -> SM traffic and smem per stage), the state path stays CTA-local.
 // State chunk geometry.  The state stream (W, m, v once in, once out) is the roofline of the
 // HBM-bound shapes, and what it achieves depends on the chunk shape more than on the depth of the
-// ring: a probe that only streams W/m/v through TMA in place (profiles/r01_state_stream_probe.md)
-// reaches 5.3 TB/s with 128 x 32 chunks and 6.0 TB/s with 64 x 64 chunks at the same 160 KB of ring
-// (longer contiguous runs per DRAM page, fewer pages open at once).
-template <int MDT, int kBlockK, int kStages, int kStateStages, int CG = 1, int CM_ = 64, int CN_ = 64>
+// ring: with fp32 moments 128 x 32 chunks x 4 slots give 0.83 of the copy peak, 64 x 64 x 4 slots 0.86
+// and 64 x 128 x 2 slots 0.90 (profiles/r01_summary.md) -- longer contiguous runs per DRAM page and
+// fewer pages open at once matter more than bytes in flight.
+template <int MDT, int kBlockK, int kStages, int kStateStages, int CG = 1, int CM_ = 64, int CN_ = 64, int P1C_ = 128, int P1S_ = 2>
 struct KernelCfg {
     static constexpr int kMomBytes = (MDT == MDT_FP32) ? 4 : (MDT == MDT_BF16 ? 2 : 1);
     static constexpr int A_STAGE = kBlockK * 128 * (BLOCK_M / 64);
@@ -94,7 +99,7 @@ struct KernelCfg {
     static constexpr int WGS = SUBS >= 2 ? 2 : 1;           // warpgroups that share one chunk
     // chunks ci and ci + PERIOD are consumed by the same warps
     static constexpr int PERIOD = RB * (SUBS >= 2 ? 1 : 2);
-    static constexpr int DONE_COUNT = (CM / SUB) * WGS * 32;
+    static constexpr int DONE_COUNT = (CM / SUB) * (MDT == MDT_INT8 ? kI8W : WGS) * 32;
     // TMA boxes: at most 128 B per row (one swizzle span), CM rows
     static constexpr int W_BOX_COLS = CN < 64 ? CN : 64;
     static constexpr int W_ROW = W_BOX_COLS * 2;
@@ -110,11 +115,13 @@ struct KernelCfg {
     static constexpr int ST_TX_BYTES = ST_STAGE;
     // INT8: a second, read-only ring feeds the absmax pass: chunks of 128 rows x 128 columns of m and
     // of v codes (one 128 x 128 B box each), two slots = one tile
-    static constexpr int P1_STAGES = (MDT == MDT_INT8) ? 2 : 0;
-    static constexpr int P1_BOX = 128 * 128;
+    static constexpr int P1_COLS = P1C_;                       // 128 or 64 columns per chunk (row bytes = swizzle span)
+    static constexpr int P1_CHUNKS = BLOCK_N / P1_COLS;
+    static constexpr int P1_STAGES = (MDT == MDT_INT8) ? P1S_ : 0;
+    static constexpr int P1_BOX = 128 * P1_COLS;
     static constexpr int P1_STAGE = 2 * P1_BOX;
     static constexpr int kNumBars = 2 * kStages + 4 + 3 * kStateStages + 2 * P1_STAGES;
-    static constexpr int XCHG_BYTES = (MDT == MDT_INT8) ? 4096 : 0;   // partial row maxima of the two warpgroups, 2 buffers
+    static constexpr int XCHG_BYTES = (MDT == MDT_INT8) ? 2 * kI8W * 1024 : 0;   // partial row maxima of the warps sharing a row, 2 buffers
     static constexpr int SMEM_BYTES = 1024 /*align slack*/ + kStages * ML_STAGE + kStateStages * ST_STAGE +
                                       P1_STAGES * P1_STAGE + kNumBars * 8 + 16 + XCHG_BYTES;
     static_assert(SMEM_BYTES <= 232448, "shared memory budget exceeded");
@@ -232,29 +239,37 @@ __device__ __forceinline__ void epi_sub_store_g(const uint32_t (&g)[32], const S
 struct Int8Smem {
     uint32_t p1, bar_p1_full, bar_p1_empty, xchg;
 };
-struct Int8Row {           // per-thread view of its row's 256-block in the current tile
+struct Int8Row {           // per-thread view of its row's 256-block in one tile
     size_t sidx;
+    float a_m, a_v;        // old block absmax as stored (loaded a tile ahead; no arithmetic on them until used)
     float bm, bv;          // beta * (old absmax / levels): dequantisation folded into the moment update
     bool valid;
+    __device__ __forceinline__ void finish(const AdamWScalars &hp) {
+        bm = __fmul_rn(hp.beta1, dequant_step(a_m, 127.0f));
+        bv = __fmul_rn(hp.beta2, dequant_step(a_v, 255.0f));
+    }
 };
 
 // pass 1: row maxima of m', v' ("absmax") over this warp's half of the columns
 template <class Cfg>
 __device__ __forceinline__ void int8_pass1(const AdamWScalars &hp, const Int8Row &R, uint32_t titer, uint32_t taddr,
-                                           const Int8Smem &S, uint32_t row_t, int wg, float &pm, float &pv) {
+                                           const Int8Smem &S, uint32_t row_t, int wg, float &pm, float &pv,
+                                           bool skip_math) {
     pm = 0.0f;
     pv = 0.0f;
+    constexpr int kSubs = Cfg::P1_COLS / SUB;              // 32-column sub-blocks per chunk; sub-block t of the
+                                                           // row goes to warp t % kI8W of the quadrant
 #pragma unroll 1
-    for (int c1 = 0; c1 < 2; ++c1) {
-        const uint32_t i1 = titer * 2 + c1, s = i1 % Cfg::P1_STAGES, ph = (i1 / Cfg::P1_STAGES) & 1u;
+    for (int c1 = 0; c1 < Cfg::P1_CHUNKS; ++c1) {
+        const uint32_t i1 = titer * Cfg::P1_CHUNKS + c1, s = i1 % Cfg::P1_STAGES, ph = (i1 / Cfg::P1_STAGES) & 1u;
         const uint32_t am = S.p1 + s * Cfg::P1_STAGE, av = am + Cfg::P1_BOX;
         mbar_wait(S.bar_p1_full + 8 * s, ph);
 #pragma unroll 1
-        for (int i = 0; i < 2; ++i) {
-            const int j32 = 2 * wg + i;                    // 32-column sub-block of the 128-column chunk
+        for (int j32 = 0; j32 < (skip_math ? 0 : kSubs); ++j32) {
+            if ((c1 * kSubs + j32) % kI8W != wg) continue;
             uint32_t g[32];
-            tmem_ld_32x32b_x32(taddr + c1 * 128 + j32 * SUB, g);
-            const uint32_t o0 = swz<128>(row_t, 2 * j32), o1 = swz<128>(row_t, 2 * j32 + 1);
+            tmem_ld_32x32b_x32(taddr + c1 * Cfg::P1_COLS + j32 * SUB, g);
+            const uint32_t o0 = swz<Cfg::P1_COLS>(row_t, 2 * j32), o1 = swz<Cfg::P1_COLS>(row_t, 2 * j32 + 1);
             const uint4 mq[2] = {lds128(am + o0), lds128(am + o1)}, vq[2] = {lds128(av + o0), lds128(av + o1)};
             tmem_ld_wait();
 #pragma unroll
@@ -284,7 +299,7 @@ __device__ __forceinline__ void int8_pass1(const AdamWScalars &hp, const Int8Row
 template <class Cfg, int kStateStages>
 __device__ __forceinline__ void int8_pass2(const AdamWScalars &hp, const Int8Row &R, float a_m, float a_v,
                                            uint32_t titer, uint32_t taddr, uint32_t sST, uint32_t bar_st_full,
-                                           uint32_t bar_st_done, uint32_t row_t, int half) {
+                                           uint32_t bar_st_done, uint32_t row_t, int wg, bool skip_math) {
     const uint32_t rb = row_t / Cfg::CM, row = row_t % Cfg::CM;
     const float bm = R.bm, bv = R.bv;
     const float inv_m = quant_inv_scale(a_m, 127.0f), inv_v = quant_inv_scale(a_v, 255.0f);
@@ -293,10 +308,13 @@ __device__ __forceinline__ void int8_pass2(const AdamWScalars &hp, const Int8Row
     for (int cb = 0; cb < Cfg::CB; ++cb) {
         const uint32_t ci = titer * Cfg::CHUNKS + cb * Cfg::RB + rb;
         const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
+        mbar_wait(bar_st_full + 8 * s, ph);
+#pragma unroll 1
+        for (int half = 0; half < Cfg::SUBS; ++half) {
+        if (skip_math || (cb * Cfg::SUBS + half) % kI8W != wg) continue;
         uint32_t g[32];
         tmem_ld_32x32b_x32(taddr + cb * Cfg::CN + half * SUB, g);
         const SubAddr<Cfg> a(sST + s * Cfg::ST_STAGE, half * SUB);
-        mbar_wait(bar_st_full + 8 * s, ph);
         tmem_ld_wait();
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
@@ -331,6 +349,7 @@ __device__ __forceinline__ void int8_pass2(const AdamWScalars &hp, const Int8Row
             sts128(aw0, make_uint4(wo[0], wo[1], wo[2], wo[3]));
             sts128(aw1, make_uint4(wo[4], wo[5], wo[6], wo[7]));
         }
+        }
         fence_proxy_async_smem();
         mbar_arrive(bar_st_done + 8 * s);
     }
@@ -345,8 +364,9 @@ __device__ __forceinline__ Int8Row int8_row(const KernelParams &P, const AdamWSc
     Int8Row R;
     R.valid = row_g < pd.out;
     R.sidx = static_cast<size_t>(R.valid ? row_g : 0) * static_cast<size_t>(pd.in / BLOCK_N) + tc.tn;
-    R.bm = __fmul_rn(hp.beta1, dequant_step(R.valid ? pd.m_scale[R.sidx] : 0.0f, 127.0f));
-    R.bv = __fmul_rn(hp.beta2, dequant_step(R.valid ? pd.v_scale[R.sidx] : 0.0f, 255.0f));
+    R.a_m = R.valid ? pd.m_scale[R.sidx] : 0.0f;
+    R.a_v = R.valid ? pd.v_scale[R.sidx] : 0.0f;
+    R.bm = R.bv = 0.0f;
     return R;
 }
 
@@ -357,18 +377,18 @@ __device__ __forceinline__ void int8_loader(const KernelParams &P, uint32_t rank
                                             const Int8Smem &S) {
     if (first_tile >= P.total_tiles) return;
     const uint32_t my_tiles = (P.total_tiles - first_tile + tile_step - 1) / tile_step;
-    const uint32_t n1 = my_tiles * 2, n2 = my_tiles * Cfg::CHUNKS;
+    const uint32_t n1 = my_tiles * Cfg::P1_CHUNKS, n2 = my_tiles * Cfg::CHUNKS;
     uint32_t i1 = 0, i2 = 0;
     TileCoord tc1 = decode_tile<CG>(P, first_tile, rank), tc2 = tc1;
     while (i1 < n1 || i2 < n2) {
         if (i1 < n1) {
             const uint32_t s = i1 % Cfg::P1_STAGES, ph = (i1 / Cfg::P1_STAGES) & 1u;
             if (mbar_test_wait(S.bar_p1_empty + 8 * s, ph ^ 1u)) {
-                if ((i1 % 2) == 0 && i1 > 0) tc1 = decode_tile<CG>(P, first_tile + (i1 / 2) * tile_step, rank);
+                if ((i1 % Cfg::P1_CHUNKS) == 0 && i1 > 0) tc1 = decode_tile<CG>(P, first_tile + (i1 / Cfg::P1_CHUNKS) * tile_step, rank);
                 const ProblemDesc &pd = P.prob[tc1.p];
                 const uint32_t full = S.bar_p1_full + 8 * s, base = S.p1 + s * Cfg::P1_STAGE;
                 mbar_expect_tx(full, Cfg::P1_STAGE);
-                const int x = tc1.tn * BLOCK_N + (i1 % 2) * 128, y = tc1.tm * BLOCK_M;
+                const int x = tc1.tn * BLOCK_N + (i1 % Cfg::P1_CHUNKS) * Cfg::P1_COLS, y = tc1.tm * BLOCK_M;
                 tma_load_2d(base, &pd.map_m1, full, x, y, kEvictNormal);
                 tma_load_2d(base + Cfg::P1_BOX, &pd.map_v1, full, x, y, kEvictNormal);
                 ++i1;
@@ -395,10 +415,10 @@ __device__ __forceinline__ void int8_loader(const KernelParams &P, uint32_t rank
 // ---------------------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------------------
-template <int MDT, int MODE, int kBlockK, int kStages, int kStateStages, int CG, int CM, int CN>
+template <int MDT, int MODE, int kBlockK, int kStages, int kStateStages, int CG, int CM, int CN, int P1C, int P1S>
 __global__ void __launch_bounds__(block_threads(MDT), 1)
 forge_fused_kernel(const __grid_constant__ KernelParams P) {
-    using Cfg = KernelCfg<MDT, kBlockK, kStages, kStateStages, CG, CM, CN>;
+    using Cfg = KernelCfg<MDT, kBlockK, kStages, kStateStages, CG, CM, CN, P1C, P1S>;
     constexpr int CHUNKS = Cfg::CHUNKS;
     const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;   // rank 0 = the pair's leader
     extern __shared__ uint8_t smem_raw[];
@@ -439,7 +459,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         }
         for (int i = 0; i < Cfg::P1_STAGES; ++i) {
             mbar_init(bar_p1_full + 8 * i, 1);
-            mbar_init(bar_p1_empty + 8 * i, 256);     // every epilogue thread reads its part of the chunk
+            mbar_init(bar_p1_empty + 8 * i, epi_warps(MDT) * 32);     // every epilogue thread reads its part of the chunk
         }
         mbar_fence_init();
     }
@@ -649,18 +669,25 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
             } else {
                 // old block scales of this row: loaded one tile ahead (global latency off the critical path)
                 if (titer == 0) i8row = int8_row<CG>(P, hp, tile, rank, row_t);
-                const Int8Row R = i8row;
+                Int8Row R = i8row;
                 if (tile + tile_step < P.total_tiles) i8row = int8_row<CG>(P, hp, tile + tile_step, rank, row_t);
+                R.finish(hp);
                 float pm, pv;
-                int8_pass1<Cfg>(hp, R, titer, taddr, i8, row_t, wg, pm, pv);
+                int8_pass1<Cfg>(hp, R, titer, taddr, i8, row_t, wg, pm, pv, (P.debug & DBG_NO_EPILOGUE) != 0);
                 // combine the two warpgroups' halves of the row (same TMEM quadrant: warps quad and 4 + quad)
-                const uint32_t xb = i8.xchg + (titer & 1u) * 2048u;
+                const uint32_t xb = i8.xchg + (titer & 1u) * (kI8W * 1024u);
                 asm volatile("st.shared.v2.f32 [%0], {%1, %2};\n" ::"r"(xb + (wg * 128u + row_t) * 8u), "f"(pm), "f"(pv) : "memory");
-                asm volatile("bar.sync %0, 64;\n" ::"r"(1u + quad) : "memory");
-                float om, ov;
-                asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];\n" : "=f"(om), "=f"(ov) : "r"(xb + ((wg ^ 1) * 128u + row_t) * 8u));
-                const float a_m = fmaxf(pm, om), a_v = fmaxf(pv, ov);
-                int8_pass2<Cfg, kStateStages>(hp, R, a_m, a_v, titer, taddr, sST, bar_st_full, bar_st_done, row_t, wg);
+                asm volatile("bar.sync %0, %1;\n" ::"r"(1u + quad), "n"(kI8W * 32) : "memory");
+                float a_m = pm, a_v = pv;
+#pragma unroll
+                for (int o = 1; o < kI8W; ++o) {
+                    float om, ov;
+                    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];\n" : "=f"(om), "=f"(ov) : "r"(xb + (((wg + o) % kI8W) * 128u + row_t) * 8u));
+                    a_m = fmaxf(a_m, om);
+                    a_v = fmaxf(a_v, ov);
+                }
+                int8_pass2<Cfg, kStateStages>(hp, R, a_m, a_v, titer, taddr, sST, bar_st_full, bar_st_done, row_t, wg,
+                                              (P.debug & DBG_NO_EPILOGUE) != 0);
                 if (wg == 0 && R.valid) {
                     const ProblemDesc &pd = P.prob[decode_tile<CG>(P, tile, rank).p];
                     pd.m_scale[R.sidx] = a_m;
