@@ -262,7 +262,64 @@ def time_unfused_baselines(layer, hp, steps):
     return res
 
 
+def run_model(args):
+    """BASELINE.json configs[4]: 32 layers + lm_head resident (75 GB of state), one optimizer step layer by
+    layer in reverse order; total step time and peak device memory with and without a materialised dW pool."""
+    import torch
+    from paper_2606_22932_b200 import binding as fb
+    from paper_2606_22932_b200 import stack, synth
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    fb.lib()
+    hp = synth.HP_DEFAULT
+    free0, total = torch.cuda.mem_get_info()
+    st = stack.build_stack(dev, tokens=args.tokens)
+    torch.cuda.synchronize()
+    stream = torch.cuda.current_stream()
+
+    def timed(fn, n, warm):
+        for i in range(warm):
+            fn(1 + i)
+        torch.cuda.synchronize()
+        torch.cuda.reset_peak_memory_stats()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for i in range(n):
+            fn(1 + warm + i)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n, torch.cuda.max_memory_allocated()
+
+    n = max(1, min(args.steps, 5))
+    launches0 = fb.forge_launch_count()
+    fused_ms, fused_peak = timed(lambda t: stack.step_fused(st, t, hp, stream), n, 1)
+    launches = (fb.forge_launch_count() - launches0) // (n + 1)
+    alg_bytes = st.params * 20.0 + st.input_bytes
+    hbm_peak, tf_burst, tf_sus, peak_src = measured_peaks()
+    pool = stack.alloc_dw_pool(st, dev)
+    pool_bytes = sum(g.numel() * 4 for layer in pool for g in layer)
+    pool_ms, pool_peak = timed(lambda t: stack.step_dw_pool(st, pool, t, hp), max(1, n // 2), 1)
+    gbs = alg_bytes / (fused_ms * 1e-3) / 1e9
+    line = {"metric": "full Llama-3.1-8B linear stack optimizer step, ms (32 layers + lm_head, BT=%d, 1xB200)" % args.tokens,
+            "value": fused_ms, "unit": "ms/step", "n_gpus": 1, "steps": n, "warmup": 1, "ms_per_step": fused_ms,
+            "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "configs[4]: 32 x 7 projections + lm_head[128256,4096], bf16 W + fp32 m/v resident, reverse layer order",
+                       "params": st.params, "state_bytes": st.state_bytes, "input_bytes": st.input_bytes, "tokens": args.tokens,
+                       "l2": "75 GB working set >> 126 MB L2"},
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak, "traffic": None,
+                         "peak_source": peak_src, "algorithmic_bytes_per_step": alg_bytes, "roofline_ms": alg_bytes / hbm_peak / 1e6},
+            "gpu_launches": int(launches),
+            "peak_device_memory": {"fused_bytes": int(fused_peak), "dw_pool_arm_bytes": int(pool_peak),
+                                   "dw_pool_bytes": int(pool_bytes), "dw_bytes_allocated_by_fused_path": 0,
+                                   "device_total_bytes": int(total)},
+            "dw_pool_arm": {"ms_per_step": pool_ms, "what": "cuBLAS fp32 dW for all layers into a 30 GB pool, then elementwise AdamW over the pool"},
+            "speedup_vs_dw_pool_arm": pool_ms / fused_ms}
+    print(json.dumps(line), flush=True)
+
+
 def run_cuda(args):
+    if args.workload == "model":
+        return run_model(args)
     import torch
     import torch.distributed as dist
     from paper_2606_22932_b200 import binding as fb
@@ -383,8 +440,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--moments", choices=["fp32", "bf16", "int8"], default="fp32")
     ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
-    ap.add_argument("--workload", choices=["layer", "q", "k", "v", "o", "gate", "up", "down"], default="layer",
-                    help="layer = BASELINE.json configs[1] (the metric); a projection name = that problem alone (configs[3])")
+    ap.add_argument("--workload", choices=["layer", "q", "k", "v", "o", "gate", "up", "down", "model"], default="layer",
+                    help="layer = BASELINE.json configs[1] (the metric); a projection name = that problem alone (configs[3]); model = configs[4]")
     ap.add_argument("--tokens", type=int, default=T_TOKENS, help="T (configs[3] sweeps 512/2048/8192 on gate)")
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, same-GPU baselines and the CPU oracle leg")
     args = ap.parse_args()

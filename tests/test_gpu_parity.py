@@ -263,3 +263,43 @@ def test_host_buffer_entry_point_matches_device_path():
     torch.cuda.synchronize()
     for k in ("W", "m", "v"):
         assert torch.equal(d[k].cpu(), h[k])
+
+
+def test_config4_full_stack_reverse_order_sampled_rows():
+    """BASELINE.json configs[4] at full size: 32 layers + lm_head resident (75 GB), one step in reverse
+    layer order through the grouped entry; lm_head and three layers are checked on sampled rows against
+    the oracle (rows are independent, so a row subset is an exact oracle for those rows)."""
+    from paper_2606_22932_b200 import stack
+    free, _ = torch.cuda.mem_get_info()
+    if free < 90e9:
+        pytest.skip("needs ~80 GB of free device memory")
+    dev = torch.device("cuda:0")
+    st = stack.build_stack(dev, tokens=512)
+    assert st.params == 32 * 218103808 + 128256 * 4096 and len(st.layers) == 33
+    hp = synth.HP_DEFAULT
+    picks = [(32, 0), (31, 6), (16, 4), (0, 0), (0, 1)]          # lm_head, L31.down, L16.gate, L0.q, L0.k
+    before = {}
+    for li, pi in picks:
+        d = st.layers[li][pi]
+        out = d["W"].shape[0]
+        rows = pu.sample_rows(out, seed=li)
+        before[(li, pi)] = [(r0, r1, synth.bf16_bits(d["W"][r0:r1]).copy(), d["m"][r0:r1].cpu().numpy().copy(),
+                             d["v"][r0:r1].cpu().numpy().copy()) for r0, r1 in rows]
+    torch.cuda.reset_peak_memory_stats()
+    base_alloc = torch.cuda.memory_allocated()
+    n = stack.step_fused(st, 10, hp)
+    torch.cuda.synchronize()
+    assert n == 33                                               # one launch per layer + lm_head
+    assert torch.cuda.max_memory_allocated() == base_alloc       # nothing gradient-shaped was allocated
+    for li, pi in picks:
+        d = st.layers[li][pi]
+        dYb, Xb = synth.bf16_bits(d["dY"]), synth.bf16_bits(d["X"])
+        T = d["X"].shape[0]
+        for r0, r1, Wb, m0, v0 in before[(li, pi)]:
+            G, E = fo.wgrad(dYb, Xb, rows=(r0, r1), with_abs=True)
+            Wp = Wb.copy()
+            fo.adamw_fp32(Wb, m0, v0, G, 10, *pu.hp_tuple(hp))
+            tol = pu.Tol(G.shape)
+            e = tol.step(G, E, T, hp)
+            pu.check_fp(synth.bf16_bits(d["W"][r0:r1]), d["m"][r0:r1].cpu().numpy(), d["v"][r0:r1].cpu().numpy(),
+                                 Wb, m0, v0, G, e, tol, hp, label=f"{d['name']}[{r0}:{r1}]", W_prev=Wp)
