@@ -254,7 +254,7 @@ struct Int8Row {           // per-thread view of its row's 256-block in one tile
 template <class Cfg>
 __device__ __forceinline__ void int8_pass1(const AdamWScalars &hp, const Int8Row &R, uint32_t titer, uint32_t taddr,
                                            const Int8Smem &S, uint32_t row_t, int wg, float &pm, float &pv,
-                                           bool skip_math) {
+                                           bool skip_math, bool no_state) {
     pm = 0.0f;
     pv = 0.0f;
     constexpr int kSubs = Cfg::P1_COLS / SUB;              // 32-column sub-blocks per chunk; sub-block t of the
@@ -263,7 +263,7 @@ __device__ __forceinline__ void int8_pass1(const AdamWScalars &hp, const Int8Row
     for (int c1 = 0; c1 < Cfg::P1_CHUNKS; ++c1) {
         const uint32_t i1 = titer * Cfg::P1_CHUNKS + c1, s = i1 % Cfg::P1_STAGES, ph = (i1 / Cfg::P1_STAGES) & 1u;
         const uint32_t am = S.p1 + s * Cfg::P1_STAGE, av = am + Cfg::P1_BOX;
-        mbar_wait(S.bar_p1_full + 8 * s, ph);
+        if (!no_state) mbar_wait(S.bar_p1_full + 8 * s, ph);
 #pragma unroll 1
         for (int j32 = 0; j32 < (skip_math ? 0 : kSubs); ++j32) {
             if ((c1 * kSubs + j32) % kI8W != wg) continue;
@@ -299,7 +299,8 @@ __device__ __forceinline__ void int8_pass1(const AdamWScalars &hp, const Int8Row
 template <class Cfg, int kStateStages>
 __device__ __forceinline__ void int8_pass2(const AdamWScalars &hp, const Int8Row &R, float a_m, float a_v,
                                            uint32_t titer, uint32_t taddr, uint32_t sST, uint32_t bar_st_full,
-                                           uint32_t bar_st_done, uint32_t row_t, int wg, bool skip_math) {
+                                           uint32_t bar_st_done, uint32_t bar_st_empty, uint32_t row_t, int wg,
+                                           bool skip_math, bool no_state) {
     const uint32_t rb = row_t / Cfg::CM, row = row_t % Cfg::CM;
     const float bm = R.bm, bv = R.bv;
     const float inv_m = quant_inv_scale(a_m, 127.0f), inv_v = quant_inv_scale(a_v, 255.0f);
@@ -308,7 +309,8 @@ __device__ __forceinline__ void int8_pass2(const AdamWScalars &hp, const Int8Row
     for (int cb = 0; cb < Cfg::CB; ++cb) {
         const uint32_t ci = titer * Cfg::CHUNKS + cb * Cfg::RB + rb;
         const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
-        mbar_wait(bar_st_full + 8 * s, ph);
+        if (!no_state) mbar_wait(bar_st_full + 8 * s, ph);
+        else mbar_wait(bar_st_empty + 8 * s, ph ^ 1u);
 #pragma unroll 1
         for (int half = 0; half < Cfg::SUBS; ++half) {
         if (skip_math || (cb * Cfg::SUBS + half) % kI8W != wg) continue;
@@ -553,7 +555,8 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
     } else if (warp == 2) {
         // ================= state loader (Alg. 1 line 6: load W_ij, m_ij, v_ij) ===================
         if constexpr (MDT == MDT_INT8) {
-            if (lane == 0) int8_loader<Cfg, kStateStages, CG>(P, rank, first_tile, tile_step, sST, bar_st_full, bar_st_empty, i8);
+            if (lane == 0 && !(P.debug & DBG_NO_STATE))
+                int8_loader<Cfg, kStateStages, CG>(P, rank, first_tile, tile_step, sST, bar_st_full, bar_st_empty, i8);
         } else if (MODE == MODE_ADAMW && lane == 0 && !(P.debug & DBG_NO_STATE)) {
             uint32_t ci = 0;  // running chunk counter
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step) {
@@ -673,7 +676,8 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                 if (tile + tile_step < P.total_tiles) i8row = int8_row<CG>(P, hp, tile + tile_step, rank, row_t);
                 R.finish(hp);
                 float pm, pv;
-                int8_pass1<Cfg>(hp, R, titer, taddr, i8, row_t, wg, pm, pv, (P.debug & DBG_NO_EPILOGUE) != 0);
+                int8_pass1<Cfg>(hp, R, titer, taddr, i8, row_t, wg, pm, pv, (P.debug & DBG_NO_EPILOGUE) != 0,
+                                (P.debug & DBG_NO_STATE) != 0);
                 // combine the two warpgroups' halves of the row (same TMEM quadrant: warps quad and 4 + quad)
                 const uint32_t xb = i8.xchg + (titer & 1u) * (kI8W * 1024u);
                 asm volatile("st.shared.v2.f32 [%0], {%1, %2};\n" ::"r"(xb + (wg * 128u + row_t) * 8u), "f"(pm), "f"(pv) : "memory");
@@ -686,8 +690,8 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                     a_m = fmaxf(a_m, om);
                     a_v = fmaxf(a_v, ov);
                 }
-                int8_pass2<Cfg, kStateStages>(hp, R, a_m, a_v, titer, taddr, sST, bar_st_full, bar_st_done, row_t, wg,
-                                              (P.debug & DBG_NO_EPILOGUE) != 0);
+                int8_pass2<Cfg, kStateStages>(hp, R, a_m, a_v, titer, taddr, sST, bar_st_full, bar_st_done, bar_st_empty,
+                                              row_t, wg, (P.debug & DBG_NO_EPILOGUE) != 0, (P.debug & DBG_NO_STATE) != 0);
                 if (wg == 0 && R.valid) {
                     const ProblemDesc &pd = P.prob[decode_tile<CG>(P, tile, rank).p];
                     pd.m_scale[R.sidx] = a_m;
