@@ -17,15 +17,16 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "forge_oracle.c")
+_SRC_FAM = os.path.join(_HERE, "forge_oracle_families.c")
 _LIB = os.path.join(_HERE, "libforge_oracle.so")
 QBLOCK = 256
 
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (no fast-math, no FMA contraction)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_FAM)):
         cmd = ["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared",
-               "-o", _LIB, _SRC, "-lm"]
+               "-o", _LIB, _SRC, _SRC_FAM, "-lm"]
         subprocess.run(cmd, check=True)
     return _LIB
 
@@ -57,6 +58,10 @@ def lib() -> ctypes.CDLL:
         L.forge_oracle_bf16_from_double_array.restype = None
         L.forge_oracle_bf16_from_double_array.argtypes = [c_void_p, c_void_p, c_size_t]
         L.forge_oracle_num_threads.restype = c_int
+        L.forge_oracle_family_step.restype = None
+        L.forge_oracle_family_step.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int, c_void_p, c_size_t,
+                                               c_long, c_float, c_float, c_float, c_float, c_float, c_float,
+                                               c_int, c_void_p]
         _lib = L
     return _lib
 
@@ -166,3 +171,26 @@ def dequantize_v(vq: np.ndarray, v_scale: np.ndarray) -> np.ndarray:
 def step_fp32(dY, X, W, m, v, step, lr, beta1, beta2, eps, wd):
     """One whole hot-path step with fp32 moments: G then AdamW, in place."""
     adamw_fp32(W, m, v, wgrad(dY, X), step, lr, beta1, beta2, eps, wd)
+
+
+# ------------------------------------------------------------------ other regime-1 families --
+FAMILIES = {"sgd": 1, "momentum": 2, "lion": 3, "rmsprop": 4, "adagrad": 5, "adamax": 6, "nadam": 7, "radam": 8}
+FAMILY_STATES = {"sgd": 0, "momentum": 1, "lion": 1, "rmsprop": 1, "adagrad": 1, "adamax": 2, "nadam": 2, "radam": 2}
+
+
+def family_step(family: str, W, s0, s1, G, step, lr, beta1=0.9, beta2=0.999, eps=1e-8, wd=0.0, momentum=0.0,
+                nesterov=False, debug: bool = False):
+    """In place step of one coordinate-wise family (forge_oracle_families.c).
+    W uint16 bf16 bits; s0/s1 float32 or uint16 (bf16 bits) arrays or None; G float64."""
+    _chk(W, np.uint16, "W"); _chk(G, np.float64, "G")
+    ns = FAMILY_STATES[family]
+    states = [s0, s1][:ns]
+    assert all(s is not None for s in states) and all(s is None for s in [s0, s1][ns:])
+    bf16 = bool(states) and states[0].dtype == np.uint16
+    for s in states:
+        _chk(s, np.uint16 if bf16 else np.float32, "state")
+        assert s.shape == W.shape
+    Wd = np.empty(W.shape, np.float64) if debug else None
+    lib().forge_oracle_family_step(FAMILIES[family], _p(W), _p(s0), _p(s1), int(bf16), _p(G), W.size, int(step),
+                                   lr, beta1, beta2, eps, wd, momentum, int(bool(nesterov)), _p(Wd))
+    return Wd

@@ -1,0 +1,145 @@
+/* TEST INFRASTRUCTURE ONLY -- CPU oracle for the other coordinate-wise ("regime 1", tile-local A and U)
+ * optimizer families of PAPER.md:267 Definition 1 / PAPER.md:716-727 Appendix I: SGD, SGD with momentum
+ * (optionally Nesterov), Lion, RMSprop, Adagrad, Adamax, NAdam, RAdam.  The paper gives no formulas for
+ * them: it verifies each "against a reference PyTorch implementation", so each function
+ * below is the textbook rule as torch.optim documents it (Lion: Chen et al. 2023, Alg. 2), written out
+ * per coordinate in fp64, one rounding to the storage type at the end, W' from the unrounded new state
+ * (reading S3).  Pinned in tests/test_oracle_families.py against torch.optim in float64.
+ * Shares nothing with the CUDA path.
+ *
+ * Hyper-parameters arrive as the ABI's floats and are promoted to double (reading S15).
+ * State tensors: s0 / s1, fp32 or bf16 bit patterns (state_bf16 != 0); absent ones are NULL.
+ *   SGD        : no state            MOMENTUM : s0 = momentum buffer    LION    : s0 = m
+ *   RMSPROP    : s0 = square avg     ADAGRAD  : s0 = sum of squares
+ *   ADAMAX     : s0 = m, s1 = u (infinity norm)     NADAM, RADAM : s0 = m, s1 = v
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+
+double forge_oracle_bf16_to_double(uint16_t b);
+uint16_t forge_oracle_bf16_from_double(double x);
+
+enum { FAM_SGD = 1, FAM_MOMENTUM = 2, FAM_LION = 3, FAM_RMSPROP = 4, FAM_ADAGRAD = 5, FAM_ADAMAX = 6,
+       FAM_NADAM = 7, FAM_RADAM = 8 };
+
+typedef struct {
+    int family;
+    long step;                 /* 1-based index of the update being applied */
+    double lr, beta1, beta2, eps, wd;
+    double momentum;           /* MOMENTUM: mu; RMSPROP: alpha is passed in beta2 */
+    int nesterov;
+} fam_hp;
+
+static double ld(const void *p, size_t i, int bf16)
+{
+    return bf16 ? forge_oracle_bf16_to_double(((const uint16_t *)p)[i]) : (double)((const float *)p)[i];
+}
+static void st(void *p, size_t i, int bf16, double x)
+{
+    if (bf16) ((uint16_t *)p)[i] = forge_oracle_bf16_from_double(x);
+    else ((float *)p)[i] = (float)x;
+}
+
+/* NAdam's momentum schedule (torch.optim.NAdam, momentum_decay psi = 4e-3):
+ * mu_t = beta1 * (1 - 0.5 * 0.96^(t*psi)); mu_product_t = prod_{i<=t} mu_i. */
+static double nadam_mu(double beta1, long t) { return beta1 * (1.0 - 0.5 * pow(0.96, (double)t * 4e-3)); }
+
+/* One coordinate.  w, s0, s1: current values; g: this step's gradient. */
+static void family_coord(const fam_hp *h, double w, double s0, double s1, double g,
+                         double *w1, double *s0n, double *s1n)
+{
+    const double t = (double)h->step;
+    *s0n = s0; *s1n = s1;
+    switch (h->family) {
+    case FAM_SGD: {                                   /* torch.optim.SGD, momentum = 0 */
+        double gp = g + h->wd * w;                    /* L2 (coupled) weight decay */
+        *w1 = w - h->lr * gp;
+        break; }
+    case FAM_MOMENTUM: {                              /* torch.optim.SGD, dampening = 0 */
+        double gp = g + h->wd * w;
+        double buf = (h->step == 1) ? gp : h->momentum * s0 + gp;   /* first step: buf = g */
+        double d = h->nesterov ? gp + h->momentum * buf : buf;
+        *w1 = w - h->lr * d;
+        *s0n = buf;
+        break; }
+    case FAM_LION: {                                  /* Chen et al. 2023, Algorithm 2 */
+        double c = h->beta1 * s0 + (1.0 - h->beta1) * g;
+        double sgn = (c > 0.0) - (c < 0.0);
+        *w1 = w * (1.0 - h->lr * h->wd) - h->lr * sgn;             /* decoupled decay */
+        *s0n = h->beta2 * s0 + (1.0 - h->beta2) * g;
+        break; }
+    case FAM_RMSPROP: {                               /* torch.optim.RMSprop, momentum 0, not centered */
+        double gp = g + h->wd * w;
+        double sq = h->beta2 * s0 + (1.0 - h->beta2) * gp * gp;    /* alpha passed as beta2 */
+        *w1 = w - h->lr * gp / (sqrt(sq) + h->eps);
+        *s0n = sq;
+        break; }
+    case FAM_ADAGRAD: {                               /* torch.optim.Adagrad, lr_decay = 0 */
+        double gp = g + h->wd * w;
+        double sum = s0 + gp * gp;
+        *w1 = w - h->lr * gp / (sqrt(sum) + h->eps);
+        *s0n = sum;
+        break; }
+    case FAM_ADAMAX: {                                /* torch.optim.Adamax */
+        double gp = g + h->wd * w;
+        double m = h->beta1 * s0 + (1.0 - h->beta1) * gp;
+        double u = fmax(h->beta2 * s1, fabs(gp) + h->eps);
+        *w1 = w - (h->lr / (1.0 - pow(h->beta1, t))) * m / u;
+        *s0n = m; *s1n = u;
+        break; }
+    case FAM_NADAM: {                                 /* torch.optim.NAdam, coupled decay */
+        double gp = g + h->wd * w;
+        double bc2 = 1.0 - pow(h->beta2, t);
+        double mu = nadam_mu(h->beta1, h->step), mu_next = nadam_mu(h->beta1, h->step + 1);
+        double prod = 1.0;
+        for (long i = 1; i <= h->step; ++i) prod *= nadam_mu(h->beta1, i);
+        double m = h->beta1 * s0 + (1.0 - h->beta1) * gp;
+        double v = h->beta2 * s1 + (1.0 - h->beta2) * gp * gp;
+        double denom = sqrt(v / bc2) + h->eps;
+        *w1 = w - h->lr * (1.0 - mu) / (1.0 - prod) * gp / denom
+                - h->lr * mu_next / (1.0 - prod * mu_next) * m / denom;
+        *s0n = m; *s1n = v;
+        break; }
+    case FAM_RADAM: {                                 /* torch.optim.RAdam, coupled decay */
+        double gp = g + h->wd * w;
+        double bc1 = 1.0 - pow(h->beta1, t), bc2 = 1.0 - pow(h->beta2, t);
+        double m = h->beta1 * s0 + (1.0 - h->beta1) * gp;
+        double v = h->beta2 * s1 + (1.0 - h->beta2) * gp * gp;
+        double rho_inf = 2.0 / (1.0 - h->beta2) - 1.0;
+        double rho_t = rho_inf - 2.0 * t * pow(h->beta2, t) / bc2;
+        double mhat = m / bc1;
+        if (rho_t > 5.0) {
+            double rect = sqrt((rho_t - 4.0) * (rho_t - 2.0) * rho_inf / ((rho_inf - 4.0) * (rho_inf - 2.0) * rho_t));
+            double adaptive = sqrt(bc2) / (sqrt(v) + h->eps);
+            *w1 = w - mhat * h->lr * adaptive * rect;
+        } else {
+            *w1 = w - mhat * h->lr;
+        }
+        *s0n = m; *s1n = v;
+        break; }
+    default:
+        *w1 = w;
+    }
+}
+
+/* n coordinates, in place.  W bf16 bits; s0/s1 fp32 or bf16 bits (NULL when the family has none).
+ * Wd (optional) receives the unrounded fp64 W'. */
+void forge_oracle_family_step(int family, uint16_t *W, void *s0, void *s1, int state_bf16, const double *G,
+                              size_t n, long step, float lr, float beta1, float beta2, float eps, float wd,
+                              float momentum, int nesterov, double *Wd)
+{
+    fam_hp h;
+    h.family = family; h.step = step; h.lr = (double)lr; h.beta1 = (double)beta1; h.beta2 = (double)beta2;
+    h.eps = (double)eps; h.wd = (double)wd; h.momentum = (double)momentum; h.nesterov = nesterov;
+#pragma omp parallel for schedule(static)
+    for (size_t i = 0; i < n; ++i) {
+        double w1, a, b;
+        family_coord(&h, forge_oracle_bf16_to_double(W[i]), s0 ? ld(s0, i, state_bf16) : 0.0,
+                     s1 ? ld(s1, i, state_bf16) : 0.0, G[i], &w1, &a, &b);
+        W[i] = forge_oracle_bf16_from_double(w1);
+        if (s0) st(s0, i, state_bf16, a);
+        if (s1) st(s1, i, state_bf16, b);
+        if (Wd) Wd[i] = w1;
+    }
+}

@@ -1,0 +1,126 @@
+"""Pins for oracle/forge_oracle_families.c (the other coordinate-wise families of PAPER.md:267 Def. 1):
+each rule is checked against torch.optim on CPU in float64 -- a library call with injected state, the
+paper's own method of verification -- over several consecutive steps, and Lion (not in
+torch.optim) against its closed forms.  The oracle's W is bf16; the comparison is made on its unrounded
+fp64 W' (debug output) and on fp32 state, chained through the oracle's own rounded values."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import forge_oracle as fo
+
+OUT, IN = 48, 64
+
+
+def bf16_bits(x: np.ndarray) -> np.ndarray:
+    return fo.f64_to_bf16(x.astype(np.float64))
+
+
+def torch_reference(family, hp):
+    p = torch.nn.Parameter(torch.zeros(OUT, IN, dtype=torch.float64))
+    if family == "sgd":
+        return p, torch.optim.SGD([p], lr=hp["lr"], weight_decay=hp["wd"])
+    if family == "momentum":
+        return p, torch.optim.SGD([p], lr=hp["lr"], weight_decay=hp["wd"], momentum=hp["momentum"], nesterov=hp["nesterov"])
+    if family == "rmsprop":
+        return p, torch.optim.RMSprop([p], lr=hp["lr"], alpha=hp["beta2"], eps=hp["eps"], weight_decay=hp["wd"])
+    if family == "adagrad":
+        return p, torch.optim.Adagrad([p], lr=hp["lr"], eps=hp["eps"], weight_decay=hp["wd"])
+    if family == "adamax":
+        return p, torch.optim.Adamax([p], lr=hp["lr"], betas=(hp["beta1"], hp["beta2"]), eps=hp["eps"], weight_decay=hp["wd"])
+    if family == "nadam":
+        return p, torch.optim.NAdam([p], lr=hp["lr"], betas=(hp["beta1"], hp["beta2"]), eps=hp["eps"], weight_decay=hp["wd"])
+    if family == "radam":
+        return p, torch.optim.RAdam([p], lr=hp["lr"], betas=(hp["beta1"], hp["beta2"]), eps=hp["eps"], weight_decay=hp["wd"])
+    raise KeyError(family)
+
+
+STATE_KEYS = {"momentum": ["momentum_buffer"], "rmsprop": ["square_avg"], "adagrad": ["sum"],
+              "adamax": ["exp_avg", "exp_inf"], "nadam": ["exp_avg", "exp_avg_sq"], "radam": ["exp_avg", "exp_avg_sq"]}
+
+
+@pytest.mark.parametrize("family,extra", [
+    ("sgd", {}), ("momentum", {"momentum": 0.9}), ("momentum", {"momentum": 0.8, "nesterov": True}),
+    ("rmsprop", {"beta2": 0.99}), ("adagrad", {"eps": 1e-10}), ("adamax", {}), ("nadam", {}), ("radam", {})])
+def test_family_matches_torch_optim_float64_over_eight_steps(family, extra):
+    """Steps 1..8 cover RAdam's un-rectified (rho_t <= 5, t <= 5 at beta2 = 0.999) and rectified branches."""
+    hp = dict(lr=1e-2, beta1=np.float32(0.9).item(), beta2=np.float32(0.999).item(), eps=1e-8, wd=0.05, momentum=0.0, nesterov=False)
+    hp.update({k: (np.float32(v).item() if isinstance(v, float) else v) for k, v in extra.items()})
+    hp["lr"], hp["eps"], hp["wd"] = (np.float32(hp[k]).item() for k in ("lr", "eps", "wd"))   # the ABI carries floats
+    rng = np.random.default_rng(11)
+    W = bf16_bits(rng.normal(0, 0.02, (OUT, IN)))
+    ns = fo.FAMILY_STATES[family]
+    states = [np.zeros((OUT, IN), np.float32) for _ in range(ns)]
+    p, opt = torch_reference(family, hp)
+    for step in range(1, 9):
+        G = rng.normal(0, 1e-2, (OUT, IN))
+        # torch starts every step from the oracle's (rounded) W and state: one-step comparison, chained inputs
+        with torch.no_grad():
+            p.copy_(torch.from_numpy(fo.bf16_to_f64(W)))
+        p.grad = torch.from_numpy(G.copy())
+        if step > 1:
+            for key, s in zip(STATE_KEYS.get(family, []), states):
+                opt.state[p][key].copy_(torch.from_numpy(s.astype(np.float64)))
+        opt.step()
+        Wd = fo.family_step(family, W, *(states + [None] * (2 - ns)), G, step, hp["lr"], hp["beta1"], hp["beta2"],
+                            hp["eps"], hp["wd"], hp["momentum"], hp["nesterov"], debug=True)
+        ref = p.detach().numpy()
+        # torch.optim.NAdam keeps mu_product in a float32 scalar tensor: 1e-7 relative on the step size
+        atol = 1e-6 * hp["lr"] if family == "nadam" else 1e-15
+        assert np.allclose(Wd, ref, rtol=1e-12, atol=atol), (family, step, np.abs(Wd - ref).max())
+        assert np.array_equal(W, fo.f64_to_bf16(Wd))                         # one RNE rounding of the fp64 W'
+        for key, s in zip(STATE_KEYS.get(family, []), states):
+            t = opt.state[p][key].numpy()
+            assert np.allclose(s, t, rtol=2e-7, atol=1e-30), (family, key, step)     # fp32 storage of the fp64 state
+
+
+def test_lion_closed_forms_and_bruteforce():
+    rng = np.random.default_rng(5)
+    lr, b1, b2, wd = (np.float32(x).item() for x in (1e-4, 0.9, 0.99, 0.1))
+    Wf = rng.normal(0, 0.02, (OUT, IN))
+    W0 = bf16_bits(Wf)
+    m0 = rng.normal(0, 1e-3, (OUT, IN)).astype(np.float32)
+    G = rng.normal(0, 1e-3, (OUT, IN))
+    G[0, :4] = 0.0
+    m0[0, :4] = 0.0                                                         # sign(0) = 0: decay only
+    W, m = W0.copy(), m0.copy()
+    Wd = fo.family_step("lion", W, m, None, G, 1, lr, b1, b2, 0.0, wd, debug=True)
+    w = fo.bf16_to_f64(W0)
+    for i in range(OUT):                                                    # Chen et al. 2023 Alg. 2, coordinate by coordinate
+        for j in range(IN):
+            c = b1 * float(m0[i, j]) + (1 - b1) * G[i, j]
+            s = 1.0 if c > 0 else (-1.0 if c < 0 else 0.0)
+            assert Wd[i, j] == w[i, j] * (1 - lr * wd) - lr * s
+            assert m[i, j] == np.float32(b2 * float(m0[i, j]) + (1 - b2) * G[i, j])
+    assert np.all(Wd[0, :4] == w[0, :4] * (1 - lr * wd))
+    # every non-degenerate coordinate moves by exactly lr (plus decay): |dW + lr*wd*w| == lr
+    moved = np.abs(Wd - w * (1 - lr * wd))
+    assert np.allclose(moved[1:], lr, rtol=1e-12)
+    # beta1 = beta2 = 0: direction is sign(g), state becomes g
+    W, m = W0.copy(), m0.copy()
+    Wd = fo.family_step("lion", W, m, None, G, 1, lr, 0.0, 0.0, 0.0, 0.0, debug=True)
+    assert np.array_equal(Wd, w - lr * np.sign(G)) and np.array_equal(m, G.astype(np.float32))
+
+
+def test_families_reduce_to_each_other_and_bf16_state():
+    rng = np.random.default_rng(9)
+    W0 = bf16_bits(rng.normal(0, 0.02, (OUT, IN)))
+    G = rng.normal(0, 1e-2, (OUT, IN))
+    lr = np.float32(1e-2).item()
+    # momentum with mu = 0 is SGD; lr = 0 leaves W untouched while state moves
+    Wa, Wb = W0.copy(), W0.copy()
+    buf = np.zeros((OUT, IN), np.float32)
+    fo.family_step("sgd", Wa, None, None, G, 3, lr, wd=0.0)
+    fo.family_step("momentum", Wb, buf, None, G, 3, lr, wd=0.0, momentum=0.0)
+    assert np.array_equal(Wa, Wb) and np.array_equal(buf, G.astype(np.float32))
+    Wc, s = W0.copy(), np.zeros((OUT, IN), np.float32)
+    fo.family_step("adagrad", Wc, s, None, G, 1, 0.0)
+    assert np.array_equal(Wc, W0) and np.array_equal(s, (G * G).astype(np.float32))
+    # bf16 state: same rule, state rounded RNE on store, W' from the unrounded state (reading S3)
+    W32, W16 = W0.copy(), W0.copy()
+    s32 = np.full((OUT, IN), 1e-4, np.float32)
+    s16 = fo.f64_to_bf16(s32.astype(np.float64))
+    s32 = fo.bf16_to_f64(s16).astype(np.float32)
+    fo.family_step("rmsprop", W32, s32, None, G, 2, lr, beta2=np.float32(0.99).item())
+    fo.family_step("rmsprop", W16, s16, None, G, 2, lr, beta2=np.float32(0.99).item())
+    assert np.array_equal(W32, W16) and np.array_equal(s16, fo.f64_to_bf16(s32.astype(np.float64)))
