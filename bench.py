@@ -338,12 +338,24 @@ def run_cuda(args):
     hp = synth.HP_DEFAULT
     mdt = MOMENT_ENUM[args.moments]
     layer = make_device_layer(args.moments, 20260622 + 1 + rank, dev, args.workload, args.tokens)
+    nst = fb.FAMILY_STATES[args.optimizer]
+    if args.optimizer != "adamw":                  # keep only the states the family has
+        if args.moments == "int8":
+            raise SystemExit("int8 state is implemented for AdamW only")
+        for d in layer:
+            v_like = d["v"]                        # non-negative: the single state of rmsprop / adagrad
+            d["v"] = d["v"] if nst >= 2 else None
+            d["m"] = (d["m"] if nst == 2 or args.optimizer in ("momentum", "lion") else v_like) if nst >= 1 else None
     arr = fb.make_problem_array(layer)
     hpt = (hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
     stream = torch.cuda.current_stream()
 
     def step(t):
-        fb.forge_wgrad_adamw_grouped(layer, t, *hpt, mdt, stream=stream, _arr=arr)
+        if args.optimizer == "adamw":
+            fb.forge_wgrad_adamw_grouped(layer, t, *hpt, mdt, stream=stream, _arr=arr)
+        else:
+            fb.forge_wgrad_step_grouped(layer, args.optimizer, t, hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"],
+                                        momentum=0.9, state_dtype=mdt, stream=stream, _arr=arr)
 
     def barrier():
         if world > 1:
@@ -371,7 +383,8 @@ def run_cuda(args):
     us_per_layer = ms_per_step * 1e3 / world       # layers processed by all ranks per step = world
 
     params, in_bytes, flops = layer_counts(args.workload, args.tokens)
-    alg_bytes = params * MOMENT_BYTES[args.moments] + in_bytes
+    state_b = {"fp32": 8.0, "bf16": 4.0}.get(args.moments, 0.0)
+    alg_bytes = params * (MOMENT_BYTES[args.moments] if args.optimizer == "adamw" else 4.0 + nst * state_b) + in_bytes
     hbm_peak, tf_burst, tf_sustained, peak_src = measured_peaks()
     kernel_ms = (evs[0].elapsed_time(evs[-1])) / args.steps       # this rank's average launch duration
     gbs = alg_bytes / (kernel_ms * 1e-3) / 1e9
@@ -384,7 +397,7 @@ def run_cuda(args):
     else:
         roofline = {"bound": "tensor", "achieved": tfs, "peak": tf_sustained, "unit": "TFLOP/s", "frac": tfs / tf_sustained,
                     "frac_of_burst_peak": tfs / tf_burst, "burst_peak": tf_burst}
-    is_headline = args.workload == "layer" and args.tokens == T_TOKENS
+    is_headline = args.workload == "layer" and args.tokens == T_TOKENS and args.optimizer == "adamw"
     roofline.update({"traffic": NCU_TRAFFIC_BYTES[args.moments] if is_headline else None, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": alg_bytes, "flops_per_launch": flops,
                      "roofline_us": max(t_hbm_us, t_tensor_us), "hbm_term_us": t_hbm_us, "tensor_term_us": t_tensor_us,
@@ -398,7 +411,8 @@ def run_cuda(args):
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": (("configs[1]: Llama-3.1-8B layer, 7 projections in one grouped launch, T=512"
                                      if args.moments == "fp32" else f"configs[2]: same layer, {args.moments} moments")
-                                    if is_headline else f"configs[3]-style: {args.workload} of a Llama-3.1-8B layer, T={args.tokens}, {args.moments} moments"),
+                                    if is_headline else f"configs[3]-style: {args.workload} of a Llama-3.1-8B layer, T={args.tokens}, "
+                                    f"{args.optimizer} with {nst} {args.moments} state tensor(s)"),
                        "moments": args.moments, "params_per_layer": params, "tokens": args.tokens,
                        "l2": "working set 4.4 GB/layer >> 126 MB L2, no flush needed",
                        "parallelism": f"replicated layers x{world}, no collective"},
@@ -442,6 +456,8 @@ def main():
     ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
     ap.add_argument("--workload", choices=["layer", "q", "k", "v", "o", "gate", "up", "down", "model"], default="layer",
                     help="layer = BASELINE.json configs[1] (the metric); a projection name = that problem alone (configs[3]); model = configs[4]")
+    ap.add_argument("--optimizer", default="adamw", choices=["adamw", "sgd", "momentum", "lion", "rmsprop", "adagrad", "adamax", "nadam", "radam"],
+                    help="SURVEY.md 8(f) rank 1: the other coordinate-wise families on the same fused mainloop")
     ap.add_argument("--tokens", type=int, default=T_TOKENS, help="T (configs[3] sweeps 512/2048/8192 on gate)")
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, same-GPU baselines and the CPU oracle leg")
     args = ap.parse_args()

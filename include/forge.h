@@ -105,6 +105,29 @@ forge_status_t forge_wgrad_adamw_grouped(const forge_problem_t *problems, int32_
                                          float eps, float wd,
                                          forge_moment_dtype_t moment_dtype, forge_stream_t stream);
 
+/* The other coordinate-wise optimizer families of the paper's Definition 1 (App. I)
+ * on the same fused mainloop: the update rules are torch.optim's (Lion: Chen et al. 2023, Alg. 2) -- the paper
+ * verifies each "against a reference PyTorch implementation".  State tensors per family, passed in
+ * forge_problem_t.m / .v (absent ones MUST be NULL, else FORGE_ERR_NULL_PTR):
+ *   SGD: none | MOMENTUM: m = momentum buffer | LION: m | RMSPROP: m = square average (alpha = beta2) |
+ *   ADAGRAD: m = sum of squares | ADAMAX: m, v = infinity norm | NADAM, RADAM: m, v | ADAMW: as forge_wgrad_adamw.
+ * Weight decay is coupled (g + wd*W) except for ADAMW and LION (decoupled).  State dtype FP32 or BF16 (INT8: ADAMW
+ * only, else FORGE_ERR_BAD_DTYPE).  `step` is 1-based (MOMENTUM: the buffer is initialised with g at step 1). */
+typedef enum {
+    FORGE_OPT_ADAMW = 0, FORGE_OPT_SGD = 1, FORGE_OPT_MOMENTUM = 2, FORGE_OPT_LION = 3, FORGE_OPT_RMSPROP = 4,
+    FORGE_OPT_ADAGRAD = 5, FORGE_OPT_ADAMAX = 6, FORGE_OPT_NADAM = 7, FORGE_OPT_RADAM = 8
+} forge_optimizer_t;
+
+typedef struct {
+    forge_optimizer_t family;
+    int32_t nesterov;        /* MOMENTUM only */
+    int64_t step;
+    float lr, beta1, beta2, eps, wd, momentum;
+} forge_opt_desc_t;
+
+forge_status_t forge_wgrad_step_grouped(const forge_problem_t *problems, int32_t count, const forge_opt_desc_t *opt,
+                                        forge_moment_dtype_t state_dtype, forge_stream_t stream);
+
 /* End-to-end convenience entry with HOST buffers (used for the e2e measurement): copies X, dY and
  * the state to device scratch it allocates and frees itself, runs forge_wgrad_adamw, copies the
  * state back and synchronises.  Same validation and return codes; all pointers are host pointers. */

@@ -21,7 +21,7 @@ QBLOCK = 256
 STATUS_NAMES = ["FORGE_OK", "FORGE_ERR_NULL_PTR", "FORGE_ERR_BAD_SHAPE", "FORGE_ERR_ALIGNMENT",
                 "FORGE_ERR_BAD_HYPERPARAM", "FORGE_ERR_BAD_DTYPE", "FORGE_ERR_UNSUPPORTED_ARCH",
                 "FORGE_ERR_CUDA"]
-EXPORTS = ["forge_wgrad_adamw", "forge_wgrad_adamw_grouped", "forge_wgrad_adamw_host",
+EXPORTS = ["forge_wgrad_adamw", "forge_wgrad_adamw_grouped", "forge_wgrad_step_grouped", "forge_wgrad_adamw_host",
            "forge_wgrad_store_g", "forge_adamw_from_g", "forge_workspace_bytes", "forge_launch_count",
            "forge_last_cuda_error", "forge_status_string", "forge_version"]
 
@@ -38,6 +38,15 @@ class forge_problem_t(ctypes.Structure):
                 ("m_scale", c_void_p), ("v_scale", c_void_p),
                 ("T", c_int32), ("out", c_int32), ("in_", c_int32)]
 
+
+class forge_opt_desc_t(ctypes.Structure):
+    _fields_ = [("family", ctypes.c_int), ("nesterov", c_int32), ("step", c_int64),
+                ("lr", c_float), ("beta1", c_float), ("beta2", c_float), ("eps", c_float), ("wd", c_float),
+                ("momentum", c_float)]
+
+
+FAMILIES = {"adamw": 0, "sgd": 1, "momentum": 2, "lion": 3, "rmsprop": 4, "adagrad": 5, "adamax": 6, "nadam": 7, "radam": 8}
+FAMILY_STATES = {"adamw": 2, "sgd": 0, "momentum": 1, "lion": 1, "rmsprop": 1, "adagrad": 1, "adamax": 2, "nadam": 2, "radam": 2}
 
 _lib = None
 
@@ -56,6 +65,9 @@ def lib() -> ctypes.CDLL:
         L.forge_wgrad_adamw.argtypes = [c_void_p] * 7 + [c_int32] * 3 + hp + [ctypes.c_int, c_void_p]
         L.forge_wgrad_adamw_grouped.restype = ctypes.c_int
         L.forge_wgrad_adamw_grouped.argtypes = [ctypes.POINTER(forge_problem_t), c_int32] + hp + [ctypes.c_int, c_void_p]
+        L.forge_wgrad_step_grouped.restype = ctypes.c_int
+        L.forge_wgrad_step_grouped.argtypes = [ctypes.POINTER(forge_problem_t), c_int32, ctypes.POINTER(forge_opt_desc_t),
+                                               ctypes.c_int, c_void_p]
         L.forge_wgrad_adamw_host.restype = ctypes.c_int
         L.forge_wgrad_adamw_host.argtypes = [c_void_p] * 7 + [c_int32] * 3 + hp + [ctypes.c_int]
         L.forge_wgrad_store_g.restype = ctypes.c_int
@@ -110,7 +122,10 @@ def make_problem_array(problems):
         g = p.get if isinstance(p, dict) else (lambda k, d=None, p=p: getattr(p, k, d))
         X, dY = g("X"), g("dY")
         arr[i].X, arr[i].dY = X.data_ptr(), dY.data_ptr()
-        arr[i].W, arr[i].m, arr[i].v = g("W").data_ptr(), g("m").data_ptr(), g("v").data_ptr()
+        m, v = g("m"), g("v")
+        arr[i].W = g("W").data_ptr()
+        arr[i].m = None if m is None else m.data_ptr()
+        arr[i].v = None if v is None else v.data_ptr()
         ms, vs = g("m_scale"), g("v_scale")
         arr[i].m_scale = None if ms is None else ms.data_ptr()
         arr[i].v_scale = None if vs is None else vs.data_ptr()
@@ -127,6 +142,18 @@ def forge_wgrad_adamw_grouped(problems, step, lr, beta1, beta2, eps, wd, moment_
                                          _stream(stream))
     if check:
         _check(st, "forge_wgrad_adamw_grouped")
+    return st
+
+
+def forge_wgrad_step_grouped(problems, family: str, step, lr, beta1=0.9, beta2=0.999, eps=1e-8, wd=0.0, momentum=0.0,
+                             nesterov=False, state_dtype=FP32, stream=None, check=True, _arr=None) -> int:
+    """include/forge.h forge_wgrad_step_grouped: the other coordinate-wise families.
+    Problems carry m / v only for the states the family has (None otherwise)."""
+    arr = make_problem_array(problems) if _arr is None else _arr
+    desc = forge_opt_desc_t(FAMILIES[family], int(bool(nesterov)), int(step), lr, beta1, beta2, eps, wd, momentum)
+    st = lib().forge_wgrad_step_grouped(arr, len(arr), ctypes.byref(desc), state_dtype, _stream(stream))
+    if check:
+        _check(st, "forge_wgrad_step_grouped")
     return st
 
 

@@ -147,11 +147,12 @@ int env_int(const char *name, int dflt) {
 // ---------------------------------------------------------------------------------------------
 // launch of one fused-kernel instantiation over <= kMaxProblems problems
 // ---------------------------------------------------------------------------------------------
-template <int MDT, int MODE, int BK, int ST, int SS, int CG = 1, int CM = 64, int CN = 64, int P1C = 128, int P1S = 2>
+template <int MDT, int MODE, int BK, int ST, int SS, int CG = 1, int CM = 64, int CN = 64, int P1C = 128, int P1S = 2,
+          int NST = 2>
 forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamWScalars &hp,
-                            const DeviceInfo &dev, cudaStream_t stream) {
-    using Cfg = KernelCfg<MDT, BK, ST, SS, CG, CM, CN, P1C, P1S>;
-    auto kernel = forge_fused_kernel<MDT, MODE, BK, ST, SS, CG, CM, CN, P1C, P1S>;
+                            const DeviceInfo &dev, cudaStream_t stream, const FamilyScalars *fs = nullptr) {
+    using Cfg = KernelCfg<MDT, BK, ST, SS, CG, CM, CN, P1C, P1S, NST>;
+    auto kernel = forge_fused_kernel<MDT, MODE, BK, ST, SS, CG, CM, CN, P1C, P1S, NST>;
     static std::once_flag once;
     static cudaError_t attr_err = cudaSuccess;
     std::call_once(once, [&] {
@@ -162,6 +163,7 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
     KernelParams P;
     std::memset(&P, 0, sizeof(P));
     P.hp = hp;
+    if (fs) P.fs = *fs;
     P.num_problems = count;
     int tiles = 0;
     constexpr CUtensorMapDataType mom_dt = (MDT == MDT_FP32) ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
@@ -173,13 +175,15 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
         bool ok = true;
         ok &= encode_2d(&d.map_dY, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.dY, p.T, p.out, 64, BK, CU_TENSOR_MAP_SWIZZLE_128B);
         ok &= encode_2d(&d.map_X, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.X, p.T, p.in, 64, BK, CU_TENSOR_MAP_SWIZZLE_128B);
-        if (MODE == MODE_ADAMW) {
+        if (MODE != MODE_STORE_G) {
             ok &= encode_2d(&d.map_W, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.W, p.out, p.in, Cfg::W_BOX_COLS, CM,
                             swizzle_for_row_bytes(Cfg::W_ROW));
-            ok &= encode_2d(&d.map_m, mom_dt, Cfg::kMomBytes, p.m, p.out, p.in, Cfg::M_BOX_COLS, CM,
-                            swizzle_for_row_bytes(Cfg::M_ROW));
-            ok &= encode_2d(&d.map_v, mom_dt, Cfg::kMomBytes, p.v, p.out, p.in, Cfg::M_BOX_COLS, CM,
-                            swizzle_for_row_bytes(Cfg::M_ROW));
+            if (NST >= 1)
+                ok &= encode_2d(&d.map_m, mom_dt, Cfg::kMomBytes, p.m, p.out, p.in, Cfg::M_BOX_COLS, CM,
+                                swizzle_for_row_bytes(Cfg::M_ROW));
+            if (NST >= 2)
+                ok &= encode_2d(&d.map_v, mom_dt, Cfg::kMomBytes, p.v, p.out, p.in, Cfg::M_BOX_COLS, CM,
+                                swizzle_for_row_bytes(Cfg::M_ROW));
             if (MDT == MDT_INT8) {   // first-pass view of the same codes: 128 rows x 128 columns per box
                 ok &= encode_2d(&d.map_m1, mom_dt, 1, p.m, p.out, p.in, P1C, 128, swizzle_for_row_bytes(P1C));
                 ok &= encode_2d(&d.map_v1, mom_dt, 1, p.v, p.out, p.in, P1C, 128, swizzle_for_row_bytes(P1C));
@@ -263,6 +267,8 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
         case 5: return launch_fused<MDT_BF16, MODE_ADAMW, 64, 4, 2, 2, 64, 64>(probs, count, hp, dev, stream);
         case 6: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 6, 2, 64, 64>(probs, count, hp, dev, stream);
         case 7: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 2, 2, 64, 128>(probs, count, hp, dev, stream);
+        case 8: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 4, 2, 32, 128>(probs, count, hp, dev, stream);
+        case 9: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 2, 8, 2, 32, 128>(probs, count, hp, dev, stream);
         default: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
         }
     case FORGE_MOMENT_INT8:
@@ -279,6 +285,114 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
     default:
         return FORGE_ERR_BAD_DTYPE;
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// the other coordinate-wise families (family_math.cuh): scalars in double from the ABI's floats
+// ---------------------------------------------------------------------------------------------
+int family_states(int family) {
+    switch (family) {
+    case FORGE_OPT_SGD: return 0;
+    case FORGE_OPT_MOMENTUM: case FORGE_OPT_LION: case FORGE_OPT_RMSPROP: case FORGE_OPT_ADAGRAD: return 1;
+    default: return 2;
+    }
+}
+
+double nadam_mu(double beta1, int64_t t) { return beta1 * (1.0 - 0.5 * std::pow(0.96, static_cast<double>(t) * 4e-3)); }
+
+FamilyScalars make_family(const forge_opt_desc_t &o) {
+    FamilyScalars f;
+    std::memset(&f, 0, sizeof(f));
+    const double lr = o.lr, b1 = o.beta1, b2 = o.beta2, eps = o.eps, wd = o.wd, mu = o.momentum, t = static_cast<double>(o.step);
+    f.decay = 1.0f;
+    f.c2 = 1.0f;
+    f.e1 = 1.0f;
+    f.step = o.lr;
+    switch (o.family) {
+    case FORGE_OPT_SGD:
+        f.cwd = o.wd;
+        break;
+    case FORGE_OPT_MOMENTUM:                       // buf = mu*buf + g' (buf = g' at step 1); d = buf or g' + mu*buf
+        f.cwd = o.wd; f.has_m = 1; f.a1 = o.step == 1 ? 0.0f : o.momentum; f.a2 = 1.0f;
+        f.c1 = o.nesterov ? o.momentum : 1.0f; f.c2 = o.nesterov ? 1.0f : 0.0f;
+        break;
+    case FORGE_OPT_LION:                           // n = sign(b1 m + (1-b1) g); m' = b2 m + (1-b2) g; decoupled decay
+        f.has_m = 1; f.lion = 1; f.l1 = o.beta1; f.l2 = 1.0f - o.beta1; f.a1 = o.beta2; f.a2 = 1.0f - o.beta2;
+        f.decay = static_cast<float>(1.0 - lr * wd);
+        break;
+    case FORGE_OPT_RMSPROP:                        // alpha is passed as beta2
+        f.cwd = o.wd; f.v_mode = V_EMA; f.b1 = o.beta2; f.b2 = 1.0f - o.beta2; f.has_denom = 1; f.e2 = o.eps;
+        break;
+    case FORGE_OPT_ADAGRAD:
+        f.cwd = o.wd; f.v_mode = V_EMA; f.b1 = 1.0f; f.b2 = 1.0f; f.has_denom = 1; f.e2 = o.eps;
+        break;
+    case FORGE_OPT_ADAMAX:                         // u = max(b2 u, |g'| + eps); w -= lr/(1-b1^t) m/u
+        f.cwd = o.wd; f.has_m = 1; f.a1 = o.beta1; f.a2 = 1.0f - o.beta1; f.c1 = 1.0f; f.c2 = 0.0f;
+        f.v_mode = V_MAX; f.b1 = o.beta2; f.e2 = o.eps; f.has_denom = 1;
+        f.step = static_cast<float>(lr / (1.0 - std::pow(b1, t)));
+        break;
+    case FORGE_OPT_NADAM: {                        // torch.optim.NAdam: momentum_decay 4e-3, coupled decay
+        double prod = 1.0;
+        for (int64_t i = 1; i <= o.step; ++i) prod *= nadam_mu(b1, i);
+        const double mu_t = nadam_mu(b1, o.step), mu_n = nadam_mu(b1, o.step + 1);
+        f.cwd = o.wd; f.has_m = 1; f.a1 = o.beta1; f.a2 = 1.0f - o.beta1;
+        f.v_mode = V_EMA; f.b1 = o.beta2; f.b2 = 1.0f - o.beta2; f.has_denom = 1;
+        f.e1 = static_cast<float>(1.0 / std::sqrt(1.0 - std::pow(b2, t))); f.e2 = o.eps;
+        f.c1 = static_cast<float>(lr * mu_n / (1.0 - prod * mu_n));
+        f.c2 = static_cast<float>(lr * (1.0 - mu_t) / (1.0 - prod));
+        f.step = 1.0f;
+        break; }
+    case FORGE_OPT_RADAM: {                        // torch.optim.RAdam, coupled decay
+        const double bc1 = 1.0 - std::pow(b1, t), bc2 = 1.0 - std::pow(b2, t);
+        const double rho_inf = 2.0 / (1.0 - b2) - 1.0, rho_t = rho_inf - 2.0 * t * std::pow(b2, t) / bc2;
+        f.cwd = o.wd; f.has_m = 1; f.a1 = o.beta1; f.a2 = 1.0f - o.beta1; f.c1 = 1.0f; f.c2 = 0.0f;
+        f.v_mode = V_EMA; f.b1 = o.beta2; f.b2 = 1.0f - o.beta2; f.e2 = o.eps;
+        if (rho_t > 5.0) {
+            const double rect = std::sqrt((rho_t - 4.0) * (rho_t - 2.0) * rho_inf / ((rho_inf - 4.0) * (rho_inf - 2.0) * rho_t));
+            f.has_denom = 1;
+            f.step = static_cast<float>(lr * std::sqrt(bc2) * rect / bc1);
+        } else {
+            f.step = static_cast<float>(lr / bc1);
+        }
+        break; }
+    default: break;
+    }
+    (void)eps; (void)mu;
+    f.kind = !f.has_m ? (f.v_mode == V_NONE ? FK_PLAIN : FK_V)
+                      : (f.lion ? FK_LION
+                                : (f.v_mode == V_NONE ? FK_M
+                                                      : (f.v_mode == V_MAX ? FK_MV_MAX : (f.has_denom ? FK_MV : FK_MV_NODENOM))));
+    return f;
+}
+
+// chunk geometry per state count: the ring is sized so that ~160 KB of state are resident
+template <int MDT>
+forge_status_t dispatch_family(const forge_problem_t *probs, int count, int nst, const FamilyScalars &fs,
+                               const DeviceInfo &dev, cudaStream_t stream) {
+    int maxT = 0;
+    for (int i = 0; i < count; ++i) maxT = probs[i].T > maxT ? probs[i].T : maxT;
+    AdamWScalars hp;
+    std::memset(&hp, 0, sizeof(hp));
+    const bool big = maxT > 1024;
+    const int forced = env_int("FORGE_CFG", -1);   // tuning sweeps only
+    if (nst == 0) {
+        if (big) return launch_fused<MDT, MODE_FAMILY, 64, 4, 4, 2, 64, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
+        if (forced == 1) return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 128, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
+        if (forced == 2) return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 64, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
+        if (forced == 3) return launch_fused<MDT, MODE_FAMILY, 32, 4, 2, 2, 128, 256, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
+        return launch_fused<MDT, MODE_FAMILY, 32, 4, 6, 2, 64, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
+    }
+    if (nst == 1) {
+        if (big) return launch_fused<MDT, MODE_FAMILY, 64, 4, 2, 2, 64, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
+        if (forced == 1) return launch_fused<MDT, MODE_FAMILY, 32, 4, 6, 2, 64, 64, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
+        if (forced == 2) return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 64, 64, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
+        if (forced == 3) return launch_fused<MDT, MODE_FAMILY, 32, 4, 2, 2, 64, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
+        // measured (momentum, fp32 / bf16 state): 32 x 128 x 4 slots 465 / 376 us, 64 x 64 x 4 483 / 396, 64 x 128 x 2 514 / 417
+        return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
+    }
+    if (big) return launch_fused<MDT, MODE_FAMILY, 64, 4, 2, 2, 64, 64, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
+    if (MDT == MDT_FP32) return launch_fused<MDT, MODE_FAMILY, 32, 4, 2, 2, 64, 128, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
+    return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 64, 64, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
 }
 
 }  // namespace
@@ -321,6 +435,43 @@ forge_status_t forge_wgrad_adamw(const void *X, const void *dY, void *W, void *m
     p.X = X; p.dY = dY; p.W = W; p.m = m; p.v = v; p.m_scale = m_scale; p.v_scale = v_scale;
     p.T = T; p.out = out; p.in = in;
     return forge_wgrad_adamw_grouped(&p, 1, step, lr, beta1, beta2, eps, wd, moment_dtype, stream);
+}
+
+forge_status_t forge_wgrad_step_grouped(const forge_problem_t *problems, int32_t count, const forge_opt_desc_t *opt,
+                                        forge_moment_dtype_t state_dtype, forge_stream_t stream) {
+    if (!problems || !opt) return FORGE_ERR_NULL_PTR;
+    if (count < 1) return FORGE_ERR_BAD_SHAPE;
+    const int fam = static_cast<int>(opt->family);
+    if (fam < FORGE_OPT_ADAMW || fam > FORGE_OPT_RADAM) return FORGE_ERR_BAD_HYPERPARAM;
+    if (fam == FORGE_OPT_ADAMW)
+        return forge_wgrad_adamw_grouped(problems, count, opt->step, opt->lr, opt->beta1, opt->beta2, opt->eps, opt->wd,
+                                         state_dtype, stream);
+    const int mdt = static_cast<int>(state_dtype);
+    if (mdt != FORGE_MOMENT_FP32 && mdt != FORGE_MOMENT_BF16) return FORGE_ERR_BAD_DTYPE;   // int8 state: AdamW only
+    forge_status_t s = validate_hp(opt->step, opt->lr, opt->beta1, opt->beta2, opt->eps, opt->wd);
+    if (s != FORGE_OK) return s;
+    if (!(opt->momentum >= 0.f && opt->momentum < 1.f)) return FORGE_ERR_BAD_HYPERPARAM;
+    const int nst = family_states(fam);
+    for (int i = 0; i < count; ++i) {
+        const forge_problem_t &p = problems[i];
+        if (!p.X || !p.dY || !p.W) return FORGE_ERR_NULL_PTR;
+        if ((nst >= 1) != (p.m != nullptr) || (nst >= 2) != (p.v != nullptr)) return FORGE_ERR_NULL_PTR;   // exactly the family's states
+        if (p.m_scale || p.v_scale) return FORGE_ERR_BAD_DTYPE;
+        if (p.T < 1 || p.out < 8 || p.in < 8 || (p.out % 8) || (p.in % 8)) return FORGE_ERR_BAD_SHAPE;
+        if (!aligned16(p.X) || !aligned16(p.dY) || !aligned16(p.W) || !aligned16(p.m) || !aligned16(p.v)) return FORGE_ERR_ALIGNMENT;
+    }
+    DeviceInfo dev;
+    s = device_info(dev);
+    if (s != FORGE_OK) return s;
+    const FamilyScalars fs = make_family(*opt);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    for (int i = 0; i < count; i += kMaxProblems) {
+        const int n = (count - i) < kMaxProblems ? (count - i) : kMaxProblems;
+        s = mdt == FORGE_MOMENT_FP32 ? dispatch_family<MDT_FP32>(problems + i, n, nst, fs, dev, st)
+                                     : dispatch_family<MDT_BF16>(problems + i, n, nst, fs, dev, st);
+        if (s != FORGE_OK) return s;
+    }
+    return FORGE_OK;
 }
 
 forge_status_t forge_wgrad_store_g(const void *X, const void *dY, float *G, int32_t T, int32_t out, int32_t in,

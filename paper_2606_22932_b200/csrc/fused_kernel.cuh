@@ -28,6 +28,7 @@
 #include <cuda_runtime.h>
 
 #include "adamw_math.cuh"
+#include "family_math.cuh"
 #include "ptx.cuh"
 
 namespace forge {
@@ -47,7 +48,7 @@ __host__ __device__ constexpr int block_threads(int mdt) { return (kCtrlWarps + 
 constexpr int kTmemCols = 512;  // 2 accumulator buffers x 256 fp32 columns
 
 enum : int { MDT_FP32 = 0, MDT_BF16 = 1, MDT_INT8 = 2 };
-enum : int { MODE_ADAMW = 0, MODE_STORE_G = 1 };
+enum : int { MODE_ADAMW = 0, MODE_STORE_G = 1, MODE_FAMILY = 2 };   // FAMILY: family_math.cuh, 0-2 state tensors
 
 struct alignas(64) ProblemDesc {
     CUtensorMap map_dY;  // [T, out] bf16, box {64, kBlockK}, SWIZZLE_128B
@@ -68,6 +69,7 @@ struct alignas(64) ProblemDesc {
 struct alignas(64) KernelParams {
     ProblemDesc prob[kMaxProblems];
     AdamWScalars hp;
+    FamilyScalars fs;    // MODE_FAMILY only
     int32_t num_problems;
     int32_t total_tiles;
     int32_t pad_;
@@ -86,8 +88,10 @@ enum : int { DBG_NO_MAINLOOP = 1, DBG_NO_STATE = 2, DBG_NO_EPILOGUE = 4 };
 // ring: with fp32 moments 128 x 32 chunks x 4 slots give 0.83 of the copy peak, 64 x 64 x 4 slots 0.86
 // and 64 x 128 x 2 slots 0.90 (profiles/r01_summary.md) -- longer contiguous runs per DRAM page and
 // fewer pages open at once matter more than bytes in flight.
-template <int MDT, int kBlockK, int kStages, int kStateStages, int CG = 1, int CM_ = 64, int CN_ = 64, int P1C_ = 128, int P1S_ = 2>
+template <int MDT, int kBlockK, int kStages, int kStateStages, int CG = 1, int CM_ = 64, int CN_ = 64, int P1C_ = 128, int P1S_ = 2,
+          int NST_ = 2>
 struct KernelCfg {
+    static constexpr int NST = NST_;                        // state tensors besides W in a chunk (AdamW: m, v)
     static constexpr int kMomBytes = (MDT == MDT_FP32) ? 4 : (MDT == MDT_BF16 ? 2 : 1);
     static constexpr int A_STAGE = kBlockK * 128 * (BLOCK_M / 64);
     static constexpr int B_STAGE = kBlockK * 128 * (BLOCK_N / 64) / CG;
@@ -111,7 +115,7 @@ struct KernelCfg {
     static constexpr int M_BOXES = CN / M_BOX_COLS;
     static constexpr int M_BOX = CM * M_ROW;
     static constexpr int M_CHUNK = M_BOXES * M_BOX;
-    static constexpr int ST_STAGE = W_CHUNK + 2 * M_CHUNK;
+    static constexpr int ST_STAGE = W_CHUNK + NST * M_CHUNK;
     static constexpr int ST_TX_BYTES = ST_STAGE;
     // INT8: a second, read-only ring feeds the absmax pass: chunks of 128 rows x 128 columns of m and
     // of v codes (one 128 x 128 B box each), two slots = one tile
@@ -212,6 +216,76 @@ __device__ __forceinline__ void epi_sub_fp(const AdamWScalars &hp, const uint32_
             sts128(av, make_uint4(f32x2_to_bf16x2(v[0]), f32x2_to_bf16x2(v[1]), f32x2_to_bf16x2(v[2]), f32x2_to_bf16x2(v[3])));
         }
         sts128(aw, make_uint4(f32x2_to_bf16x2(w[0]), f32x2_to_bf16x2(w[1]), f32x2_to_bf16x2(w[2]), f32x2_to_bf16x2(w[3])));
+    }
+}
+
+// the other coordinate-wise families (family_math.cuh): 0, 1 or 2 state tensors in the chunk image
+template <int MDT, class Cfg, bool HAS_M, int V_MODE, bool LION, bool DENOM>
+__device__ __forceinline__ void epi_sub_family_t(const FamilyScalars &fs, const uint32_t (&g)[32],
+                                                 const SubAddr<Cfg> &a, uint32_t row) {
+    constexpr int NST = Cfg::NST;
+    constexpr bool ONE_IS_V = (NST == 1) && !HAS_M;        // a single state tensor is the momentum when the
+                                                           // family has one, else the second-moment state
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const uint32_t aw = a.w + swz<Cfg::W_ROW>(row, a.pw + j);
+        const uint4 wq = lds128(aw);
+        f32x2 w[4] = {bf16x2_to_f32x2(wq.x), bf16x2_to_f32x2(wq.y), bf16x2_to_f32x2(wq.z), bf16x2_to_f32x2(wq.w)};
+        f32x2 s[2][4];                                     // s[0]: state 0, s[1]: state 1
+        uint32_t as[2][2];
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) s[t][e] = 0ull;
+            if (t >= NST) continue;
+            const uint32_t base = t == 0 ? a.m : a.v;
+            if constexpr (MDT == MDT_FP32) {
+                as[t][0] = base + swz<Cfg::M_ROW>(row, a.pm + 2 * j);
+                as[t][1] = base + swz<Cfg::M_ROW>(row, a.pm + 2 * j + 1);
+                const uint4 x = lds128(as[t][0]), y = lds128(as[t][1]);
+                s[t][0] = pk2u(x.x, x.y); s[t][1] = pk2u(x.z, x.w); s[t][2] = pk2u(y.x, y.y); s[t][3] = pk2u(y.z, y.w);
+            } else {
+                as[t][0] = base + swz<Cfg::M_ROW>(row, a.pm + j);
+                const uint4 x = lds128(as[t][0]);
+                s[t][0] = bf16x2_to_f32x2(x.x); s[t][1] = bf16x2_to_f32x2(x.y);
+                s[t][2] = bf16x2_to_f32x2(x.z); s[t][3] = bf16x2_to_f32x2(x.w);
+            }
+        }
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const f32x2 gg = pk2u(g[8 * j + 2 * e], g[8 * j + 2 * e + 1]);
+            if constexpr (ONE_IS_V) family_update2<HAS_M, V_MODE, LION, DENOM>(fs, gg, w[e], s[1][e], s[0][e]);
+            else family_update2<HAS_M, V_MODE, LION, DENOM>(fs, gg, w[e], s[0][e], s[1][e]);
+        }
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+            if (t >= NST) continue;
+            if constexpr (MDT == MDT_FP32) {
+                sts128(as[t][0], make_uint4(lo2u(s[t][0]), hi2u(s[t][0]), lo2u(s[t][1]), hi2u(s[t][1])));
+                sts128(as[t][1], make_uint4(lo2u(s[t][2]), hi2u(s[t][2]), lo2u(s[t][3]), hi2u(s[t][3])));
+            } else {
+                sts128(as[t][0], make_uint4(f32x2_to_bf16x2(s[t][0]), f32x2_to_bf16x2(s[t][1]),
+                                            f32x2_to_bf16x2(s[t][2]), f32x2_to_bf16x2(s[t][3])));
+            }
+        }
+        sts128(aw, make_uint4(f32x2_to_bf16x2(w[0]), f32x2_to_bf16x2(w[1]), f32x2_to_bf16x2(w[2]), f32x2_to_bf16x2(w[3])));
+    }
+}
+
+// one uniform switch per sub-block on the family's structure; only the kinds its state count allows
+template <int MDT, class Cfg>
+__device__ __forceinline__ void epi_sub_family(const FamilyScalars &fs, const uint32_t (&g)[32],
+                                               const SubAddr<Cfg> &a, uint32_t row) {
+    if constexpr (Cfg::NST == 0) {
+        epi_sub_family_t<MDT, Cfg, false, V_NONE, false, false>(fs, g, a, row);
+    } else if constexpr (Cfg::NST == 1) {
+        if (fs.kind == FK_M) epi_sub_family_t<MDT, Cfg, true, V_NONE, false, false>(fs, g, a, row);
+        else if (fs.kind == FK_LION) epi_sub_family_t<MDT, Cfg, true, V_NONE, true, false>(fs, g, a, row);
+        else epi_sub_family_t<MDT, Cfg, false, V_EMA, false, true>(fs, g, a, row);
+    } else {
+        if (fs.kind == FK_MV) epi_sub_family_t<MDT, Cfg, true, V_EMA, false, true>(fs, g, a, row);
+        else if (fs.kind == FK_MV_MAX) epi_sub_family_t<MDT, Cfg, true, V_MAX, false, true>(fs, g, a, row);
+        else epi_sub_family_t<MDT, Cfg, true, V_EMA, false, false>(fs, g, a, row);
     }
 }
 
@@ -417,10 +491,12 @@ __device__ __forceinline__ void int8_loader(const KernelParams &P, uint32_t rank
 // ---------------------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------------------
-template <int MDT, int MODE, int kBlockK, int kStages, int kStateStages, int CG, int CM, int CN, int P1C, int P1S>
+template <int MDT, int MODE, int kBlockK, int kStages, int kStateStages, int CG, int CM, int CN, int P1C, int P1S, int NST>
 __global__ void __launch_bounds__(block_threads(MDT), 1)
 forge_fused_kernel(const __grid_constant__ KernelParams P) {
-    using Cfg = KernelCfg<MDT, kBlockK, kStages, kStateStages, CG, CM, CN, P1C, P1S>;
+    using Cfg = KernelCfg<MDT, kBlockK, kStages, kStateStages, CG, CM, CN, P1C, P1S, NST>;
+    static_assert(MODE == MODE_FAMILY || NST == 2, "AdamW and the store-G twin use the two-state chunk image");
+    static_assert(MODE != MODE_FAMILY || MDT != MDT_INT8, "int8 state is implemented for AdamW only");
     constexpr int CHUNKS = Cfg::CHUNKS;
     const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;   // rank 0 = the pair's leader
     extern __shared__ uint8_t smem_raw[];
@@ -557,7 +633,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         if constexpr (MDT == MDT_INT8) {
             if (lane == 0 && !(P.debug & DBG_NO_STATE))
                 int8_loader<Cfg, kStateStages, CG>(P, rank, first_tile, tile_step, sST, bar_st_full, bar_st_empty, i8);
-        } else if (MODE == MODE_ADAMW && lane == 0 && !(P.debug & DBG_NO_STATE)) {
+        } else if (MODE != MODE_STORE_G && lane == 0 && !(P.debug & DBG_NO_STATE)) {
             uint32_t ci = 0;  // running chunk counter
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step) {
                 const TileCoord tc = decode_tile<CG>(P, tile, rank);
@@ -572,13 +648,17 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
 #pragma unroll
                     for (int i = 0; i < Cfg::W_BOXES; ++i)
                         tma_load_2d(base + i * Cfg::W_BOX, &pd.map_W, full, x + i * Cfg::W_BOX_COLS, y, kEvictFirst);
+                    if constexpr (NST >= 1) {
 #pragma unroll
-                    for (int i = 0; i < Cfg::M_BOXES; ++i)
-                        tma_load_2d(base + Cfg::W_CHUNK + i * Cfg::M_BOX, &pd.map_m, full, x + i * Cfg::M_BOX_COLS, y, kEvictFirst);
+                        for (int i = 0; i < Cfg::M_BOXES; ++i)
+                            tma_load_2d(base + Cfg::W_CHUNK + i * Cfg::M_BOX, &pd.map_m, full, x + i * Cfg::M_BOX_COLS, y, kEvictFirst);
+                    }
+                    if constexpr (NST >= 2) {
 #pragma unroll
-                    for (int i = 0; i < Cfg::M_BOXES; ++i)
-                        tma_load_2d(base + Cfg::W_CHUNK + Cfg::M_CHUNK + i * Cfg::M_BOX, &pd.map_v, full,
-                                    x + i * Cfg::M_BOX_COLS, y, kEvictFirst);
+                        for (int i = 0; i < Cfg::M_BOXES; ++i)
+                            tma_load_2d(base + Cfg::W_CHUNK + Cfg::M_CHUNK + i * Cfg::M_BOX, &pd.map_v, full,
+                                        x + i * Cfg::M_BOX_COLS, y, kEvictFirst);
+                    }
                 }
             }
         }
@@ -606,15 +686,17 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                     const int x = tc.tn * BLOCK_N + (c / Cfg::RB) * CN, y = tc.tm * BLOCK_M + (c % Cfg::RB) * CM;
                     if (P.debug & DBG_NO_STATE) {
                     } else {
-                        if constexpr (MODE == MODE_ADAMW) {
+                        if constexpr (MODE != MODE_STORE_G) {
 #pragma unroll
                             for (int i = 0; i < Cfg::W_BOXES; ++i)
                                 tma_store_2d(&pd.map_W, base + i * Cfg::W_BOX, x + i * Cfg::W_BOX_COLS, y, kEvictFirst);
                         }
+                        if constexpr (NST >= 1) {
 #pragma unroll
-                        for (int i = 0; i < Cfg::M_BOXES; ++i)      // MODE_STORE_G: the m image carries G
-                            tma_store_2d(&pd.map_m, base + Cfg::W_CHUNK + i * Cfg::M_BOX, x + i * Cfg::M_BOX_COLS, y, kEvictFirst);
-                        if constexpr (MODE == MODE_ADAMW) {
+                            for (int i = 0; i < Cfg::M_BOXES; ++i)      // MODE_STORE_G: the m image carries G
+                                tma_store_2d(&pd.map_m, base + Cfg::W_CHUNK + i * Cfg::M_BOX, x + i * Cfg::M_BOX_COLS, y, kEvictFirst);
+                        }
+                        if constexpr (MODE != MODE_STORE_G && NST >= 2) {
 #pragma unroll
                             for (int i = 0; i < Cfg::M_BOXES; ++i)
                                 tma_store_2d(&pd.map_v, base + Cfg::W_CHUNK + Cfg::M_CHUNK + i * Cfg::M_BOX,
@@ -653,7 +735,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                     const uint32_t ci = titer * CHUNKS + cb * Cfg::RB + rb;
                     const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
                     const uint32_t base = sST + s * Cfg::ST_STAGE;
-                    if (MODE == MODE_ADAMW && !(P.debug & DBG_NO_STATE)) mbar_wait(bar_st_full + 8 * s, ph);
+                    if (MODE != MODE_STORE_G && !(P.debug & DBG_NO_STATE)) mbar_wait(bar_st_full + 8 * s, ph);
                     else mbar_wait(bar_st_empty + 8 * s, ph ^ 1u);
                     for (int j32 = (Cfg::SUBS >= 2 ? wg : 0); j32 < Cfg::SUBS; j32 += Cfg::WGS) {
                         uint32_t g[32];
@@ -662,6 +744,8 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                         tmem_ld_wait();
                         if constexpr (MODE == MODE_ADAMW) {
                             if (!(P.debug & DBG_NO_EPILOGUE)) epi_sub_fp<MDT, Cfg>(hp, g, a, row);
+                        } else if constexpr (MODE == MODE_FAMILY) {
+                            epi_sub_family<MDT, Cfg>(P.fs, g, a, row);
                         } else {
                             epi_sub_store_g<Cfg>(g, a, row);
                         }

@@ -1,0 +1,107 @@
+"""GPU parity for the other coordinate-wise optimizer families:
+forge_wgrad_step_grouped through the C ABI against oracle/forge_oracle_families.c on the same seeded inputs.
+Tolerance: W within 1 bf16 ulp of the oracle (+ the fp32 evaluation error of the update) wherever the
+gradient is determined (|g| > 4e, e the fp32 accumulation bound of north_star), elsewhere within the
+family's largest step; state to relative 1e-4 plus the propagated accumulation error."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import forge_oracle as fo
+from paper_2606_22932_b200 import binding as fb
+from paper_2606_22932_b200 import synth
+import parity_util as pu
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+F = np.float32
+
+CASES = {
+    "sgd": dict(lr=1e-2, wd=0.05),
+    "momentum": dict(lr=1e-2, wd=0.05, momentum=0.9),
+    "nesterov": dict(lr=1e-2, wd=0.05, momentum=0.8, nesterov=True),
+    "lion": dict(lr=1e-4, beta1=0.9, beta2=0.99, wd=0.1),
+    "rmsprop": dict(lr=1e-3, beta2=0.99, eps=1e-8, wd=0.01),
+    "adagrad": dict(lr=1e-2, eps=1e-10, wd=0.0),
+    "adamax": dict(lr=2e-3, beta1=0.9, beta2=0.999, eps=1e-8, wd=0.01),
+    "nadam": dict(lr=2e-3, beta1=0.9, beta2=0.999, eps=1e-8, wd=0.01),
+    "radam": dict(lr=1e-3, beta1=0.9, beta2=0.999, eps=1e-8, wd=0.01),
+}
+
+
+def run_case(name, T, out, inn, steps, state_bf16=False, seed=3):
+    fam = "momentum" if name == "nesterov" else name
+    kw = dict(beta1=0.9, beta2=0.999, eps=1e-8, wd=0.0, momentum=0.0, nesterov=False)
+    kw.update(CASES[name])
+    lr = kw.pop("lr")
+    ns = fb.FAMILY_STATES[fam]
+    p0 = synth.make_problem("f", T, out, inn, seed, sigma_dy=1e-2)
+    Wg = p0.W.to(DEV).clone()
+    Wo = synth.bf16_bits(p0.W).copy()
+    sdt = torch.bfloat16 if state_bf16 else torch.float32
+    # non-trivial initial state (v-like states non-negative), identical bits on both sides
+    init = [p0.m * 10, p0.v.sqrt() if fam == "adamax" else p0.v * 100][:ns] if fam not in ("rmsprop", "adagrad") else [p0.v * 100]
+    sg = [t.to(sdt).to(DEV) for t in init]
+    so = [synth.bf16_bits(t.to(sdt)).copy() if state_bf16 else t.numpy().copy() for t in init]
+    exact = []
+    for step in steps:
+        pin = synth.make_problem("f", T, out, inn, seed + step, sigma_dy=1e-2)
+        X, dY = pin.X.to(DEV), pin.dY.to(DEV)
+        prob = dict(X=X, dY=dY, W=Wg, m=sg[0] if ns >= 1 else None, v=sg[1] if ns >= 2 else None)
+        fb.forge_wgrad_step_grouped([prob], fam, step, lr, state_dtype=fb.BF16 if state_bf16 else fb.FP32, **kw)
+        G, E = fo.wgrad(synth.bf16_bits(pin.dY), synth.bf16_bits(pin.X), with_abs=True)
+        Wprev = fo.bf16_to_f64(Wo)
+        fo.family_step(fam, Wo, *(so + [None] * (2 - ns)), G, step, lr, kw["beta1"], kw["beta2"], kw["eps"], kw["wd"],
+                       kw["momentum"], kw["nesterov"])
+        torch.cuda.synchronize()
+        Wr, Wd = fo.bf16_to_f64(Wo), fo.bf16_to_f64(synth.bf16_bits(Wg))
+        e = T * 2.0 ** -23 * E
+        dW = np.abs(Wd - Wr)
+        # one bf16 ulp (the larger binade's when the two results straddle a power of two) + fp32 evaluation error
+        # and, for the rules that are LINEAR in g (SGD, momentum), the accumulation bound itself: dW = lr * dg
+        # (it only matters where W - lr*g cancels to ~0 and an ulp of the result is far below fp32 eps of W)
+        ulp = (np.maximum(pu.bf16_ulp(Wr), pu.bf16_ulp(Wd)) + 2.0 ** -20 * (np.abs(Wprev) + np.abs(Wr - Wprev))
+               + 2 * lr * e)
+        big = max(4 * lr, 4 * np.abs(Wr - Wprev).max())            # the family's largest step (sign-like rules flip by 2 steps)
+        sure = np.abs(G) > 4 * e
+        bad = np.where(sure, dW > len(exact) * ulp + ulp, dW > big)
+        assert not bad.any(), f"{name} step {step}: {bad.sum()} W outside tolerance, worst {dW.max():.3e}"
+        exact.append(float((synth.bf16_bits(Wg) == Wo).mean()))
+        for a, b in zip(sg, so):
+            ag = fo.bf16_to_f64(synth.bf16_bits(a)) if state_bf16 else a.cpu().numpy().astype(np.float64)
+            bo = fo.bf16_to_f64(b) if state_bf16 else b.astype(np.float64)
+            tol = (2.0 ** -7 if state_bf16 else 2e-4) * np.abs(bo) + 8 * e * (1 + 2 * np.abs(G)) + 1e-30
+            assert np.all(np.abs(ag - bo) <= tol), f"{name} step {step}: state off by {np.abs(ag - bo).max():.3e}"
+        # chain both sides from the ORACLE's values so one-ulp flips do not accumulate into the next step's check
+        Wg.copy_(synth.bits_to_bf16(Wo).to(DEV))
+        for a, b in zip(sg, so):
+            a.copy_((synth.bits_to_bf16(b) if state_bf16 else torch.from_numpy(b)).to(DEV))
+    assert min(exact) > 0.98, f"{name}: only {min(exact):.4f} of W bit-identical to the oracle"
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_family_small_shapes_three_steps_fp32_state(name):
+    run_case(name, T=200, out=136, inn=264, steps=(1, 2, 7))
+
+
+@pytest.mark.parametrize("name", ["momentum", "lion", "rmsprop", "adamax", "radam"])
+def test_family_bf16_state(name):
+    run_case(name, T=96, out=256, inn=512, steps=(1, 6), state_bf16=True)
+
+
+@pytest.mark.parametrize("name", ["sgd", "lion", "nadam"])
+def test_family_large_t_variant(name):
+    run_case(name, T=2048, out=256, inn=512, steps=(3,))
+
+
+def test_family_argument_validation():
+    p = synth.make_problem("f", 64, 128, 256, 1)
+    X, dY, W, m = p.X.to(DEV), p.dY.to(DEV), p.W.to(DEV), p.m.to(DEV)
+    W0 = W.clone()
+    # SGD must not be given state; momentum must; int8 state is AdamW-only; bad momentum
+    assert fb.forge_wgrad_step_grouped([dict(X=X, dY=dY, W=W, m=m, v=None)], "sgd", 1, 1e-2, check=False) == 1
+    assert fb.forge_wgrad_step_grouped([dict(X=X, dY=dY, W=W, m=None, v=None)], "momentum", 1, 1e-2, check=False) == 1
+    assert fb.forge_wgrad_step_grouped([dict(X=X, dY=dY, W=W, m=m, v=None)], "lion", 1, 1e-2, state_dtype=fb.INT8, check=False) == 5
+    assert fb.forge_wgrad_step_grouped([dict(X=X, dY=dY, W=W, m=m, v=None)], "momentum", 1, 1e-2, momentum=1.5, check=False) == 4
+    torch.cuda.synchronize()
+    assert torch.equal(W, W0)
