@@ -128,6 +128,14 @@ typedef struct {
 forge_status_t forge_wgrad_step_grouped(const forge_problem_t *problems, int32_t count, const forge_opt_desc_t *opt,
                                         forge_moment_dtype_t state_dtype, forge_stream_t stream);
 
+/* Accumulate-into-state (the paper's regime 2; Muon's A-step): for every problem
+ * B <- mu * B + dY^T X in place, "through the GEMM's own beta": no gradient is materialised and no weight is read
+ * or written.  B[out,in] (fp32 or bf16) is passed in forge_problem_t.m; W, v and the scales MUST be NULL
+ * (FORGE_ERR_BAD_DTYPE otherwise).  mu >= 0 and finite.  The state-global weight update that follows in Muon
+ * (Newton-Schulz over the resident B) is out of scope. */
+forge_status_t forge_wgrad_accumulate_grouped(const forge_problem_t *problems, int32_t count, float mu,
+                                              forge_moment_dtype_t state_dtype, forge_stream_t stream);
+
 /* End-to-end convenience entry with HOST buffers (used for the e2e measurement): copies X, dY and
  * the state to device scratch it allocates and frees itself, runs forge_wgrad_adamw, copies the
  * state back and synchronises.  Same validation and return codes; all pointers are host pointers. */

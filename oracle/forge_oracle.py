@@ -58,6 +58,8 @@ def lib() -> ctypes.CDLL:
         L.forge_oracle_bf16_from_double_array.restype = None
         L.forge_oracle_bf16_from_double_array.argtypes = [c_void_p, c_void_p, c_size_t]
         L.forge_oracle_num_threads.restype = c_int
+        L.forge_oracle_accumulate.restype = None
+        L.forge_oracle_accumulate.argtypes = [c_void_p, c_int, c_void_p, c_size_t, c_float]
         L.forge_oracle_family_step.restype = None
         L.forge_oracle_family_step.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int, c_void_p, c_size_t,
                                                c_long, c_float, c_float, c_float, c_float, c_float, c_float,
@@ -194,3 +196,12 @@ def family_step(family: str, W, s0, s1, G, step, lr, beta1=0.9, beta2=0.999, eps
     lib().forge_oracle_family_step(FAMILIES[family], _p(W), _p(s0), _p(s1), int(bf16), _p(G), W.size, int(step),
                                    lr, beta1, beta2, eps, wd, momentum, int(bool(nesterov)), _p(Wd))
     return Wd
+
+
+def accumulate(B, G, mu):
+    """In place B <- mu*B + G (Muon's A-step); B float32 or uint16 bf16 bits, G float64."""
+    _chk(G, np.float64, "G")
+    bf16 = B.dtype == np.uint16
+    _chk(B, np.uint16 if bf16 else np.float32, "B")
+    assert B.shape == G.shape
+    lib().forge_oracle_accumulate(_p(B), int(bf16), _p(G), B.size, mu)

@@ -143,3 +143,13 @@ void forge_oracle_family_step(int family, uint16_t *W, void *s0, void *s1, int s
         if (Wd) Wd[i] = w1;
     }
 }
+
+/* Accumulate-into-state, the paper's regime 2 ("B <- mu B + G is tile-local and affine, so the
+ * weight-gradient multiply accumulates in place into the momentum buffer through the GEMM's own beta";
+ * PAPER.md:757-759 Muon's A-step).  Per coordinate in fp64, one rounding to the storage type. */
+void forge_oracle_accumulate(void *B, int state_bf16, const double *G, size_t n, float mu)
+{
+    const double m = (double)mu;
+#pragma omp parallel for schedule(static)
+    for (size_t i = 0; i < n; ++i) st(B, i, state_bf16, m * ld(B, i, state_bf16) + G[i]);
+}

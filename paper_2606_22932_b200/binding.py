@@ -21,7 +21,7 @@ QBLOCK = 256
 STATUS_NAMES = ["FORGE_OK", "FORGE_ERR_NULL_PTR", "FORGE_ERR_BAD_SHAPE", "FORGE_ERR_ALIGNMENT",
                 "FORGE_ERR_BAD_HYPERPARAM", "FORGE_ERR_BAD_DTYPE", "FORGE_ERR_UNSUPPORTED_ARCH",
                 "FORGE_ERR_CUDA"]
-EXPORTS = ["forge_wgrad_adamw", "forge_wgrad_adamw_grouped", "forge_wgrad_step_grouped", "forge_wgrad_adamw_host",
+EXPORTS = ["forge_wgrad_adamw", "forge_wgrad_adamw_grouped", "forge_wgrad_step_grouped", "forge_wgrad_accumulate_grouped", "forge_wgrad_adamw_host",
            "forge_wgrad_store_g", "forge_adamw_from_g", "forge_workspace_bytes", "forge_launch_count",
            "forge_last_cuda_error", "forge_status_string", "forge_version"]
 
@@ -68,6 +68,8 @@ def lib() -> ctypes.CDLL:
         L.forge_wgrad_step_grouped.restype = ctypes.c_int
         L.forge_wgrad_step_grouped.argtypes = [ctypes.POINTER(forge_problem_t), c_int32, ctypes.POINTER(forge_opt_desc_t),
                                                ctypes.c_int, c_void_p]
+        L.forge_wgrad_accumulate_grouped.restype = ctypes.c_int
+        L.forge_wgrad_accumulate_grouped.argtypes = [ctypes.POINTER(forge_problem_t), c_int32, c_float, ctypes.c_int, c_void_p]
         L.forge_wgrad_adamw_host.restype = ctypes.c_int
         L.forge_wgrad_adamw_host.argtypes = [c_void_p] * 7 + [c_int32] * 3 + hp + [ctypes.c_int]
         L.forge_wgrad_store_g.restype = ctypes.c_int
@@ -122,8 +124,8 @@ def make_problem_array(problems):
         g = p.get if isinstance(p, dict) else (lambda k, d=None, p=p: getattr(p, k, d))
         X, dY = g("X"), g("dY")
         arr[i].X, arr[i].dY = X.data_ptr(), dY.data_ptr()
-        m, v = g("m"), g("v")
-        arr[i].W = g("W").data_ptr()
+        m, v, W = g("m"), g("v"), g("W")
+        arr[i].W = None if W is None else W.data_ptr()
         arr[i].m = None if m is None else m.data_ptr()
         arr[i].v = None if v is None else v.data_ptr()
         ms, vs = g("m_scale"), g("v_scale")
@@ -154,6 +156,16 @@ def forge_wgrad_step_grouped(problems, family: str, step, lr, beta1=0.9, beta2=0
     st = lib().forge_wgrad_step_grouped(arr, len(arr), ctypes.byref(desc), state_dtype, _stream(stream))
     if check:
         _check(st, "forge_wgrad_step_grouped")
+    return st
+
+
+def forge_wgrad_accumulate_grouped(problems, mu, state_dtype=FP32, stream=None, check=True) -> int:
+    """include/forge.h forge_wgrad_accumulate_grouped: B <- mu*B + dY^T X in place; problems carry
+    X, dY and m = B only."""
+    arr = make_problem_array(problems)
+    st = lib().forge_wgrad_accumulate_grouped(arr, len(arr), mu, state_dtype, _stream(stream))
+    if check:
+        _check(st, "forge_wgrad_accumulate_grouped")
     return st
 
 

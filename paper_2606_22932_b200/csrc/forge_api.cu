@@ -151,7 +151,7 @@ template <int MDT, int MODE, int BK, int ST, int SS, int CG = 1, int CM = 64, in
           int NST = 2>
 forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamWScalars &hp,
                             const DeviceInfo &dev, cudaStream_t stream, const FamilyScalars *fs = nullptr) {
-    using Cfg = KernelCfg<MDT, BK, ST, SS, CG, CM, CN, P1C, P1S, NST>;
+    using Cfg = KernelCfg<MDT, BK, ST, SS, CG, CM, CN, P1C, P1S, NST, (MODE == MODE_ACCUM) ? 0 : 1>;
     auto kernel = forge_fused_kernel<MDT, MODE, BK, ST, SS, CG, CM, CN, P1C, P1S, NST>;
     static std::once_flag once;
     static cudaError_t attr_err = cudaSuccess;
@@ -176,8 +176,9 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
         ok &= encode_2d(&d.map_dY, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.dY, p.T, p.out, 64, BK, CU_TENSOR_MAP_SWIZZLE_128B);
         ok &= encode_2d(&d.map_X, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.X, p.T, p.in, 64, BK, CU_TENSOR_MAP_SWIZZLE_128B);
         if (MODE != MODE_STORE_G) {
-            ok &= encode_2d(&d.map_W, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.W, p.out, p.in, Cfg::W_BOX_COLS, CM,
-                            swizzle_for_row_bytes(Cfg::W_ROW));
+            if (MODE != MODE_ACCUM)
+                ok &= encode_2d(&d.map_W, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.W, p.out, p.in, Cfg::W_BOX_COLS, CM,
+                                swizzle_for_row_bytes(Cfg::W_ROW));
             if (NST >= 1)
                 ok &= encode_2d(&d.map_m, mom_dt, Cfg::kMomBytes, p.m, p.out, p.in, Cfg::M_BOX_COLS, CM,
                                 swizzle_for_row_bytes(Cfg::M_ROW));
@@ -469,6 +470,45 @@ forge_status_t forge_wgrad_step_grouped(const forge_problem_t *problems, int32_t
         const int n = (count - i) < kMaxProblems ? (count - i) : kMaxProblems;
         s = mdt == FORGE_MOMENT_FP32 ? dispatch_family<MDT_FP32>(problems + i, n, nst, fs, dev, st)
                                      : dispatch_family<MDT_BF16>(problems + i, n, nst, fs, dev, st);
+        if (s != FORGE_OK) return s;
+    }
+    return FORGE_OK;
+}
+
+forge_status_t forge_wgrad_accumulate_grouped(const forge_problem_t *problems, int32_t count, float mu,
+                                              forge_moment_dtype_t state_dtype, forge_stream_t stream) {
+    if (!problems) return FORGE_ERR_NULL_PTR;
+    if (count < 1) return FORGE_ERR_BAD_SHAPE;
+    const int mdt = static_cast<int>(state_dtype);
+    if (mdt != FORGE_MOMENT_FP32 && mdt != FORGE_MOMENT_BF16) return FORGE_ERR_BAD_DTYPE;
+    if (!std::isfinite(mu) || mu < 0.f) return FORGE_ERR_BAD_HYPERPARAM;
+    int maxT = 0;
+    for (int i = 0; i < count; ++i) {
+        const forge_problem_t &p = problems[i];
+        if (!p.X || !p.dY || !p.m) return FORGE_ERR_NULL_PTR;
+        if (p.W || p.v || p.m_scale || p.v_scale) return FORGE_ERR_BAD_DTYPE;      // B only: no weight is touched
+        if (p.T < 1 || p.out < 8 || p.in < 8 || (p.out % 8) || (p.in % 8)) return FORGE_ERR_BAD_SHAPE;
+        if (!aligned16(p.X) || !aligned16(p.dY) || !aligned16(p.m)) return FORGE_ERR_ALIGNMENT;
+        maxT = p.T > maxT ? p.T : maxT;
+    }
+    DeviceInfo dev;
+    forge_status_t s = device_info(dev);
+    if (s != FORGE_OK) return s;
+    AdamWScalars hp;
+    std::memset(&hp, 0, sizeof(hp));
+    FamilyScalars fs;
+    std::memset(&fs, 0, sizeof(fs));
+    fs.a1 = mu;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    for (int i = 0; i < count; i += kMaxProblems) {
+        const int n = (count - i) < kMaxProblems ? (count - i) : kMaxProblems;
+        const forge_problem_t *pp = problems + i;
+        if (mdt == FORGE_MOMENT_FP32)
+            s = maxT > 1024 ? launch_fused<MDT_FP32, MODE_ACCUM, 64, 4, 2, 2, 64, 128, 128, 2, 1>(pp, n, hp, dev, st, &fs)
+                            : launch_fused<MDT_FP32, MODE_ACCUM, 32, 4, 4, 2, 32, 128, 128, 2, 1>(pp, n, hp, dev, st, &fs);
+        else
+            s = maxT > 1024 ? launch_fused<MDT_BF16, MODE_ACCUM, 64, 4, 2, 2, 64, 128, 128, 2, 1>(pp, n, hp, dev, st, &fs)
+                            : launch_fused<MDT_BF16, MODE_ACCUM, 32, 4, 4, 2, 32, 128, 128, 2, 1>(pp, n, hp, dev, st, &fs);
         if (s != FORGE_OK) return s;
     }
     return FORGE_OK;

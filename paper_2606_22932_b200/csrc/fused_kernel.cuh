@@ -48,7 +48,8 @@ __host__ __device__ constexpr int block_threads(int mdt) { return (kCtrlWarps + 
 constexpr int kTmemCols = 512;  // 2 accumulator buffers x 256 fp32 columns
 
 enum : int { MDT_FP32 = 0, MDT_BF16 = 1, MDT_INT8 = 2 };
-enum : int { MODE_ADAMW = 0, MODE_STORE_G = 1, MODE_FAMILY = 2 };   // FAMILY: family_math.cuh, 0-2 state tensors
+enum : int { MODE_ADAMW = 0, MODE_STORE_G = 1, MODE_FAMILY = 2,      // FAMILY: family_math.cuh, 0-2 state tensors
+             MODE_ACCUM = 3 };                                        // B <- mu*B + G, no weight
 
 struct alignas(64) ProblemDesc {
     CUtensorMap map_dY;  // [T, out] bf16, box {64, kBlockK}, SWIZZLE_128B
@@ -89,8 +90,9 @@ enum : int { DBG_NO_MAINLOOP = 1, DBG_NO_STATE = 2, DBG_NO_EPILOGUE = 4 };
 // and 64 x 128 x 2 slots 0.90 (profiles/r01_summary.md) -- longer contiguous runs per DRAM page and
 // fewer pages open at once matter more than bytes in flight.
 template <int MDT, int kBlockK, int kStages, int kStateStages, int CG = 1, int CM_ = 64, int CN_ = 64, int P1C_ = 128, int P1S_ = 2,
-          int NST_ = 2>
+          int NST_ = 2, int HASW_ = 1>
 struct KernelCfg {
+    static constexpr int HASW = HASW_;                      // the chunk image carries W (not in MODE_ACCUM)
     static constexpr int NST = NST_;                        // state tensors besides W in a chunk (AdamW: m, v)
     static constexpr int kMomBytes = (MDT == MDT_FP32) ? 4 : (MDT == MDT_BF16 ? 2 : 1);
     static constexpr int A_STAGE = kBlockK * 128 * (BLOCK_M / 64);
@@ -109,7 +111,7 @@ struct KernelCfg {
     static constexpr int W_ROW = W_BOX_COLS * 2;
     static constexpr int W_BOXES = CN / W_BOX_COLS;
     static constexpr int W_BOX = CM * W_ROW;
-    static constexpr int W_CHUNK = W_BOXES * W_BOX;
+    static constexpr int W_CHUNK = HASW ? W_BOXES * W_BOX : 0;
     static constexpr int M_BOX_COLS = CN < 128 / kMomBytes ? CN : 128 / kMomBytes;
     static constexpr int M_ROW = M_BOX_COLS * kMomBytes;
     static constexpr int M_BOXES = CN / M_BOX_COLS;
@@ -286,6 +288,32 @@ __device__ __forceinline__ void epi_sub_family(const FamilyScalars &fs, const ui
         if (fs.kind == FK_MV) epi_sub_family_t<MDT, Cfg, true, V_EMA, false, true>(fs, g, a, row);
         else if (fs.kind == FK_MV_MAX) epi_sub_family_t<MDT, Cfg, true, V_MAX, false, true>(fs, g, a, row);
         else epi_sub_family_t<MDT, Cfg, true, V_EMA, false, false>(fs, g, a, row);
+    }
+}
+
+// accumulate-into-state (regime 2): B <- mu*B + G "through the GEMM's own beta";
+// the chunk image holds B only, no weight is read or written and no gradient exists
+template <int MDT, class Cfg>
+__device__ __forceinline__ void epi_sub_accum(float mu, const uint32_t (&g)[32], const SubAddr<Cfg> &a, uint32_t row) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        f32x2 b[4];
+        if constexpr (MDT == MDT_FP32) {
+            const uint32_t a0 = a.m + swz<Cfg::M_ROW>(row, a.pm + 2 * j), a1 = a.m + swz<Cfg::M_ROW>(row, a.pm + 2 * j + 1);
+            const uint4 x = lds128(a0), y = lds128(a1);
+            b[0] = pk2u(x.x, x.y); b[1] = pk2u(x.z, x.w); b[2] = pk2u(y.x, y.y); b[3] = pk2u(y.z, y.w);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) b[e] = fma2(bc2(mu), b[e], pk2u(g[8 * j + 2 * e], g[8 * j + 2 * e + 1]));
+            sts128(a0, make_uint4(lo2u(b[0]), hi2u(b[0]), lo2u(b[1]), hi2u(b[1])));
+            sts128(a1, make_uint4(lo2u(b[2]), hi2u(b[2]), lo2u(b[3]), hi2u(b[3])));
+        } else {
+            const uint32_t a0 = a.m + swz<Cfg::M_ROW>(row, a.pm + j);
+            const uint4 x = lds128(a0);
+            b[0] = bf16x2_to_f32x2(x.x); b[1] = bf16x2_to_f32x2(x.y); b[2] = bf16x2_to_f32x2(x.z); b[3] = bf16x2_to_f32x2(x.w);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) b[e] = fma2(bc2(mu), b[e], pk2u(g[8 * j + 2 * e], g[8 * j + 2 * e + 1]));
+            sts128(a0, make_uint4(f32x2_to_bf16x2(b[0]), f32x2_to_bf16x2(b[1]), f32x2_to_bf16x2(b[2]), f32x2_to_bf16x2(b[3])));
+        }
     }
 }
 
@@ -494,9 +522,11 @@ __device__ __forceinline__ void int8_loader(const KernelParams &P, uint32_t rank
 template <int MDT, int MODE, int kBlockK, int kStages, int kStateStages, int CG, int CM, int CN, int P1C, int P1S, int NST>
 __global__ void __launch_bounds__(block_threads(MDT), 1)
 forge_fused_kernel(const __grid_constant__ KernelParams P) {
-    using Cfg = KernelCfg<MDT, kBlockK, kStages, kStateStages, CG, CM, CN, P1C, P1S, NST>;
-    static_assert(MODE == MODE_FAMILY || NST == 2, "AdamW and the store-G twin use the two-state chunk image");
-    static_assert(MODE != MODE_FAMILY || MDT != MDT_INT8, "int8 state is implemented for AdamW only");
+    constexpr int HASW = (MODE == MODE_ACCUM) ? 0 : 1;
+    using Cfg = KernelCfg<MDT, kBlockK, kStages, kStateStages, CG, CM, CN, P1C, P1S, NST, HASW>;
+    static_assert(MODE == MODE_FAMILY || MODE == MODE_ACCUM || NST == 2, "AdamW and the store-G twin use the two-state chunk image");
+    static_assert(MODE != MODE_ACCUM || NST == 1, "accumulate-into-state has exactly one state tensor");
+    static_assert((MODE != MODE_FAMILY && MODE != MODE_ACCUM) || MDT != MDT_INT8, "int8 state is implemented for AdamW only");
     constexpr int CHUNKS = Cfg::CHUNKS;
     const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;   // rank 0 = the pair's leader
     extern __shared__ uint8_t smem_raw[];
@@ -645,9 +675,11 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                     mbar_expect_tx(full, Cfg::ST_TX_BYTES);
                     const uint32_t base = sST + s * Cfg::ST_STAGE;
                     const int x = tc.tn * BLOCK_N + (c / Cfg::RB) * CN, y = tc.tm * BLOCK_M + (c % Cfg::RB) * CM;
+                    if constexpr (HASW) {
 #pragma unroll
-                    for (int i = 0; i < Cfg::W_BOXES; ++i)
-                        tma_load_2d(base + i * Cfg::W_BOX, &pd.map_W, full, x + i * Cfg::W_BOX_COLS, y, kEvictFirst);
+                        for (int i = 0; i < Cfg::W_BOXES; ++i)
+                            tma_load_2d(base + i * Cfg::W_BOX, &pd.map_W, full, x + i * Cfg::W_BOX_COLS, y, kEvictFirst);
+                    }
                     if constexpr (NST >= 1) {
 #pragma unroll
                         for (int i = 0; i < Cfg::M_BOXES; ++i)
@@ -686,7 +718,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                     const int x = tc.tn * BLOCK_N + (c / Cfg::RB) * CN, y = tc.tm * BLOCK_M + (c % Cfg::RB) * CM;
                     if (P.debug & DBG_NO_STATE) {
                     } else {
-                        if constexpr (MODE != MODE_STORE_G) {
+                        if constexpr (MODE != MODE_STORE_G && HASW) {
 #pragma unroll
                             for (int i = 0; i < Cfg::W_BOXES; ++i)
                                 tma_store_2d(&pd.map_W, base + i * Cfg::W_BOX, x + i * Cfg::W_BOX_COLS, y, kEvictFirst);
@@ -746,6 +778,8 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                             if (!(P.debug & DBG_NO_EPILOGUE)) epi_sub_fp<MDT, Cfg>(hp, g, a, row);
                         } else if constexpr (MODE == MODE_FAMILY) {
                             epi_sub_family<MDT, Cfg>(P.fs, g, a, row);
+                        } else if constexpr (MODE == MODE_ACCUM) {
+                            epi_sub_accum<MDT, Cfg>(P.fs.a1, g, a, row);
                         } else {
                             epi_sub_store_g<Cfg>(g, a, row);
                         }

@@ -105,3 +105,34 @@ def test_family_argument_validation():
     assert fb.forge_wgrad_step_grouped([dict(X=X, dY=dY, W=W, m=m, v=None)], "momentum", 1, 1e-2, momentum=1.5, check=False) == 4
     torch.cuda.synchronize()
     assert torch.equal(W, W0)
+
+
+@pytest.mark.parametrize("T,out,inn,bf16", [(200, 136, 264, False), (512, 384, 768, True), (2048, 256, 512, False)])
+def test_accumulate_into_state_matches_oracle(T, out, inn, bf16):
+    """B <- mu*B + dY^T X with no weight and no gradient buffer.
+    |dB| <= e (the fp32 accumulation bound of north_star) + the storage rounding."""
+    mu = 0.95
+    p = synth.make_problem("a", T, out, inn, 17, sigma_dy=1e-2)
+    B0 = p.m * 100
+    sdt = torch.bfloat16 if bf16 else torch.float32
+    Bg = B0.to(sdt).to(DEV)
+    Bo = synth.bf16_bits(B0.to(sdt)).copy() if bf16 else B0.numpy().copy()
+    X, dY = p.X.to(DEV), p.dY.to(DEV)
+    X0, dY0 = X.clone(), dY.clone()
+    n0 = fb.forge_launch_count()
+    fb.forge_wgrad_accumulate_grouped([dict(X=X, dY=dY, W=None, m=Bg, v=None)], mu, state_dtype=fb.BF16 if bf16 else fb.FP32)
+    torch.cuda.synchronize()
+    assert fb.forge_launch_count() - n0 == 1 and torch.equal(X, X0) and torch.equal(dY, dY0)
+    G, E = fo.wgrad(synth.bf16_bits(p.dY), synth.bf16_bits(p.X), with_abs=True)
+    fo.accumulate(Bo, G, mu)
+    e = T * 2.0 ** -23 * E
+    got = fo.bf16_to_f64(synth.bf16_bits(Bg)) if bf16 else Bg.cpu().numpy().astype(np.float64)
+    ref = fo.bf16_to_f64(Bo) if bf16 else Bo.astype(np.float64)
+    tol = e + (2.0 ** -7 if bf16 else 2.0 ** -22) * np.abs(ref)
+    assert np.all(np.abs(got - ref) <= tol), np.abs(got - ref).max()
+    # the worst-case bound must not hide a systematic error: bf16 results are almost all bit-identical, fp32 ones
+    # agree to the typical (not worst-case) fp32 accumulation error
+    same = (synth.bf16_bits(Bg) == Bo).mean() if bf16 else np.isclose(got, ref, rtol=2e-5, atol=1e-9).mean()
+    assert same > 0.97
+    # W / v must be absent: the call refuses and touches nothing
+    assert fb.forge_wgrad_accumulate_grouped([dict(X=X, dY=dY, W=p.W.to(DEV), m=Bg, v=None)], mu, check=False) == 5

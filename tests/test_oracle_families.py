@@ -124,3 +124,29 @@ def test_families_reduce_to_each_other_and_bf16_state():
     fo.family_step("rmsprop", W32, s32, None, G, 2, lr, beta2=np.float32(0.99).item())
     fo.family_step("rmsprop", W16, s16, None, G, 2, lr, beta2=np.float32(0.99).item())
     assert np.array_equal(W32, W16) and np.array_equal(s16, fo.f64_to_bf16(s32.astype(np.float64)))
+
+
+def test_accumulate_into_state_is_addmm_with_beta():
+    """B <- mu B + dY^T X "through the GEMM's own beta" == torch.addmm(B, dY^T, X, beta=mu)."""
+    rng = np.random.default_rng(21)
+    T = 40
+    dY = fo.f64_to_bf16(rng.normal(0, 1e-2, (T, OUT)))
+    X = fo.f64_to_bf16(rng.normal(0, 1.0, (T, IN)))
+    B0 = rng.normal(0, 1e-3, (OUT, IN)).astype(np.float32)
+    mu = np.float32(0.95).item()
+    B = B0.copy()
+    fo.accumulate(B, fo.wgrad(dY, X), mu)
+    ref = torch.addmm(torch.from_numpy(B0.astype(np.float64)), torch.from_numpy(fo.bf16_to_f64(dY)).t(),
+                      torch.from_numpy(fo.bf16_to_f64(X)), beta=mu).numpy()
+    assert np.allclose(B, ref, rtol=1e-7, atol=1e-12)
+    # mu = 0 stores the gradient itself; G = 0 only decays; bf16 storage is one RNE rounding of the same value
+    Bz = B0.copy()
+    fo.accumulate(Bz, fo.wgrad(dY, X), 0.0)
+    assert np.array_equal(Bz, fo.wgrad(dY, X).astype(np.float32))
+    Bd = B0.copy()
+    fo.accumulate(Bd, np.zeros((OUT, IN)), mu)
+    assert np.array_equal(Bd, (mu * B0.astype(np.float64)).astype(np.float32))
+    Bb = fo.f64_to_bf16(B0.astype(np.float64))
+    exp = fo.f64_to_bf16(mu * fo.bf16_to_f64(Bb) + fo.wgrad(dY, X))
+    fo.accumulate(Bb, fo.wgrad(dY, X), mu)
+    assert np.array_equal(Bb, exp)
