@@ -128,6 +128,18 @@ typedef struct {
 forge_status_t forge_wgrad_step_grouped(const forge_problem_t *problems, int32_t count, const forge_opt_desc_t *opt,
                                         forge_moment_dtype_t state_dtype, forge_stream_t stream);
 
+/* One layer's backward for the linear weights in ONE call (Alg. 1 line 1 + lines 2-11): first the
+ * input gradients dX[i][T,in] = dY_i . W_i (bf16, fp32 accumulate; a plain library GEMM -- cuBLAS, as in the paper)
+ * from the PRE-update weights, then, stream-ordered behind every one of them, the fused weight-gradient + AdamW
+ * step that overwrites W in place.  This closes the ordering hazard forge_wgrad_adamw leaves to the caller
+ * (296 Remark 2).  dX is a HOST array of `count` device pointers, one output per problem (the
+ * caller sums the dX of projections that share an input).  cuBLAS keeps its own small workspace; no
+ * gradient-shaped buffer is allocated.  Validation and errors as forge_wgrad_adamw_grouped; nothing is enqueued
+ * on a non-OK return. */
+forge_status_t forge_layer_backward_grouped(const forge_problem_t *problems, void *const *dX, int32_t count,
+                                            int64_t step, float lr, float beta1, float beta2, float eps, float wd,
+                                            forge_moment_dtype_t moment_dtype, forge_stream_t stream);
+
 /* Accumulate-into-state (the paper's regime 2; Muon's A-step): for every problem
  * B <- mu * B + dY^T X in place, "through the GEMM's own beta": no gradient is materialised and no weight is read
  * or written.  B[out,in] (fp32 or bf16) is passed in forge_problem_t.m; W, v and the scales MUST be NULL

@@ -205,3 +205,12 @@ def accumulate(B, G, mu):
     _chk(B, np.uint16 if bf16 else np.float32, "B")
     assert B.shape == G.shape
     lib().forge_oracle_accumulate(_p(B), int(bf16), _p(G), B.size, mu)
+
+
+# ------------------------------------------------------------------ input gradient ----------
+def dgrad(dY: np.ndarray, W: np.ndarray) -> np.ndarray:
+    """dX = dY . W from the PRE-update W (Algorithm 1 line 1), the plain definition:
+    dX[t,q] = sum_p dY[t,p] W[p,q] in fp64 (numpy matmul as the library primitive).  dY [T,out], W [out,in]
+    uint16 bf16 bits; returns float64 [T,in] (round with f64_to_bf16 for the stored bf16 dX)."""
+    _chk(dY, np.uint16, "dY"); _chk(W, np.uint16, "W")
+    return bf16_to_f64(dY) @ bf16_to_f64(W)

@@ -21,7 +21,7 @@ QBLOCK = 256
 STATUS_NAMES = ["FORGE_OK", "FORGE_ERR_NULL_PTR", "FORGE_ERR_BAD_SHAPE", "FORGE_ERR_ALIGNMENT",
                 "FORGE_ERR_BAD_HYPERPARAM", "FORGE_ERR_BAD_DTYPE", "FORGE_ERR_UNSUPPORTED_ARCH",
                 "FORGE_ERR_CUDA"]
-EXPORTS = ["forge_wgrad_adamw", "forge_wgrad_adamw_grouped", "forge_wgrad_step_grouped", "forge_wgrad_accumulate_grouped", "forge_wgrad_adamw_host",
+EXPORTS = ["forge_wgrad_adamw", "forge_wgrad_adamw_grouped", "forge_wgrad_step_grouped", "forge_wgrad_accumulate_grouped", "forge_layer_backward_grouped", "forge_wgrad_adamw_host",
            "forge_wgrad_store_g", "forge_adamw_from_g", "forge_workspace_bytes", "forge_launch_count",
            "forge_last_cuda_error", "forge_status_string", "forge_version"]
 
@@ -70,6 +70,9 @@ def lib() -> ctypes.CDLL:
                                                ctypes.c_int, c_void_p]
         L.forge_wgrad_accumulate_grouped.restype = ctypes.c_int
         L.forge_wgrad_accumulate_grouped.argtypes = [ctypes.POINTER(forge_problem_t), c_int32, c_float, ctypes.c_int, c_void_p]
+        L.forge_layer_backward_grouped.restype = ctypes.c_int
+        L.forge_layer_backward_grouped.argtypes = [ctypes.POINTER(forge_problem_t), ctypes.POINTER(c_void_p), c_int32] + hp + \
+                                                  [ctypes.c_int, c_void_p]
         L.forge_wgrad_adamw_host.restype = ctypes.c_int
         L.forge_wgrad_adamw_host.argtypes = [c_void_p] * 7 + [c_int32] * 3 + hp + [ctypes.c_int]
         L.forge_wgrad_store_g.restype = ctypes.c_int
@@ -156,6 +159,17 @@ def forge_wgrad_step_grouped(problems, family: str, step, lr, beta1=0.9, beta2=0
     st = lib().forge_wgrad_step_grouped(arr, len(arr), ctypes.byref(desc), state_dtype, _stream(stream))
     if check:
         _check(st, "forge_wgrad_step_grouped")
+    return st
+
+
+def forge_layer_backward_grouped(problems, dX, step, lr, beta1, beta2, eps, wd, moment_dtype, stream=None, check=True) -> int:
+    """include/forge.h forge_layer_backward_grouped: dX[i] = dY_i W_i from the pre-update W, then the fused step."""
+    arr = make_problem_array(problems)
+    ptrs = (c_void_p * len(dX))(*[t.data_ptr() for t in dX])
+    st = lib().forge_layer_backward_grouped(arr, ptrs, len(arr), int(step), lr, beta1, beta2, eps, wd, moment_dtype,
+                                            _stream(stream))
+    if check:
+        _check(st, "forge_layer_backward_grouped")
     return st
 
 

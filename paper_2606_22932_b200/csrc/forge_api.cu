@@ -8,6 +8,7 @@
 #include <cstring>
 #include <mutex>
 
+#include <cublas_v2.h>
 #include <cuda.h>
 #include <cuda_runtime.h>
 
@@ -512,6 +513,42 @@ forge_status_t forge_wgrad_accumulate_grouped(const forge_problem_t *problems, i
         if (s != FORGE_OK) return s;
     }
     return FORGE_OK;
+}
+
+forge_status_t forge_layer_backward_grouped(const forge_problem_t *problems, void *const *dX, int32_t count,
+                                            int64_t step, float lr, float beta1, float beta2, float eps, float wd,
+                                            forge_moment_dtype_t moment_dtype, forge_stream_t stream) {
+    if (!problems || !dX) return FORGE_ERR_NULL_PTR;
+    if (count < 1) return FORGE_ERR_BAD_SHAPE;
+    const int mdt = static_cast<int>(moment_dtype);
+    if (mdt < 0 || mdt > 2) return FORGE_ERR_BAD_DTYPE;
+    forge_status_t s = validate_hp(step, lr, beta1, beta2, eps, wd);
+    if (s != FORGE_OK) return s;
+    for (int i = 0; i < count; ++i) {          // everything is validated before anything is enqueued
+        s = validate_problem(problems[i], mdt);
+        if (s != FORGE_OK) return s;
+        if (!dX[i]) return FORGE_ERR_NULL_PTR;
+        if (!aligned16(dX[i])) return FORGE_ERR_ALIGNMENT;
+    }
+    DeviceInfo dev;
+    s = device_info(dev);
+    if (s != FORGE_OK) return s;
+    static thread_local cublasHandle_t handle = nullptr;
+    if (!handle && cublasCreate(&handle) != CUBLAS_STATUS_SUCCESS) return cuda_fail(cudaErrorInitializationError);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    if (cublasSetStream(handle, st) != CUBLAS_STATUS_SUCCESS) return cuda_fail(cudaErrorUnknown);
+    // 1. dX = dY . W from the PRE-update W (Alg. 1 line 1; 296 Remark 2).  Row-major
+    //    dX[T,in] = dY[T,out] W[out,in] is the column-major product dX^T[in,T] = W^T[in,out] dY^T[out,T].
+    const float one = 1.0f, zero = 0.0f;
+    for (int i = 0; i < count; ++i) {
+        const forge_problem_t &p = problems[i];
+        cublasStatus_t cs = cublasGemmEx(handle, CUBLAS_OP_N, CUBLAS_OP_N, p.in, p.T, p.out, &one, p.W, CUDA_R_16BF, p.in,
+                                         p.dY, CUDA_R_16BF, p.out, &zero, dX[i], CUDA_R_16BF, p.in, CUBLAS_COMPUTE_32F,
+                                         CUBLAS_GEMM_DEFAULT);
+        if (cs != CUBLAS_STATUS_SUCCESS) return cuda_fail(cudaErrorUnknown);
+    }
+    // 2. the fused weight-gradient + AdamW step, stream-ordered after every dgrad GEMM that reads W
+    return forge_wgrad_adamw_grouped(problems, count, step, lr, beta1, beta2, eps, wd, moment_dtype, stream);
 }
 
 forge_status_t forge_wgrad_store_g(const void *X, const void *dY, float *G, int32_t T, int32_t out, int32_t in,

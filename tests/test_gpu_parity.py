@@ -303,3 +303,33 @@ def test_config4_full_stack_reverse_order_sampled_rows():
             e = tol.step(G, E, T, hp)
             pu.check_fp(synth.bf16_bits(d["W"][r0:r1]), d["m"][r0:r1].cpu().numpy(), d["v"][r0:r1].cpu().numpy(),
                                  Wb, m0, v0, G, e, tol, hp, label=f"{d['name']}[{r0}:{r1}]", W_prev=Wp)
+
+
+def test_layer_backward_dgrad_reads_pre_update_weights_then_fused_step():
+    """SURVEY.md 8(f) rank 2 (Alg. 1 line 1; 64; 296): forge_layer_backward_grouped computes
+    dX = dY . W from the PRE-update W, then the fused step; W/m/v must equal the plain grouped call bit for bit."""
+    ps = [synth.make_problem("a", 200, 136, 264, 31), synth.make_problem("b", 96, 256, 512, 32)]
+    probs, twins, dXs = [], [], []
+    for p in ps:
+        probs.append(dict(X=p.X.to(DEV), dY=p.dY.to(DEV), W=p.W.to(DEV).clone(), m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone()))
+        twins.append(dict(X=p.X.to(DEV), dY=p.dY.to(DEV), W=p.W.to(DEV).clone(), m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone()))
+        dXs.append(torch.full((p.T, p.inn), float("nan"), dtype=torch.bfloat16, device=DEV))
+    fb.forge_layer_backward_grouped(probs, dXs, *hp_args(10), fb.FP32)
+    fb.forge_wgrad_adamw_grouped(twins, *hp_args(10), fb.FP32)
+    torch.cuda.synchronize()
+    for p, d, t, dX in zip(ps, probs, twins, dXs):
+        assert torch.equal(d["W"], t["W"]) and torch.equal(d["m"], t["m"]) and torch.equal(d["v"], t["v"])
+        assert not torch.equal(d["W"].cpu(), p.W)                                    # the step did happen
+        ref = fo.dgrad(synth.bf16_bits(p.dY), synth.bf16_bits(p.W))                  # oracle, PRE-update W
+        got = fo.bf16_to_f64(synth.bf16_bits(dX))
+        bound = p.out * 2.0 ** -23 * (np.abs(fo.bf16_to_f64(synth.bf16_bits(p.dY))) @ np.abs(fo.bf16_to_f64(synth.bf16_bits(p.W))))
+        assert np.all(np.abs(got - ref) <= pu.bf16_ulp(ref) + bound), np.abs(got - ref).max()
+        assert float((synth.bf16_bits(dX) == fo.f64_to_bf16(ref)).mean()) > 0.98
+        post = fo.dgrad(synth.bf16_bits(p.dY), synth.bf16_bits(d["W"]))              # what a mis-ordered call would give
+        assert float((synth.bf16_bits(dX) == fo.f64_to_bf16(post)).mean()) < 0.9
+    # a bad argument in the second problem: nothing is enqueued, nothing changes
+    W0 = probs[0]["W"].clone()
+    bad = [probs[0], dict(probs[1], m=None)]
+    assert fb.forge_layer_backward_grouped(bad, dXs, *hp_args(11), fb.FP32, check=False) == 1
+    torch.cuda.synchronize()
+    assert torch.equal(probs[0]["W"], W0)

@@ -184,3 +184,23 @@ def test_bf16_moment_mode_is_same_update_with_rounded_state():
     assert np.array_equal(Wd32, Wd16) and np.array_equal(md32, md16) and np.array_equal(vd32, vd16)
     assert np.array_equal(W1, W2)
     assert np.array_equal(m2, fo.f64_to_bf16(md16)) and np.array_equal(v2, fo.f64_to_bf16(vd16))
+
+
+def test_dgrad_exact_rational_bruteforce_and_adjoint_identity():
+    """oracle dgrad (PAPER.md:74 line 1) against exact rational arithmetic on a tiny case, and against the
+    adjoint identity <dX, X> = <G, W> that ties it to the pinned wgrad: sum_tq dX[t,q] X[t,q] = sum_pq G[p,q] W[p,q]."""
+    from fractions import Fraction
+    rng = np.random.default_rng(3)
+    T, out, inn = 3, 4, 5
+    dY = fo.f64_to_bf16(rng.normal(0, 1, (T, out)))
+    W = fo.f64_to_bf16(rng.normal(0, 1, (out, inn)))
+    X = fo.f64_to_bf16(rng.normal(0, 1, (T, inn)))
+    dX = fo.dgrad(dY, W)
+    dYf, Wf = fo.bf16_to_f64(dY), fo.bf16_to_f64(W)
+    for t in range(T):
+        for q in range(inn):
+            exact = sum(Fraction(float(dYf[t, p])) * Fraction(float(Wf[p, q])) for p in range(out))
+            assert abs(Fraction(float(dX[t, q])) - exact) <= abs(exact) * Fraction(1, 2 ** 50) + Fraction(1, 2 ** 200)
+    G = fo.wgrad(dY, X)
+    lhs, rhs = float((dX * fo.bf16_to_f64(X)).sum()), float((G * Wf).sum())
+    assert abs(lhs - rhs) <= 1e-12 * (abs(lhs) + abs(rhs) + 1)
