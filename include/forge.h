@@ -128,6 +128,15 @@ typedef struct {
 forge_status_t forge_wgrad_step_grouped(const forge_problem_t *problems, int32_t count, const forge_opt_desc_t *opt,
                                         forge_moment_dtype_t state_dtype, forge_stream_t stream);
 
+/* AdamW with the paper's "SR-store" recipe (1287-1296): identical to forge_wgrad_adamw_grouped except
+ * that W' is committed to bf16 by STOCHASTIC rounding instead of RNE (m, v unchanged; FP32 or BF16 moments).
+ * 16 random bits per weight element come from a counter-based generator keyed (seed, step, index of the problem
+ * in this call, row, col) -- the same call with the same seed is bitwise reproducible; out = (bits(fp32 W') + r16)
+ * >> 16, i.e. the fp32 value is rounded away from zero with probability (its low 16 bits) / 65536 (unbiased). */
+forge_status_t forge_wgrad_adamw_sr_grouped(const forge_problem_t *problems, int32_t count, int64_t step, float lr,
+                                           float beta1, float beta2, float eps, float wd,
+                                           forge_moment_dtype_t moment_dtype, uint64_t seed, forge_stream_t stream);
+
 /* One layer's backward for the linear weights in ONE call (Alg. 1 line 1 + lines 2-11): first the
  * input gradients dX[i][T,in] = dY_i . W_i (bf16, fp32 accumulate; a plain library GEMM -- cuBLAS, as in the paper)
  * from the PRE-update weights, then, stream-ordered behind every one of them, the fused weight-gradient + AdamW

@@ -58,6 +58,13 @@ def lib() -> ctypes.CDLL:
         L.forge_oracle_bf16_from_double_array.restype = None
         L.forge_oracle_bf16_from_double_array.argtypes = [c_void_p, c_void_p, c_size_t]
         L.forge_oracle_num_threads.restype = c_int
+        L.forge_oracle_sr_bits.restype = ctypes.c_uint32
+        L.forge_oracle_sr_bits.argtypes = [ctypes.c_uint64, c_long, ctypes.c_uint32, ctypes.c_uint32, ctypes.c_uint32]
+        L.forge_oracle_bf16_sr_from_double.restype = ctypes.c_uint16
+        L.forge_oracle_bf16_sr_from_double.argtypes = [c_double, ctypes.c_uint32]
+        L.forge_oracle_adamw_fp32_sr.restype = None
+        L.forge_oracle_adamw_fp32_sr.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_int, c_long,
+                                                 c_float, c_float, c_float, c_float, c_float, ctypes.c_uint64, ctypes.c_uint32]
         L.forge_oracle_accumulate.restype = None
         L.forge_oracle_accumulate.argtypes = [c_void_p, c_int, c_void_p, c_size_t, c_float]
         L.forge_oracle_family_step.restype = None
@@ -214,3 +221,21 @@ def dgrad(dY: np.ndarray, W: np.ndarray) -> np.ndarray:
     uint16 bf16 bits; returns float64 [T,in] (round with f64_to_bf16 for the stored bf16 dX)."""
     _chk(dY, np.uint16, "dY"); _chk(W, np.uint16, "W")
     return bf16_to_f64(dY) @ bf16_to_f64(W)
+
+
+# ------------------------------------------------------------------ stochastic-rounding store
+def sr_bits(seed, step, stream, row, col) -> int:
+    """The 16 random bits of weight element (row, col) (forge_oracle_families.c, reading S16)."""
+    return int(lib().forge_oracle_sr_bits(int(seed), int(step), int(stream), int(row), int(col)))
+
+
+def bf16_sr(x: float, r16: int) -> int:
+    return int(lib().forge_oracle_bf16_sr_from_double(float(x), int(r16)))
+
+
+def adamw_fp32_sr(W, m, v, G, step, lr, beta1, beta2, eps, wd, seed, stream=0):
+    """AdamW with fp32 moments and the stochastic-rounding store of W, in place."""
+    _chk(W, np.uint16, "W"); _chk(m, np.float32, "m"); _chk(v, np.float32, "v"); _chk(G, np.float64, "G")
+    assert W.ndim == 2 and W.shape == m.shape == v.shape == G.shape
+    lib().forge_oracle_adamw_fp32_sr(_p(W), _p(m), _p(v), _p(G), W.shape[0], W.shape[1], int(step), lr, beta1, beta2,
+                                     eps, wd, int(seed), int(stream))

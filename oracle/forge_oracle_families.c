@@ -153,3 +153,49 @@ void forge_oracle_accumulate(void *B, int state_bf16, const double *G, size_t n,
 #pragma omp parallel for schedule(static)
     for (size_t i = 0; i < n; ++i) st(B, i, state_bf16, m * ld(B, i, state_bf16) + G[i]);
 }
+
+/* ---------------------------------------------------------------- stochastic-rounding store --
+ * The paper's "SR-store" recipe (1287-1296: "the bf16 weight is the only copy, committed by
+ * stochastic rounding"; microcheck PAPER.md:1450 "dead zone, unbiasedness").  The paper gives no generator,
+ * so both sides implement the same counter-based one (reading S16): 16 random bits per weight
+ * element from (seed, step, stream, row, col) through the murmur3 finaliser; the decision is taken in the
+ * kernel's precision: x = fp32(W'), out = (bits(x) + r16) >> 16, i.e. round away from zero with probability
+ * (low 16 bits) / 65536 -- unbiased on the fp32 value.  Inf / NaN take the RNE path. */
+static uint32_t fmix32(uint32_t h)
+{
+    h ^= h >> 16; h *= 0x85EBCA6Bu; h ^= h >> 13; h *= 0xC2B2AE35u; h ^= h >> 16;
+    return h;
+}
+uint32_t forge_oracle_sr_bits(uint64_t seed, long step, uint32_t stream, uint32_t row, uint32_t col)
+{
+    uint32_t inner = fmix32((uint32_t)(seed >> 32) ^ ((uint32_t)step * 0x85EBCA77u) ^ (stream * 0xC2B2AE3Du));
+    uint32_t rowkey = fmix32((row * 0x9E3779B1u) ^ (uint32_t)seed ^ inner);
+    return fmix32(rowkey ^ (col * 0x27D4EB2Fu)) >> 16;
+}
+uint16_t forge_oracle_bf16_sr_from_double(double x, uint32_t r16)
+{
+    float f = (float)x;                                   /* the kernel's arithmetic type */
+    uint32_t b;
+    __builtin_memcpy(&b, &f, 4);
+    if ((b & 0x7F800000u) == 0x7F800000u) return forge_oracle_bf16_from_double(x);
+    return (uint16_t)((b + r16) >> 16);
+}
+
+/* AdamW (Algorithm 1) with fp32 moments and the SR store of W; W is [out, in]. */
+void forge_oracle_adamw_fp32_sr(uint16_t *W, float *m, float *v, const double *G, int out, int in, long step,
+                                float lr, float beta1, float beta2, float eps, float wd, uint64_t seed, uint32_t stream)
+{
+    const double b1 = beta1, b2 = beta2, bc1 = 1.0 - pow(b1, (double)step), bc2 = 1.0 - pow(b2, (double)step);
+#pragma omp parallel for schedule(static)
+    for (int p = 0; p < out; ++p)
+        for (int q = 0; q < in; ++q) {
+            size_t i = (size_t)p * in + q;
+            double w = forge_oracle_bf16_to_double(W[i]);
+            double m1 = b1 * (double)m[i] + (1.0 - b1) * G[i];
+            double v1 = b2 * (double)v[i] + (1.0 - b2) * G[i] * G[i];
+            double w1 = (1.0 - (double)lr * (double)wd) * w - (double)lr * (m1 / bc1) / (sqrt(v1 / bc2) + (double)eps);
+            W[i] = forge_oracle_bf16_sr_from_double(w1, forge_oracle_sr_bits(seed, step, stream, (uint32_t)p, (uint32_t)q));
+            m[i] = (float)m1;
+            v[i] = (float)v1;
+        }
+}

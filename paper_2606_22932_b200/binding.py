@@ -21,7 +21,7 @@ QBLOCK = 256
 STATUS_NAMES = ["FORGE_OK", "FORGE_ERR_NULL_PTR", "FORGE_ERR_BAD_SHAPE", "FORGE_ERR_ALIGNMENT",
                 "FORGE_ERR_BAD_HYPERPARAM", "FORGE_ERR_BAD_DTYPE", "FORGE_ERR_UNSUPPORTED_ARCH",
                 "FORGE_ERR_CUDA"]
-EXPORTS = ["forge_wgrad_adamw", "forge_wgrad_adamw_grouped", "forge_wgrad_step_grouped", "forge_wgrad_accumulate_grouped", "forge_layer_backward_grouped", "forge_wgrad_adamw_host",
+EXPORTS = ["forge_wgrad_adamw", "forge_wgrad_adamw_grouped", "forge_wgrad_step_grouped", "forge_wgrad_accumulate_grouped", "forge_layer_backward_grouped", "forge_wgrad_adamw_sr_grouped", "forge_wgrad_adamw_host",
            "forge_wgrad_store_g", "forge_adamw_from_g", "forge_workspace_bytes", "forge_launch_count",
            "forge_last_cuda_error", "forge_status_string", "forge_version"]
 
@@ -70,6 +70,9 @@ def lib() -> ctypes.CDLL:
                                                ctypes.c_int, c_void_p]
         L.forge_wgrad_accumulate_grouped.restype = ctypes.c_int
         L.forge_wgrad_accumulate_grouped.argtypes = [ctypes.POINTER(forge_problem_t), c_int32, c_float, ctypes.c_int, c_void_p]
+        L.forge_wgrad_adamw_sr_grouped.restype = ctypes.c_int
+        L.forge_wgrad_adamw_sr_grouped.argtypes = [ctypes.POINTER(forge_problem_t), c_int32] + hp + \
+                                                  [ctypes.c_int, ctypes.c_uint64, c_void_p]
         L.forge_layer_backward_grouped.restype = ctypes.c_int
         L.forge_layer_backward_grouped.argtypes = [ctypes.POINTER(forge_problem_t), ctypes.POINTER(c_void_p), c_int32] + hp + \
                                                   [ctypes.c_int, c_void_p]
@@ -159,6 +162,16 @@ def forge_wgrad_step_grouped(problems, family: str, step, lr, beta1=0.9, beta2=0
     st = lib().forge_wgrad_step_grouped(arr, len(arr), ctypes.byref(desc), state_dtype, _stream(stream))
     if check:
         _check(st, "forge_wgrad_step_grouped")
+    return st
+
+
+def forge_wgrad_adamw_sr_grouped(problems, step, lr, beta1, beta2, eps, wd, moment_dtype, seed, stream=None, check=True) -> int:
+    """include/forge.h forge_wgrad_adamw_sr_grouped: AdamW with the stochastic-rounding store of W."""
+    arr = make_problem_array(problems)
+    st = lib().forge_wgrad_adamw_sr_grouped(arr, len(arr), int(step), lr, beta1, beta2, eps, wd, moment_dtype, int(seed),
+                                            _stream(stream))
+    if check:
+        _check(st, "forge_wgrad_adamw_sr_grouped")
     return st
 
 

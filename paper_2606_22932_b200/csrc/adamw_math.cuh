@@ -115,6 +115,32 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
 }
 __device__ __forceinline__ uint32_t f32x2_to_bf16x2(f32x2 p) { return pack_bf16(lo2(p), hi2(p)); }
 
+// ------------------------------------------------------------------ stochastic-rounding store
+// The paper's "SR-store" recipe: the bf16 weight is committed by stochastic rounding.
+// 16 random bits per element from a counter-based generator keyed (seed, step, stream, row, col) through the
+// murmur3 finaliser (reading S16); out = (bits(x) + r16) >> 16 rounds the fp32 value away from zero with
+// probability (low 16 bits) / 65536.  Inf / NaN take the RNE path.
+__device__ __forceinline__ uint32_t fmix32(uint32_t h) {
+    h ^= h >> 16; h *= 0x85EBCA6Bu; h ^= h >> 13; h *= 0xC2B2AE35u; h ^= h >> 16;
+    return h;
+}
+__host__ __device__ inline uint32_t sr_inner_key_host(uint32_t seed_hi, uint32_t step, uint32_t stream) {
+    uint32_t h = seed_hi ^ (step * 0x85EBCA77u) ^ (stream * 0xC2B2AE3Du);
+    h ^= h >> 16; h *= 0x85EBCA6Bu; h ^= h >> 13; h *= 0xC2B2AE35u; h ^= h >> 16;
+    return h;
+}
+__device__ __forceinline__ uint32_t sr_row_key(uint32_t row, uint32_t seed_lo, uint32_t inner) {
+    return fmix32((row * 0x9E3779B1u) ^ seed_lo ^ inner);
+}
+__device__ __forceinline__ uint32_t sr_bf16(float x, uint32_t rowkey, uint32_t col) {
+    const uint32_t b = __float_as_uint(x);
+    if ((b & 0x7F800000u) == 0x7F800000u) return pack_bf16(x, 0.0f) & 0xFFFFu;
+    return (b + (fmix32(rowkey ^ (col * 0x27D4EB2Fu)) >> 16)) >> 16;
+}
+__device__ __forceinline__ uint32_t f32x2_to_bf16x2_sr(f32x2 p, uint32_t rowkey, uint32_t col) {
+    return sr_bf16(lo2(p), rowkey, col) | (sr_bf16(hi2(p), rowkey, col + 1u) << 16);
+}
+
 // ------------------------------------------------------------------ int8 blockwise ---------
 // PAPER.md:316 with BASELINE.json's 256-blocks: scale a = block absmax (fp32);
 // m code = rint(x * (127/a)) in [-127,127]; v code = max(1, rint(x * (255/a))) in [1,255];

@@ -151,7 +151,8 @@ int env_int(const char *name, int dflt) {
 template <int MDT, int MODE, int BK, int ST, int SS, int CG = 1, int CM = 64, int CN = 64, int P1C = 128, int P1S = 2,
           int NST = 2>
 forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamWScalars &hp,
-                            const DeviceInfo &dev, cudaStream_t stream, const FamilyScalars *fs = nullptr) {
+                            const DeviceInfo &dev, cudaStream_t stream, const FamilyScalars *fs = nullptr,
+                            uint64_t sr_seed = 0, uint32_t sr_step = 0, uint32_t sr_stream0 = 0) {
     using Cfg = KernelCfg<MDT, BK, ST, SS, CG, CM, CN, P1C, P1S, NST, (MODE == MODE_ACCUM) ? 0 : 1>;
     auto kernel = forge_fused_kernel<MDT, MODE, BK, ST, SS, CG, CM, CN, P1C, P1S, NST>;
     static std::once_flag once;
@@ -202,9 +203,11 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
         d.in = p.in;
         d.tiles_n = (p.in + BLOCK_N - 1) / BLOCK_N;
         d.tile_begin = tiles;
+        d.sr_inner = sr_inner_key_host(static_cast<uint32_t>(sr_seed >> 32), sr_step, sr_stream0 + static_cast<uint32_t>(i));
         tiles += ((p.out + BLOCK_M * CG - 1) / (BLOCK_M * CG)) * d.tiles_n;   // (128*CG) x 256 work units
     }
     P.total_tiles = tiles;
+    P.sr_seed_lo = static_cast<uint32_t>(sr_seed);
     P.debug = env_int("FORGE_ABLATE", 0);          // profiling ablations only (profiles/): results are wrong when set
     int grid = dev.sm_count / CG;                  // persistent: one CTA (or CTA pair) per SM (pair)
     const int forced = env_int("FORGE_GRID", 0);   // debug/determinism tests only
@@ -510,6 +513,42 @@ forge_status_t forge_wgrad_accumulate_grouped(const forge_problem_t *problems, i
         else
             s = maxT > 1024 ? launch_fused<MDT_BF16, MODE_ACCUM, 64, 4, 2, 2, 64, 128, 128, 2, 1>(pp, n, hp, dev, st, &fs)
                             : launch_fused<MDT_BF16, MODE_ACCUM, 32, 4, 4, 2, 32, 128, 128, 2, 1>(pp, n, hp, dev, st, &fs);
+        if (s != FORGE_OK) return s;
+    }
+    return FORGE_OK;
+}
+
+forge_status_t forge_wgrad_adamw_sr_grouped(const forge_problem_t *problems, int32_t count, int64_t step, float lr,
+                                           float beta1, float beta2, float eps, float wd,
+                                           forge_moment_dtype_t moment_dtype, uint64_t seed, forge_stream_t stream) {
+    if (!problems) return FORGE_ERR_NULL_PTR;
+    if (count < 1) return FORGE_ERR_BAD_SHAPE;
+    const int mdt = static_cast<int>(moment_dtype);
+    if (mdt != FORGE_MOMENT_FP32 && mdt != FORGE_MOMENT_BF16) return FORGE_ERR_BAD_DTYPE;
+    forge_status_t s = validate_hp(step, lr, beta1, beta2, eps, wd);
+    if (s != FORGE_OK) return s;
+    int maxT = 0;
+    for (int i = 0; i < count; ++i) {
+        s = validate_problem(problems[i], mdt);
+        if (s != FORGE_OK) return s;
+        maxT = problems[i].T > maxT ? problems[i].T : maxT;
+    }
+    DeviceInfo dev;
+    s = device_info(dev);
+    if (s != FORGE_OK) return s;
+    const AdamWScalars hp = make_scalars(step, lr, beta1, beta2, eps, wd);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const uint32_t st32 = static_cast<uint32_t>(step);
+    for (int i = 0; i < count; i += kMaxProblems) {    // the random stream of a problem is its index in the call
+        const int n = (count - i) < kMaxProblems ? (count - i) : kMaxProblems;
+        const forge_problem_t *pp = problems + i;
+        const uint32_t s0 = static_cast<uint32_t>(i);
+        if (mdt == FORGE_MOMENT_FP32)
+            s = maxT > 1024 ? launch_fused<MDT_FP32, MODE_ADAMW_SR, 64, 4, 2, 2, 64, 64>(pp, n, hp, dev, st, nullptr, seed, st32, s0)
+                            : launch_fused<MDT_FP32, MODE_ADAMW_SR, 32, 4, 2, 2, 64, 128>(pp, n, hp, dev, st, nullptr, seed, st32, s0);
+        else
+            s = maxT > 1024 ? launch_fused<MDT_BF16, MODE_ADAMW_SR, 64, 4, 2, 2, 64, 64>(pp, n, hp, dev, st, nullptr, seed, st32, s0)
+                            : launch_fused<MDT_BF16, MODE_ADAMW_SR, 32, 4, 4, 2, 64, 64>(pp, n, hp, dev, st, nullptr, seed, st32, s0);
         if (s != FORGE_OK) return s;
     }
     return FORGE_OK;

@@ -49,7 +49,8 @@ constexpr int kTmemCols = 512;  // 2 accumulator buffers x 256 fp32 columns
 
 enum : int { MDT_FP32 = 0, MDT_BF16 = 1, MDT_INT8 = 2 };
 enum : int { MODE_ADAMW = 0, MODE_STORE_G = 1, MODE_FAMILY = 2,      // FAMILY: family_math.cuh, 0-2 state tensors
-             MODE_ACCUM = 3 };                                        // B <- mu*B + G, no weight
+             MODE_ACCUM = 3,                                          // B <- mu*B + G, no weight
+             MODE_ADAMW_SR = 4 };                                     // AdamW, stochastic-rounding store of W
 
 struct alignas(64) ProblemDesc {
     CUtensorMap map_dY;  // [T, out] bf16, box {64, kBlockK}, SWIZZLE_128B
@@ -64,7 +65,7 @@ struct alignas(64) ProblemDesc {
     int32_t T, out, in;
     int32_t tiles_n;     // ceil(in / 256)
     int32_t tile_begin;  // first linear tile index of this problem
-    int32_t pad_;
+    uint32_t sr_inner;   // MODE_ADAMW_SR: fmix32(seed_hi ^ step ^ stream) of this problem
 };
 
 struct alignas(64) KernelParams {
@@ -73,7 +74,7 @@ struct alignas(64) KernelParams {
     FamilyScalars fs;    // MODE_FAMILY only
     int32_t num_problems;
     int32_t total_tiles;
-    int32_t pad_;
+    uint32_t sr_seed_lo; // MODE_ADAMW_SR
     int32_t debug;       // ablation switches for profiling ONLY (results are wrong when set):
                          // 1 = no operand loads / MMA, 2 = no state loads / stores, 4 = no epilogue math
 };
@@ -184,9 +185,9 @@ struct SubAddr {
 // ---------------------------------------------------------------------------------------------
 // epilogue bodies: one thread = one W row of the chunk, one 32-column sub-block at a time
 // ---------------------------------------------------------------------------------------------
-template <int MDT, class Cfg>
+template <int MDT, class Cfg, bool SR = false>
 __device__ __forceinline__ void epi_sub_fp(const AdamWScalars &hp, const uint32_t (&g)[32],
-                                           const SubAddr<Cfg> &a, uint32_t row) {
+                                           const SubAddr<Cfg> &a, uint32_t row, uint32_t rowkey = 0, uint32_t col0 = 0) {
     // 4 groups of 8 columns: one 16 B piece of W (8 bf16) + matching moments, as 4 coordinate pairs
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
@@ -217,7 +218,13 @@ __device__ __forceinline__ void epi_sub_fp(const AdamWScalars &hp, const uint32_
             sts128(am, make_uint4(f32x2_to_bf16x2(m[0]), f32x2_to_bf16x2(m[1]), f32x2_to_bf16x2(m[2]), f32x2_to_bf16x2(m[3])));
             sts128(av, make_uint4(f32x2_to_bf16x2(v[0]), f32x2_to_bf16x2(v[1]), f32x2_to_bf16x2(v[2]), f32x2_to_bf16x2(v[3])));
         }
-        sts128(aw, make_uint4(f32x2_to_bf16x2(w[0]), f32x2_to_bf16x2(w[1]), f32x2_to_bf16x2(w[2]), f32x2_to_bf16x2(w[3])));
+        if constexpr (SR) {
+            const uint32_t c = col0 + 8 * j;
+            sts128(aw, make_uint4(f32x2_to_bf16x2_sr(w[0], rowkey, c), f32x2_to_bf16x2_sr(w[1], rowkey, c + 2),
+                                  f32x2_to_bf16x2_sr(w[2], rowkey, c + 4), f32x2_to_bf16x2_sr(w[3], rowkey, c + 6)));
+        } else {
+            sts128(aw, make_uint4(f32x2_to_bf16x2(w[0]), f32x2_to_bf16x2(w[1]), f32x2_to_bf16x2(w[2]), f32x2_to_bf16x2(w[3])));
+        }
     }
 }
 
@@ -524,6 +531,7 @@ __global__ void __launch_bounds__(block_threads(MDT), 1)
 forge_fused_kernel(const __grid_constant__ KernelParams P) {
     constexpr int HASW = (MODE == MODE_ACCUM) ? 0 : 1;
     using Cfg = KernelCfg<MDT, kBlockK, kStages, kStateStages, CG, CM, CN, P1C, P1S, NST, HASW>;
+    static_assert(MODE != MODE_ADAMW_SR || MDT != MDT_INT8, "the SR store is implemented for fp32 / bf16 moments");
     static_assert(MODE == MODE_FAMILY || MODE == MODE_ACCUM || NST == 2, "AdamW and the store-G twin use the two-state chunk image");
     static_assert(MODE != MODE_ACCUM || NST == 1, "accumulate-into-state has exactly one state tensor");
     static_assert((MODE != MODE_FAMILY && MODE != MODE_ACCUM) || MDT != MDT_INT8, "int8 state is implemented for AdamW only");
@@ -761,6 +769,12 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
             if (!(P.debug & DBG_NO_MAINLOOP)) mbar_wait(bar_tm_full + 8 * as, aph);
             tc_fence_after();
             const uint32_t taddr = tmem_base + ((quad * 32u) << 16) + as * BLOCK_N;
+            uint32_t sr_rowkey = 0, sr_col0 = 0;
+            if constexpr (MODE == MODE_ADAMW_SR) {
+                const TileCoord tc = decode_tile<CG>(P, tile, rank);
+                sr_rowkey = sr_row_key(static_cast<uint32_t>(tc.tm * BLOCK_M) + row_t, P.sr_seed_lo, P.prob[tc.p].sr_inner);
+                sr_col0 = static_cast<uint32_t>(tc.tn * BLOCK_N);
+            }
             if constexpr (MDT != MDT_INT8) {
                 for (int cb = 0; cb < Cfg::CB; ++cb) {
                     if (Cfg::SUBS < 2 && (cb & 1) != wg) continue;
@@ -776,6 +790,8 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                         tmem_ld_wait();
                         if constexpr (MODE == MODE_ADAMW) {
                             if (!(P.debug & DBG_NO_EPILOGUE)) epi_sub_fp<MDT, Cfg>(hp, g, a, row);
+                        } else if constexpr (MODE == MODE_ADAMW_SR) {
+                            epi_sub_fp<MDT, Cfg, true>(hp, g, a, row, sr_rowkey, sr_col0 + cb * CN + j32 * SUB);
                         } else if constexpr (MODE == MODE_FAMILY) {
                             epi_sub_family<MDT, Cfg>(P.fs, g, a, row);
                         } else if constexpr (MODE == MODE_ACCUM) {

@@ -136,3 +136,37 @@ def test_accumulate_into_state_matches_oracle(T, out, inn, bf16):
     assert same > 0.97
     # W / v must be absent: the call refuses and touches nothing
     assert fb.forge_wgrad_accumulate_grouped([dict(X=X, dY=dY, W=p.W.to(DEV), m=Bg, v=None)], mu, check=False) == 5
+
+
+def test_adamw_stochastic_rounding_store_matches_oracle_generator():
+    """the SR store.  Both sides implement the same counter-based
+    generator, so the result is deterministic: m, v as the RNE call; W one of the two bf16 neighbours of W', equal
+    to the oracle's choice except where the kernel's fp32 W' and fp32(oracle W') differ in their low bits."""
+    ps = [synth.make_problem("a", 200, 136, 264, 41), synth.make_problem("b", 96, 256, 512, 42)]
+    hp = synth.HP_DEFAULT
+    hpt = (hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
+    probs = [dict(X=p.X.to(DEV), dY=p.dY.to(DEV), W=p.W.to(DEV).clone(), m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone()) for p in ps]
+    twins = [dict(X=p.X.to(DEV), dY=p.dY.to(DEV), W=p.W.to(DEV).clone(), m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone()) for p in ps]
+    again = [dict(X=p.X.to(DEV), dY=p.dY.to(DEV), W=p.W.to(DEV).clone(), m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone()) for p in ps]
+    seed = (7 << 40) + 12345
+    fb.forge_wgrad_adamw_sr_grouped(probs, 10, *hpt, fb.FP32, seed)
+    fb.forge_wgrad_adamw_sr_grouped(again, 10, *hpt, fb.FP32, seed)
+    fb.forge_wgrad_adamw_grouped(twins, 10, *hpt, fb.FP32)
+    torch.cuda.synchronize()
+    for i, (p, d, t, a) in enumerate(zip(ps, probs, twins, again)):
+        assert torch.equal(d["m"], t["m"]) and torch.equal(d["v"], t["v"])           # only the store of W differs
+        assert torch.equal(d["W"], a["W"])                                           # reproducible for a fixed seed
+        Wo, mo, vo = synth.bf16_bits(p.W).copy(), p.m.numpy().copy(), p.v.numpy().copy()
+        G = fo.wgrad(synth.bf16_bits(p.dY), synth.bf16_bits(p.X))
+        fo.adamw_fp32_sr(Wo, mo, vo, G, 10, *hpt, seed=seed, stream=i)
+        Wg = synth.bf16_bits(d["W"])
+        assert np.abs(Wg.astype(np.int32) - Wo.astype(np.int32)).max() <= 1          # always a neighbour
+        assert float((Wg == Wo).mean()) > 0.995, float((Wg == Wo).mean())
+        Wr = synth.bf16_bits(t["W"])
+        assert np.abs(Wg.astype(np.int32) - Wr.astype(np.int32)).max() <= 1 and float((Wg != Wr).mean()) > 0.2
+    # bf16 moments run too; int8 is refused
+    fb.forge_wgrad_adamw_sr_grouped([dict(X=ps[0].X.to(DEV), dY=ps[0].dY.to(DEV), W=ps[0].W.to(DEV).clone(),
+                                          m=ps[0].m.to(torch.bfloat16).to(DEV), v=ps[0].v.to(torch.bfloat16).to(DEV))],
+                                    3, *hpt, fb.BF16, 5)
+    assert fb.forge_wgrad_adamw_sr_grouped(probs, 11, *hpt, fb.INT8, seed, check=False) == 5
+    torch.cuda.synchronize()

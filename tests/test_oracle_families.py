@@ -150,3 +150,59 @@ def test_accumulate_into_state_is_addmm_with_beta():
     exp = fo.f64_to_bf16(mu * fo.bf16_to_f64(Bb) + fo.wgrad(dY, X))
     fo.accumulate(Bb, fo.wgrad(dY, X), mu)
     assert np.array_equal(Bb, exp)
+
+
+def test_stochastic_rounding_store_dead_zone_unbiasedness_and_bounds():
+    """PAPER.md:1450 SR microcheck ("dead zone, unbiasedness": RNE drift 0.000, SR -8.195e-4 vs -8.0e-4 target):
+    an update far below half a bf16 ulp never moves an RNE weight, while the SR weight drifts by the exact amount
+    on average.  Plus: SR returns one of the two bf16 neighbours of x, exactly x when x is representable, and its
+    up-probability is the fp32 fraction."""
+    w0, delta, steps, n = 1.0, -8.0e-6, 100, 4096                 # bf16 ulp below 1.0 is 2^-8 = 3.9e-3 >> |delta|
+    rne = fo.f64_to_bf16(np.full(n, w0))
+    for _ in range(steps):
+        rne = fo.f64_to_bf16(fo.bf16_to_f64(rne) + delta)
+    assert np.all(fo.bf16_to_f64(rne) == w0)                       # dead zone: drift exactly 0
+    sr = fo.f64_to_bf16(np.full(n, w0))
+    for step in range(1, steps + 1):
+        cur = fo.bf16_to_f64(sr)
+        sr = np.array([fo.bf16_sr(cur[i] + delta, fo.sr_bits(1234, step, 0, i // 64, i % 64)) for i in range(n)], np.uint16)
+    drift = float((fo.bf16_to_f64(sr) - w0).mean())
+    target = steps * delta                                         # -8.0e-4, the paper's target
+    sigma = np.sqrt(steps * abs(delta) * 2.0 ** -8 / n)            # binomial spread of the mean
+    assert abs(drift - target) < 5 * sigma, (drift, target)
+    # neighbours, exactness, probability
+    rng = np.random.default_rng(0)
+    for x in rng.normal(0, 1, 200):
+        lo_hi = {int(fo.bf16_sr(x, 0)), int(fo.bf16_sr(x, 0xFFFF))}
+        f = np.float32(x)
+        trunc = int(f.view(np.uint32)) >> 16
+        assert lo_hi <= {trunc, trunc + 1}
+        frac = int(f.view(np.uint32)) & 0xFFFF
+        ups = sum(int(fo.bf16_sr(x, r)) == trunc + 1 for r in range(0, 65536, 257))
+        assert abs(ups / 256 - frac / 65536) < 0.01
+    exact = float(fo.bf16_to_f64(fo.f64_to_bf16(np.array([0.7])))[0])
+    assert all(fo.bf16_sr(exact, r) == int(fo.f64_to_bf16(np.array([exact]))[0]) for r in (0, 1, 0x8000, 0xFFFF))
+    # the generator: 16 bits, depends on every key, roughly uniform
+    base = fo.sr_bits(1, 2, 3, 4, 5)
+    assert 0 <= base < 65536 and len({base, fo.sr_bits(2, 2, 3, 4, 5), fo.sr_bits(1, 3, 3, 4, 5), fo.sr_bits(1, 2, 4, 4, 5),
+                                      fo.sr_bits(1, 2, 3, 5, 5), fo.sr_bits(1, 2, 3, 4, 6), fo.sr_bits(1 << 40, 2, 3, 4, 5)}) == 7
+    bits = np.array([fo.sr_bits(9, 1, 0, r, c) for r in range(64) for c in range(64)])
+    assert abs(bits.mean() / 65535 - 0.5) < 0.02 and abs((bits & 1).mean() - 0.5) < 0.03
+
+
+def test_adamw_sr_equals_rne_oracle_up_to_the_final_rounding():
+    rng = np.random.default_rng(4)
+    W0 = bf16_bits(rng.normal(0, 0.02, (OUT, IN)))
+    m0 = rng.normal(0, 1e-4, (OUT, IN)).astype(np.float32)
+    v0 = np.abs(rng.normal(0, 1e-6, (OUT, IN))).astype(np.float32)
+    G = rng.normal(0, 1e-2, (OUT, IN))
+    hp = (np.float32(1e-3).item(), np.float32(0.9).item(), np.float32(0.999).item(), 1e-8, np.float32(0.1).item())
+    Wr, mr, vr = W0.copy(), m0.copy(), v0.copy()
+    Wd, _, _ = fo.adamw_fp32(Wr, mr, vr, G, 7, *hp, debug=True)
+    Ws, ms, vs = W0.copy(), m0.copy(), v0.copy()
+    fo.adamw_fp32_sr(Ws, ms, vs, G, 7, *hp, seed=99, stream=2)
+    assert np.array_equal(ms, mr) and np.array_equal(vs, vr)       # only the store of W differs
+    for i in range(0, OUT, 7):
+        for j in range(0, IN, 5):
+            assert int(Ws[i, j]) == fo.bf16_sr(Wd[i, j], fo.sr_bits(99, 7, 2, i, j))
+    assert np.all(np.abs(Ws.astype(np.int32) - Wr.astype(np.int32)) <= 1)
