@@ -65,6 +65,14 @@ def lib() -> ctypes.CDLL:
         L.forge_oracle_adamw_fp32_sr.restype = None
         L.forge_oracle_adamw_fp32_sr.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_int, c_long,
                                                  c_float, c_float, c_float, c_float, c_float, ctypes.c_uint64, ctypes.c_uint32]
+        L.forge_oracle_e4m3_from_float.restype = ctypes.c_uint8
+        L.forge_oracle_e4m3_from_float.argtypes = [c_float]
+        L.forge_oracle_e4m3_to_double.restype = c_double
+        L.forge_oracle_e4m3_to_double.argtypes = [ctypes.c_uint8]
+        L.forge_oracle_fp8_quantize.restype = None
+        L.forge_oracle_fp8_quantize.argtypes = [c_void_p, c_size_t, c_void_p, c_void_p]
+        L.forge_oracle_adamw_fp8.restype = None
+        L.forge_oracle_adamw_fp8.argtypes = [c_void_p] * 6 + [c_size_t, c_long, c_float, c_float, c_float, c_float, c_float]
         L.forge_oracle_accumulate.restype = None
         L.forge_oracle_accumulate.argtypes = [c_void_p, c_int, c_void_p, c_size_t, c_float]
         L.forge_oracle_family_step.restype = None
@@ -239,3 +247,36 @@ def adamw_fp32_sr(W, m, v, G, step, lr, beta1, beta2, eps, wd, seed, stream=0):
     assert W.ndim == 2 and W.shape == m.shape == v.shape == G.shape
     lib().forge_oracle_adamw_fp32_sr(_p(W), _p(m), _p(v), _p(G), W.shape[0], W.shape[1], int(step), lr, beta1, beta2,
                                      eps, wd, int(seed), int(stream))
+
+
+# ------------------------------------------------------------------ fp8 (e4m3) moments ------
+def e4m3_from_float(t: float) -> int:
+    return int(lib().forge_oracle_e4m3_from_float(float(np.float32(t))))
+
+
+def e4m3_to_double(code: int) -> float:
+    return float(lib().forge_oracle_e4m3_to_double(int(code)))
+
+
+def fp8_quantize(x: np.ndarray):
+    """fp32 tensor -> (e4m3 codes uint8, scale float32[2] = [amax/448, 0]) (reading S17)."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    code = np.empty(x.shape, np.uint8)
+    scale = np.zeros(2, np.float32)
+    lib().forge_oracle_fp8_quantize(_p(x), x.size, _p(code), _p(scale))
+    return code, scale
+
+
+def fp8_dequantize(code: np.ndarray, scale) -> np.ndarray:
+    lut = np.array([e4m3_to_double(c) for c in range(256)])
+    return lut[code] * float(scale[0])
+
+
+def adamw_fp8(W, mq, vq, m_scale, v_scale, G, step, lr, beta1, beta2, eps, wd):
+    """In place AdamW with e4m3 moments, per-tensor delayed scaling (reading S17).
+    m_scale / v_scale float32[2]: [0] scale in use, [1] amax of this step's m' / v' (max-accumulated)."""
+    _chk(W, np.uint16, "W"); _chk(mq, np.uint8, "mq"); _chk(vq, np.uint8, "vq"); _chk(G, np.float64, "G")
+    _chk(m_scale, np.float32, "m_scale"); _chk(v_scale, np.float32, "v_scale")
+    assert W.shape == mq.shape == vq.shape == G.shape and m_scale.shape == v_scale.shape == (2,)
+    lib().forge_oracle_adamw_fp8(_p(W), _p(mq), _p(vq), _p(m_scale), _p(v_scale), _p(G), W.size, int(step),
+                                 lr, beta1, beta2, eps, wd)

@@ -199,3 +199,80 @@ void forge_oracle_adamw_fp32_sr(uint16_t *W, float *m, float *v, const double *G
             v[i] = (float)v1;
         }
 }
+
+/* ---------------------------------------------------------------- fp8 moments ---------------
+ * "FORGE fp8 states (per-tensor scale) ... per-tensor scaled with delayed scaling, so its error is reported
+ * rather than bounded".  The paper fixes neither the format nor the scaling rule; DESIGN.md
+ * reading S17: m and v are stored as e4m3 (4 exponent bits, bias 7, 3 mantissa bits, max finite 448, no Inf)
+ * codes of x / s with one fp32 scale s per tensor; DELAYED scaling: the scale in use was derived by the caller
+ * from the amax the previous step reported (s = amax_prev / 448); this step reports its own amax of m', v'
+ * for the next one.  Values beyond 448 s saturate (round-to-nearest-even, satfinite -- the hardware cvt).
+ * The code decision is taken in the kernel's precision: code = e4m3(fp32(fp32(x) * fp32(1/s))). */
+uint8_t forge_oracle_e4m3_from_float(float t)
+{
+    uint32_t b;
+    __builtin_memcpy(&b, &t, 4);
+    uint8_t sign = (uint8_t)((b >> 24) & 0x80u);
+    double a = fabs((double)t);
+    if (t != t) return (uint8_t)(sign | 0x7Fu);            /* NaN */
+    if (a > 448.0) return (uint8_t)(sign | 0x7Eu);         /* satfinite (includes Inf) */
+    if (a < 0.015625) {                                    /* below the smallest normal 2^-6: subnormal grid 2^-9 */
+        int q = (int)rint(a * 512.0);                      /* ties to even; q == 8 is the smallest normal, code 0x08 */
+        return (uint8_t)(sign | (uint8_t)q);
+    }
+    int e;
+    double f = frexp(a, &e);                               /* a = f * 2^e, f in [0.5, 1) */
+    double mant = f * 2.0; e -= 1;                         /* mant in [1, 2) */
+    int q = (int)rint((mant - 1.0) * 8.0);
+    if (q == 8) { q = 0; e += 1; }
+    int code = ((e + 7) << 3) | q;
+    if (code > 0x7E) code = 0x7E;
+    return (uint8_t)(sign | (uint8_t)code);
+}
+double forge_oracle_e4m3_to_double(uint8_t c)
+{
+    double s = (c & 0x80u) ? -1.0 : 1.0;
+    int e = (c >> 3) & 0xF, q = c & 7;
+    if (e == 0xF && q == 7) return NAN;
+    if (e == 0) return s * (double)q * 0.001953125;        /* q * 2^-9 */
+    return s * (1.0 + (double)q / 8.0) * ldexp(1.0, e - 7);
+}
+static float fp8_inv_scale(float s) { volatile float r = (s > 0.0f) ? 1.0f / s : 0.0f; return r; }
+
+/* quantise one fp32 tensor: scale = amax / 448, codes as above */
+void forge_oracle_fp8_quantize(const float *x, size_t n, uint8_t *code, float *scale)
+{
+    float amax = 0.0f;
+    for (size_t i = 0; i < n; ++i) { float a = fabsf(x[i]); if (a > amax) amax = a; }
+    volatile float s = amax / 448.0f;
+    *scale = s;
+    float inv = fp8_inv_scale(s);
+    for (size_t i = 0; i < n; ++i) { volatile float t = x[i] * inv; code[i] = forge_oracle_e4m3_from_float(t); }
+}
+
+/* AdamW (Algorithm 1) with e4m3 moments.  m_scale / v_scale: [0] = scale in use (read),
+ * [1] = amax of this step's m' / v' (max-accumulated into the incoming value). */
+void forge_oracle_adamw_fp8(uint16_t *W, uint8_t *mq, uint8_t *vq, float *m_scale, float *v_scale, const double *G,
+                            size_t n, long step, float lr, float beta1, float beta2, float eps, float wd)
+{
+    const double b1 = beta1, b2 = beta2, bc1 = 1.0 - pow(b1, (double)step), bc2 = 1.0 - pow(b2, (double)step);
+    const double sm = (double)m_scale[0], sv = (double)v_scale[0];
+    const float inv_m = fp8_inv_scale(m_scale[0]), inv_v = fp8_inv_scale(v_scale[0]);
+    float am = m_scale[1], av = v_scale[1];
+#pragma omp parallel for schedule(static) reduction(max : am, av)
+    for (size_t i = 0; i < n; ++i) {
+        double w = forge_oracle_bf16_to_double(W[i]);
+        double m1 = b1 * (forge_oracle_e4m3_to_double(mq[i]) * sm) + (1.0 - b1) * G[i];
+        double v1 = b2 * (forge_oracle_e4m3_to_double(vq[i]) * sv) + (1.0 - b2) * G[i] * G[i];
+        double w1 = (1.0 - (double)lr * (double)wd) * w - (double)lr * (m1 / bc1) / (sqrt(v1 / bc2) + (double)eps);
+        W[i] = forge_oracle_bf16_from_double(w1);
+        volatile float tm = (float)m1 * inv_m, tv = (float)v1 * inv_v;
+        mq[i] = forge_oracle_e4m3_from_float(tm);
+        vq[i] = forge_oracle_e4m3_from_float(tv);
+        float fm = fabsf((float)m1), fv = fabsf((float)v1);
+        if (fm > am) am = fm;
+        if (fv > av) av = fv;
+    }
+    m_scale[1] = am;
+    v_scale[1] = av;
+}

@@ -206,3 +206,60 @@ def test_adamw_sr_equals_rne_oracle_up_to_the_final_rounding():
         for j in range(0, IN, 5):
             assert int(Ws[i, j]) == fo.bf16_sr(Wd[i, j], fo.sr_bits(99, 7, 2, i, j))
     assert np.all(np.abs(Ws.astype(np.int32) - Wr.astype(np.int32)) <= 1)
+
+
+def test_e4m3_codec_against_torch_float8_and_by_hand():
+    """e4m3 (bias 7, 3 mantissa bits, max 448, subnormal grid 2^-9): every code decodes like torch.float8_e4m3fn;
+    encoding matches torch's RNE cast wherever torch does not overflow; beyond 448 the oracle saturates (the
+    hardware cvt.rn.satfinite; torch's cast returns NaN there)."""
+    codes = torch.arange(256, dtype=torch.uint8)
+    ref = codes.view(torch.float8_e4m3fn).float().numpy()
+    mine = np.array([fo.e4m3_to_double(c) for c in range(256)])
+    assert np.array_equal(np.isnan(ref), np.isnan(mine)) and np.array_equal(ref[~np.isnan(ref)], mine[~np.isnan(mine)])
+    rng = np.random.default_rng(8)
+    xs = np.concatenate([rng.normal(0, 100, 20000), rng.normal(0, 0.02, 20000), rng.uniform(-448, 448, 20000),
+                         mine[~np.isnan(mine)], (mine[:-1] + mine[1:])[~np.isnan(mine[:-1] + mine[1:])] / 2]).astype(np.float32)
+    xs = xs[np.abs(xs) <= 448]
+    tref = torch.from_numpy(xs).to(torch.float8_e4m3fn).view(torch.uint8).numpy()
+    got = np.array([fo.e4m3_from_float(x) for x in xs], np.uint8)
+    nz = (tref & 0x7F) != 0                                   # +0 / -0 of tiny negatives: compare magnitudes only there
+    assert np.array_equal(got[nz], tref[nz]) and np.all((got[~nz] & 0x7F) == 0)
+    # by hand: ties to even on the subnormal grid, carry into the exponent, saturation, NaN
+    assert fo.e4m3_from_float(2.0 ** -10) == 0 and fo.e4m3_from_float(1.5 * 2.0 ** -10) == 1
+    assert fo.e4m3_from_float(3 * 2.0 ** -10) == 2                       # 1.5 grid units: tie -> even (2)
+    assert fo.e4m3_from_float(1.9375) == 0x40 and fo.e4m3_from_float(1.0) == 0x38 and fo.e4m3_from_float(-1.0) == 0xB8
+    assert fo.e4m3_from_float(448.0) == 0x7E and fo.e4m3_from_float(1e9) == 0x7E and fo.e4m3_from_float(-1e9) == 0xFE
+    assert fo.e4m3_from_float(float("inf")) == 0x7E and (fo.e4m3_from_float(float("nan")) & 0x7F) == 0x7F
+
+
+def test_fp8_quantiser_and_step_properties():
+    rng = np.random.default_rng(12)
+    x = rng.normal(0, 1e-4, (OUT, IN)).astype(np.float32)
+    code, scale = fo.fp8_quantize(x)
+    assert scale[0] == np.float32(np.abs(x).max() / np.float32(448.0))
+    deq = fo.fp8_dequantize(code, scale)
+    # relative error <= 2^-4 (3 mantissa bits) for normals, absolute <= half the subnormal grid below
+    err = np.abs(deq - x)
+    assert np.all(err <= np.maximum(np.abs(x) * 2.0 ** -4, 2.0 ** -10 * scale[0]) * 1.0001)
+    assert (code.flatten()[np.abs(x).argmax()] & 0x7F) == 0x7E            # the absmax element maps to +-448
+    # one AdamW step: consistent with the fp32-moment oracle started from the dequantised state
+    W0 = bf16_bits(rng.normal(0, 0.02, (OUT, IN)))
+    v0 = np.abs(rng.normal(0, 1e-6, (OUT, IN))).astype(np.float32)
+    vq, vs = fo.fp8_quantize(v0)
+    G = rng.normal(0, 1e-2, (OUT, IN))
+    hp = (np.float32(1e-3).item(), np.float32(0.9).item(), np.float32(0.999).item(), 1e-8, np.float32(0.1).item())
+    Wr = W0.copy(); mr = fo.fp8_dequantize(code, scale).astype(np.float32); vr = fo.fp8_dequantize(vq, vs).astype(np.float32)
+    m_in, v_in = mr.astype(np.float64), vr.astype(np.float64)
+    fo.adamw_fp32(Wr, mr, vr, G, 5, *hp)
+    Wq, mq2, vq2, ms, vs2 = W0.copy(), code.copy(), vq.copy(), scale.copy(), vs.copy()
+    fo.adamw_fp8(Wq, mq2, vq2, ms, vs2, G, 5, *hp)
+    assert np.array_equal(Wq, Wr)                                        # W' comes from the unrounded m', v' (S3)
+    assert ms[0] == scale[0] and np.isclose(ms[1], np.abs(mr).max(), rtol=1e-6) and np.isclose(vs2[1], vr.max(), rtol=1e-6)
+    # stored m' = e4m3(m' / s): decoding recovers m' to 2^-4 relative (or saturates at 448 s when m' outgrew the old scale)
+    mdeq = fo.fp8_dequantize(mq2, ms)
+    lim = 448.0 * float(ms[0])
+    ok = np.abs(mdeq - np.clip(mr, -lim, lim)) <= np.maximum(np.abs(mr) * 2.0 ** -4, 2.0 ** -10 * ms[0]) * 1.001
+    assert ok.all()
+    # delayed scaling: feeding the reported amax back gives a scale under which nothing saturates
+    nxt = np.float32(ms[1] / np.float32(448.0))
+    assert np.abs(mr).max() <= 448.0 * float(nxt) * (1 + 1e-6)
