@@ -28,12 +28,12 @@ if ROOT not in sys.path:
 
 METRIC = "fused wgrad+AdamW us/layer (Llama-3.1-8B layer, 7 projections, BT=512, 1xB200)"
 UNIT = "us/layer"
-MOMENT_BYTES = {"fp32": 20.0, "bf16": 12.0, "int8": 8.0 + 2 * 2 * 4 / 256}   # SURVEY.md 8(d), B/element
-MOMENT_ENUM = {"fp32": 0, "bf16": 1, "int8": 2}
+MOMENT_BYTES = {"fp32": 20.0, "bf16": 12.0, "int8": 8.0 + 2 * 2 * 4 / 256, "fp8": 8.0}   # SURVEY.md 8(d), B/element
+MOMENT_ENUM = {"fp32": 0, "bf16": 1, "int8": 2, "fp8": 3}
 T_TOKENS = 512
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed
 # ncu --set full capture (profiles/); None until a capture of the current kernel exists.
-NCU_TRAFFIC_BYTES = {"fp32": 4376165000, "bf16": 2747416000, "int8": 1868895000}
+NCU_TRAFFIC_BYTES = {"fp32": 4376165000, "bf16": 2747416000, "int8": 1868895000, "fp8": None}
 
 
 def measured_peaks():
@@ -122,6 +122,13 @@ def make_device_layer(moments: str, seed: int, device, workload: str = "layer", 
             d["m"], d["v"] = p.m, p.v
         elif moments == "bf16":
             d["m"], d["v"] = p.m.to(torch.bfloat16), p.v.to(torch.bfloat16)
+        elif moments == "fp8":
+            # e4m3 codes of x / s, s = amax / 448 (torch's cast; initial state only), scale pair [s, amax-out]
+            sm, sv = p.m.abs().amax() / 448.0, p.v.amax() / 448.0
+            d["m"] = (p.m / sm).to(torch.float8_e4m3fn).view(torch.uint8)
+            d["v"] = (p.v / sv).to(torch.float8_e4m3fn).view(torch.uint8)
+            d["m_scale"] = torch.stack([sm, torch.zeros_like(sm)]).float().contiguous()
+            d["v_scale"] = torch.stack([sv, torch.zeros_like(sv)]).float().contiguous()
         else:
             # seed codes/scales with torch ops only (initial state; the method's arithmetic starts at step 1)
             nb = p.inn // 256
@@ -340,8 +347,8 @@ def run_cuda(args):
     layer = make_device_layer(args.moments, 20260622 + 1 + rank, dev, args.workload, args.tokens)
     nst = fb.FAMILY_STATES[args.optimizer]
     if args.optimizer != "adamw":                  # keep only the states the family has
-        if args.moments == "int8":
-            raise SystemExit("int8 state is implemented for AdamW only")
+        if args.moments in ("int8", "fp8"):
+            raise SystemExit("int8 / fp8 state is implemented for AdamW only")
         for d in layer:
             v_like = d["v"]                        # non-negative: the single state of rmsprop / adagrad
             d["v"] = d["v"] if nst >= 2 else None
@@ -452,7 +459,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=30)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--moments", choices=["fp32", "bf16", "int8"], default="fp32")
+    ap.add_argument("--moments", choices=["fp32", "bf16", "int8", "fp8"], default="fp32")
     ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
     ap.add_argument("--workload", choices=["layer", "q", "k", "v", "o", "gate", "up", "down", "model"], default="layer",
                     help="layer = BASELINE.json configs[1] (the metric); a projection name = that problem alone (configs[3]); model = configs[4]")

@@ -65,7 +65,13 @@ typedef enum {
 typedef enum {
     FORGE_MOMENT_FP32 = 0,
     FORGE_MOMENT_BF16 = 1,
-    FORGE_MOMENT_INT8 = 2
+    FORGE_MOMENT_INT8 = 2,
+    FORGE_MOMENT_FP8 = 3     /* e4m3 codes, ONE fp32 scale per tensor with delayed scaling:
+                              * m, v are uint8 e4m3 codes of x / s; m_scale / v_scale point to float[2]:
+                              * [0] = the scale s in use (read; the caller derives it from the amax the previous
+                              * step reported, s = amax / 448), [1] = amax of this step's m' / v' (the kernel
+                              * max-accumulates into it: set it to 0 before the call).  Values beyond 448 s
+                              * saturate.  in % 16 == 0.  forge_wgrad_adamw[_grouped] and forge_layer_backward_grouped only. */
 } forge_moment_dtype_t;
 
 /* CUDA stream handle; identical to cudaStream_t / CUstream.  NULL is the legacy default stream. */

@@ -16,7 +16,7 @@ import torch
 
 from . import build as _build
 
-FP32, BF16, INT8 = 0, 1, 2
+FP32, BF16, INT8, FP8 = 0, 1, 2, 3
 QBLOCK = 256
 STATUS_NAMES = ["FORGE_OK", "FORGE_ERR_NULL_PTR", "FORGE_ERR_BAD_SHAPE", "FORGE_ERR_ALIGNMENT",
                 "FORGE_ERR_BAD_HYPERPARAM", "FORGE_ERR_BAD_DTYPE", "FORGE_ERR_UNSUPPORTED_ARCH",
@@ -102,7 +102,7 @@ def _stream(stream):
 
 
 def moment_dtype_of(m: torch.Tensor) -> int:
-    return {torch.float32: FP32, torch.bfloat16: BF16, torch.int8: INT8}[m.dtype]
+    return {torch.float32: FP32, torch.bfloat16: BF16, torch.int8: INT8, torch.uint8: FP8}[m.dtype]   # uint8 m = e4m3 codes
 
 
 def _check(status: int, where: str):

@@ -141,6 +141,29 @@ __device__ __forceinline__ uint32_t f32x2_to_bf16x2_sr(f32x2 p, uint32_t rowkey,
     return sr_bf16(lo2(p), rowkey, col) | (sr_bf16(hi2(p), rowkey, col + 1u) << 16);
 }
 
+// ------------------------------------------------------------------ fp8 (e4m3) moments ------
+// PAPER.md:359-362 "fp8 states (per-tensor scale) ... delayed scaling" (reading S17): stored code =
+// e4m3(x / s) with one fp32 scale per tensor; the hardware converters do the work.
+// two e4m3 codes (low 16 bits of `pair`) -> two floats holding the code values
+__device__ __forceinline__ f32x2 e4m3x2_to_f32x2(uint32_t pair) {
+    uint32_t h2;
+    asm("{\n\t.reg .b16 t;\n\tcvt.u16.u32 t, %1;\n\tcvt.rn.f16x2.e4m3x2 %0, t;\n\t}\n" : "=r"(h2) : "r"(pair));
+    float lo, hi;
+    asm("{\n\t.reg .b16 a, b;\n\tmov.b32 {a, b}, %2;\n\tcvt.f32.f16 %0, a;\n\tcvt.f32.f16 %1, b;\n\t}\n"
+        : "=f"(lo), "=f"(hi)
+        : "r"(h2));
+    return pk2(lo, hi);
+}
+// two floats -> two e4m3 codes (round to nearest even, saturate to +-448), `lo` in the low byte
+__device__ __forceinline__ uint32_t f32x2_to_e4m3x2(f32x2 p) {
+    uint32_t r;
+    asm("{\n\t.reg .b16 t;\n\tcvt.rn.satfinite.e4m3x2.f32 t, %2, %1;\n\tcvt.u32.u16 %0, t;\n\t}\n"
+        : "=r"(r)
+        : "f"(lo2(p)), "f"(hi2(p)));
+    return r;
+}
+__device__ __forceinline__ float fp8_inv_scale(float s) { return s > 0.0f ? __fdiv_rn(1.0f, s) : 0.0f; }
+
 // ------------------------------------------------------------------ int8 blockwise ---------
 // PAPER.md:316 with BASELINE.json's 256-blocks: scale a = block absmax (fp32);
 // m code = rint(x * (127/a)) in [-127,127]; v code = max(1, rint(x * (255/a))) in [1,255];

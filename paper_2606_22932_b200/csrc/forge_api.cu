@@ -84,9 +84,9 @@ forge_status_t validate_hp(int64_t step, float lr, float b1, float b2, float eps
 
 forge_status_t validate_state(const void *W, const void *m, const void *v, const float *ms, const float *vs,
                               int32_t out, int32_t in, int mdt) {
-    if (mdt < 0 || mdt > 2) return FORGE_ERR_BAD_DTYPE;
+    if (mdt < 0 || mdt > 3) return FORGE_ERR_BAD_DTYPE;
     if (!W || !m || !v) return FORGE_ERR_NULL_PTR;
-    if (mdt == FORGE_MOMENT_INT8) {
+    if (mdt == FORGE_MOMENT_INT8 || mdt == FORGE_MOMENT_FP8) {
         if (!ms || !vs) return FORGE_ERR_NULL_PTR;
     } else if (ms || vs) {
         return FORGE_ERR_BAD_DTYPE;   // scales are meaningful for INT8 only
@@ -94,8 +94,10 @@ forge_status_t validate_state(const void *W, const void *m, const void *v, const
     if (out < 8 || in < 8 || (out % 8) != 0 || (in % 8) != 0) return FORGE_ERR_BAD_SHAPE;
     if (mdt == FORGE_MOMENT_BF16 && (in % 8) != 0) return FORGE_ERR_BAD_SHAPE;
     if (mdt == FORGE_MOMENT_INT8 && (in % FORGE_QBLOCK) != 0) return FORGE_ERR_BAD_SHAPE;
+    if (mdt == FORGE_MOMENT_FP8 && (in % 16) != 0) return FORGE_ERR_BAD_SHAPE;    // 16-byte rows of 1-byte codes
     if (!aligned16(W) || !aligned16(m) || !aligned16(v)) return FORGE_ERR_ALIGNMENT;
-    if (mdt == FORGE_MOMENT_INT8 && ((reinterpret_cast<uintptr_t>(ms) & 3u) || (reinterpret_cast<uintptr_t>(vs) & 3u)))
+    if ((mdt == FORGE_MOMENT_INT8 || mdt == FORGE_MOMENT_FP8) &&
+        ((reinterpret_cast<uintptr_t>(ms) & 3u) || (reinterpret_cast<uintptr_t>(vs) & 3u)))
         return FORGE_ERR_ALIGNMENT;
     return FORGE_OK;
 }
@@ -170,7 +172,7 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
     int tiles = 0;
     constexpr CUtensorMapDataType mom_dt = (MDT == MDT_FP32) ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
                                            : (MDT == MDT_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16
-                                                              : CU_TENSOR_MAP_DATA_TYPE_UINT8);
+                                                              : CU_TENSOR_MAP_DATA_TYPE_UINT8);   // int8 and fp8 codes
     for (int i = 0; i < count; ++i) {
         const forge_problem_t &p = probs[i];
         ProblemDesc &d = P.prob[i];
@@ -273,6 +275,9 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
         case 6: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 6, 2, 64, 64>(probs, count, hp, dev, stream);
         case 7: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 2, 2, 64, 128>(probs, count, hp, dev, stream);
         case 8: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 4, 2, 32, 128>(probs, count, hp, dev, stream);
+        case 10: return launch_fused<MDT_BF16, MODE_ADAMW, 64, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 11: return launch_fused<MDT_BF16, MODE_ADAMW, 64, 3, 4, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 12: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 6, 4, 2, 64, 64>(probs, count, hp, dev, stream);
         case 9: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 2, 8, 2, 32, 128>(probs, count, hp, dev, stream);
         default: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
         }
@@ -283,9 +288,26 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
         case 3: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 4, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
         case 4: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 2, 4, 2, 128, 64, 64, 3>(probs, count, hp, dev, stream);
         case 5: return launch_fused<MDT_INT8, MODE_ADAMW, 64, 2, 2, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 8: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 5, 2, 2, 128, 64>(probs, count, hp, dev, stream);
         case 6: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 2, 2, 128, 64, 64, 4>(probs, count, hp, dev, stream);
         case 7: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 4, 2, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
         default: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 2, 2, 128, 64>(probs, count, hp, dev, stream);
+        }
+    case FORGE_MOMENT_FP8:
+        switch (variant) {
+        case 1: return launch_fused<MDT_FP8, MODE_ADAMW, 32, 4, 4, 2, 64, 128>(probs, count, hp, dev, stream);
+        case 2: return launch_fused<MDT_FP8, MODE_ADAMW, 32, 4, 8, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 3: return launch_fused<MDT_FP8, MODE_ADAMW, 32, 4, 4, 2, 32, 128>(probs, count, hp, dev, stream);
+        case 5: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 6: return launch_fused<MDT_FP8, MODE_ADAMW, 32, 8, 4, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 7: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 6, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 8: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 8, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 9: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 4, 6, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 10: return launch_fused<MDT_FP8, MODE_ADAMW, 32, 6, 6, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 11: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 4, 2, 64, 128>(probs, count, hp, dev, stream);
+        case 12: return launch_fused<MDT_FP8, MODE_ADAMW, 32, 4, 6, 2, 64, 64>(probs, count, hp, dev, stream);
+        // 8 B/element of state: the T = 512 mainloop needs the deeper operand ring (96 KB) more than the state ring does
+        default: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 4, 2, 64, 128>(probs, count, hp, dev, stream);
         }
     default:
         return FORGE_ERR_BAD_DTYPE;
@@ -385,14 +407,21 @@ forge_status_t dispatch_family(const forge_problem_t *probs, int count, int nst,
         if (forced == 1) return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 128, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
         if (forced == 2) return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 64, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
         if (forced == 3) return launch_fused<MDT, MODE_FAMILY, 32, 4, 2, 2, 128, 256, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
-        return launch_fused<MDT, MODE_FAMILY, 32, 4, 6, 2, 64, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
+        if (forced == 4) return launch_fused<MDT, MODE_FAMILY, 64, 4, 6, 2, 64, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
+        if (forced == 5) return launch_fused<MDT, MODE_FAMILY, 64, 3, 6, 2, 64, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
+        if (forced == 6) return launch_fused<MDT, MODE_FAMILY, 32, 4, 6, 2, 64, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
+        // measured: 128 KB operand ring 229 us / layer, 64 KB 298 us (4 B/element of state: the mainloop is the long pole)
+        return launch_fused<MDT, MODE_FAMILY, 64, 4, 6, 2, 64, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
     }
     if (nst == 1) {
         if (big) return launch_fused<MDT, MODE_FAMILY, 64, 4, 2, 2, 64, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
         if (forced == 1) return launch_fused<MDT, MODE_FAMILY, 32, 4, 6, 2, 64, 64, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
         if (forced == 2) return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 64, 64, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
         if (forced == 3) return launch_fused<MDT, MODE_FAMILY, 32, 4, 2, 2, 64, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
+        if (forced == 4) return launch_fused<MDT, MODE_FAMILY, 64, 4, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
+        if (forced == 5) return launch_fused<MDT, MODE_FAMILY, 64, 3, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
         // measured (momentum, fp32 / bf16 state): 32 x 128 x 4 slots 465 / 376 us, 64 x 64 x 4 483 / 396, 64 x 128 x 2 514 / 417
+        if (MDT == MDT_BF16) return launch_fused<MDT, MODE_FAMILY, 64, 4, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
         return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
     }
     if (big) return launch_fused<MDT, MODE_FAMILY, 64, 4, 2, 2, 64, 64, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
@@ -413,7 +442,7 @@ forge_status_t forge_wgrad_adamw_grouped(const forge_problem_t *problems, int32_
     if (!problems) return FORGE_ERR_NULL_PTR;
     if (count < 1) return FORGE_ERR_BAD_SHAPE;
     const int mdt = static_cast<int>(moment_dtype);
-    if (mdt < 0 || mdt > 2) return FORGE_ERR_BAD_DTYPE;
+    if (mdt < 0 || mdt > 3) return FORGE_ERR_BAD_DTYPE;
     forge_status_t s = validate_hp(step, lr, beta1, beta2, eps, wd);
     if (s != FORGE_OK) return s;
     for (int i = 0; i < count; ++i) {
@@ -509,10 +538,10 @@ forge_status_t forge_wgrad_accumulate_grouped(const forge_problem_t *problems, i
         const forge_problem_t *pp = problems + i;
         if (mdt == FORGE_MOMENT_FP32)
             s = maxT > 1024 ? launch_fused<MDT_FP32, MODE_ACCUM, 64, 4, 2, 2, 64, 128, 128, 2, 1>(pp, n, hp, dev, st, &fs)
-                            : launch_fused<MDT_FP32, MODE_ACCUM, 32, 4, 4, 2, 32, 128, 128, 2, 1>(pp, n, hp, dev, st, &fs);
+                            : launch_fused<MDT_FP32, MODE_ACCUM, 64, 4, 4, 2, 32, 128, 128, 2, 1>(pp, n, hp, dev, st, &fs);
         else
             s = maxT > 1024 ? launch_fused<MDT_BF16, MODE_ACCUM, 64, 4, 2, 2, 64, 128, 128, 2, 1>(pp, n, hp, dev, st, &fs)
-                            : launch_fused<MDT_BF16, MODE_ACCUM, 32, 4, 4, 2, 32, 128, 128, 2, 1>(pp, n, hp, dev, st, &fs);
+                            : launch_fused<MDT_BF16, MODE_ACCUM, 64, 4, 4, 2, 32, 128, 128, 2, 1>(pp, n, hp, dev, st, &fs);
         if (s != FORGE_OK) return s;
     }
     return FORGE_OK;
@@ -560,7 +589,7 @@ forge_status_t forge_layer_backward_grouped(const forge_problem_t *problems, voi
     if (!problems || !dX) return FORGE_ERR_NULL_PTR;
     if (count < 1) return FORGE_ERR_BAD_SHAPE;
     const int mdt = static_cast<int>(moment_dtype);
-    if (mdt < 0 || mdt > 2) return FORGE_ERR_BAD_DTYPE;
+    if (mdt < 0 || mdt > 3) return FORGE_ERR_BAD_DTYPE;
     forge_status_t s = validate_hp(step, lr, beta1, beta2, eps, wd);
     if (s != FORGE_OK) return s;
     for (int i = 0; i < count; ++i) {          // everything is validated before anything is enqueued
@@ -617,6 +646,7 @@ forge_status_t forge_adamw_from_g(const float *G, void *W, void *m, void *v, flo
                                   float eps, float wd, forge_moment_dtype_t moment_dtype, forge_stream_t stream) {
     if (!G) return FORGE_ERR_NULL_PTR;
     const int mdt = static_cast<int>(moment_dtype);
+    if (mdt == FORGE_MOMENT_FP8) return FORGE_ERR_BAD_DTYPE;   // the unfused twin covers fp32 / bf16 / int8
     forge_status_t s = validate_hp(step, lr, beta1, beta2, eps, wd);
     if (s != FORGE_OK) return s;
     s = validate_state(W, m, v, m_scale, v_scale, out, in, mdt);

@@ -47,7 +47,7 @@ __host__ __device__ constexpr int epi_warps(int mdt) { return mdt == 2 /*MDT_INT
 __host__ __device__ constexpr int block_threads(int mdt) { return (kCtrlWarps + epi_warps(mdt)) * 32; }
 constexpr int kTmemCols = 512;  // 2 accumulator buffers x 256 fp32 columns
 
-enum : int { MDT_FP32 = 0, MDT_BF16 = 1, MDT_INT8 = 2 };
+enum : int { MDT_FP32 = 0, MDT_BF16 = 1, MDT_INT8 = 2, MDT_FP8 = 3 };
 enum : int { MODE_ADAMW = 0, MODE_STORE_G = 1, MODE_FAMILY = 2,      // FAMILY: family_math.cuh, 0-2 state tensors
              MODE_ACCUM = 3,                                          // B <- mu*B + G, no weight
              MODE_ADAMW_SR = 4 };                                     // AdamW, stochastic-rounding store of W
@@ -95,7 +95,7 @@ template <int MDT, int kBlockK, int kStages, int kStateStages, int CG = 1, int C
 struct KernelCfg {
     static constexpr int HASW = HASW_;                      // the chunk image carries W (not in MODE_ACCUM)
     static constexpr int NST = NST_;                        // state tensors besides W in a chunk (AdamW: m, v)
-    static constexpr int kMomBytes = (MDT == MDT_FP32) ? 4 : (MDT == MDT_BF16 ? 2 : 1);
+    static constexpr int kMomBytes = (MDT == MDT_FP32) ? 4 : (MDT == MDT_BF16 ? 2 : 1);   // int8 and fp8: 1
     static constexpr int A_STAGE = kBlockK * 128 * (BLOCK_M / 64);
     static constexpr int B_STAGE = kBlockK * 128 * (BLOCK_N / 64) / CG;
     static constexpr int ML_STAGE = A_STAGE + B_STAGE;
@@ -225,6 +225,50 @@ __device__ __forceinline__ void epi_sub_fp(const AdamWScalars &hp, const uint32_
         } else {
             sts128(aw, make_uint4(f32x2_to_bf16x2(w[0]), f32x2_to_bf16x2(w[1]), f32x2_to_bf16x2(w[2]), f32x2_to_bf16x2(w[3])));
         }
+    }
+}
+
+// fp8 (e4m3) moments with per-tensor delayed scaling: ONE pass -- the scale in use comes from
+// the previous step, this step only reports its amax -- so the mode streams like bf16 at int8's byte count
+struct Fp8Row {
+    float bm, bv, inv_m, inv_v;    // beta * scale (dequantisation folded into the moment update), 1 / scale
+};
+template <class Cfg>
+__device__ __forceinline__ void epi_sub_fp8(const AdamWScalars &hp, const Fp8Row &R, const uint32_t (&g)[32],
+                                            const SubAddr<Cfg> &a, uint32_t row, float &pm, float &pv) {
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+        const uint32_t o = swz<Cfg::M_ROW>(row, a.pm + j);
+        const uint32_t am = a.m + o, av = a.v + o;
+        const uint4 mq = lds128(am), vq = lds128(av);
+        const uint32_t aw0 = a.w + swz<Cfg::W_ROW>(row, a.pw + 2 * j), aw1 = a.w + swz<Cfg::W_ROW>(row, a.pw + 2 * j + 1);
+        const uint4 w0 = lds128(aw0), w1 = lds128(aw1);
+        const uint32_t mw[4] = {mq.x, mq.y, mq.z, mq.w}, vw[4] = {vq.x, vq.y, vq.z, vq.w};
+        const uint32_t ww[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+        uint32_t mo[4], vo[4], wo[8];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            uint32_t mc = 0, vc = 0;
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int gi = 16 * j + 4 * q + 2 * e;
+                f32x2 m, v, w = bf16x2_to_f32x2(ww[2 * q + e]);
+                adamw_moments2_q(hp, pk2u(g[gi], g[gi + 1]), e4m3x2_to_f32x2(mw[q] >> (16 * e)), e4m3x2_to_f32x2(vw[q] >> (16 * e)),
+                                 R.bm, R.bv, m, v);
+                adamw_weight2(hp, m, v, w);
+                wo[2 * q + e] = f32x2_to_bf16x2(w);
+                pm = fmaxf(pm, fmaxf(fabsf(lo2(m)), fabsf(hi2(m))));
+                pv = fmaxf(pv, fmaxf(lo2(v), hi2(v)));
+                mc |= f32x2_to_e4m3x2(mul2(m, bc2(R.inv_m))) << (16 * e);
+                vc |= f32x2_to_e4m3x2(mul2(v, bc2(R.inv_v))) << (16 * e);
+            }
+            mo[q] = mc;
+            vo[q] = vc;
+        }
+        sts128(am, make_uint4(mo[0], mo[1], mo[2], mo[3]));
+        sts128(av, make_uint4(vo[0], vo[1], vo[2], vo[3]));
+        sts128(aw0, make_uint4(wo[0], wo[1], wo[2], wo[3]));
+        sts128(aw1, make_uint4(wo[4], wo[5], wo[6], wo[7]));
     }
 }
 
@@ -531,7 +575,8 @@ __global__ void __launch_bounds__(block_threads(MDT), 1)
 forge_fused_kernel(const __grid_constant__ KernelParams P) {
     constexpr int HASW = (MODE == MODE_ACCUM) ? 0 : 1;
     using Cfg = KernelCfg<MDT, kBlockK, kStages, kStateStages, CG, CM, CN, P1C, P1S, NST, HASW>;
-    static_assert(MODE != MODE_ADAMW_SR || MDT != MDT_INT8, "the SR store is implemented for fp32 / bf16 moments");
+    static_assert(MODE != MODE_ADAMW_SR || (MDT != MDT_INT8 && MDT != MDT_FP8), "the SR store is implemented for fp32 / bf16 moments");
+    static_assert(MDT != MDT_FP8 || MODE == MODE_ADAMW, "fp8 moments are implemented for AdamW");
     static_assert(MODE == MODE_FAMILY || MODE == MODE_ACCUM || NST == 2, "AdamW and the store-G twin use the two-state chunk image");
     static_assert(MODE != MODE_ACCUM || NST == 1, "accumulate-into-state has exactly one state tensor");
     static_assert((MODE != MODE_FAMILY && MODE != MODE_ACCUM) || MDT != MDT_INT8, "int8 state is implemented for AdamW only");
@@ -775,6 +820,16 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                 sr_rowkey = sr_row_key(static_cast<uint32_t>(tc.tm * BLOCK_M) + row_t, P.sr_seed_lo, P.prob[tc.p].sr_inner);
                 sr_col0 = static_cast<uint32_t>(tc.tn * BLOCK_N);
             }
+            Fp8Row f8{};
+            float f8_pm = 0.0f, f8_pv = 0.0f;
+            if constexpr (MDT == MDT_FP8) {
+                const ProblemDesc &pd = P.prob[decode_tile<CG>(P, tile, rank).p];
+                const float sm = __ldg(pd.m_scale), sv = __ldg(pd.v_scale);     // [0] = scale in use (previous step's amax / 448)
+                f8.bm = __fmul_rn(hp.beta1, sm);
+                f8.bv = __fmul_rn(hp.beta2, sv);
+                f8.inv_m = fp8_inv_scale(sm);
+                f8.inv_v = fp8_inv_scale(sv);
+            }
             if constexpr (MDT != MDT_INT8) {
                 for (int cb = 0; cb < Cfg::CB; ++cb) {
                     if (Cfg::SUBS < 2 && (cb & 1) != wg) continue;
@@ -788,7 +843,9 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                         tmem_ld_32x32b_x32(taddr + cb * CN + j32 * SUB, g);
                         const SubAddr<Cfg> a(base, j32 * SUB);
                         tmem_ld_wait();
-                        if constexpr (MODE == MODE_ADAMW) {
+                        if constexpr (MODE == MODE_ADAMW && MDT == MDT_FP8) {
+                            if (!(P.debug & DBG_NO_EPILOGUE)) epi_sub_fp8<Cfg>(hp, f8, g, a, row, f8_pm, f8_pv);
+                        } else if constexpr (MODE == MODE_ADAMW) {
                             if (!(P.debug & DBG_NO_EPILOGUE)) epi_sub_fp<MDT, Cfg>(hp, g, a, row);
                         } else if constexpr (MODE == MODE_ADAMW_SR) {
                             epi_sub_fp<MDT, Cfg, true>(hp, g, a, row, sr_rowkey, sr_col0 + cb * CN + j32 * SUB);
@@ -802,6 +859,18 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                     }
                     fence_proxy_async_smem();
                     mbar_arrive(bar_st_done + 8 * s);
+                }
+                if constexpr (MDT == MDT_FP8) {          // this step's amax of m', v' for the NEXT step's scale
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) {
+                        f8_pm = fmaxf(f8_pm, __shfl_xor_sync(0xffffffffu, f8_pm, o));
+                        f8_pv = fmaxf(f8_pv, __shfl_xor_sync(0xffffffffu, f8_pv, o));
+                    }
+                    if (lane == 0) {                     // non-negative floats order like their bit patterns
+                        const ProblemDesc &pd = P.prob[decode_tile<CG>(P, tile, rank).p];
+                        atomicMax(reinterpret_cast<unsigned int *>(pd.m_scale + 1), __float_as_uint(f8_pm));
+                        atomicMax(reinterpret_cast<unsigned int *>(pd.v_scale + 1), __float_as_uint(f8_pv));
+                    }
                 }
             } else {
                 // old block scales of this row: loaded one tile ahead (global latency off the critical path)

@@ -65,7 +65,9 @@ def test_argument_validation_happens_before_any_cuda_call(lib):
     assert _call(lib, hp=(1, 1e-3, 0.9, -0.1, 1e-8, 0.1)) == BAD_HP
     assert _call(lib, hp=(1, 1e-3, 0.9, 0.999, float("nan"), 0.1)) == BAD_HP
     assert _call(lib, hp=(1, 1e-3, 0.9, 0.999, 1e-8, -1.0)) == BAD_HP
-    assert _call(lib, mdt=3) == BAD_DT and _call(lib, mdt=-1) == BAD_DT
+    assert _call(lib, mdt=4) == BAD_DT and _call(lib, mdt=-1) == BAD_DT
+    assert _call(lib, mdt=3) == NULL_PTR                      # FP8 needs its scale / amax pairs
+    assert _call(lib, mdt=3, ms=0x6000, vs=0x7000, inn=264) == BAD_SHAPE   # in % 16 for 1-byte codes
     assert _call(lib, mdt=0, ms=0x6000, vs=0x7000) == BAD_DT  # scales only with INT8
     assert _call(lib, mdt=2) == NULL_PTR                      # INT8 needs scales
     assert _call(lib, mdt=2, ms=0x6000, vs=0x7000, inn=384) == BAD_SHAPE   # in % 256

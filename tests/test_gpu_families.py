@@ -170,3 +170,41 @@ def test_adamw_stochastic_rounding_store_matches_oracle_generator():
                                     3, *hpt, fb.BF16, 5)
     assert fb.forge_wgrad_adamw_sr_grouped(probs, 11, *hpt, fb.INT8, seed, check=False) == 5
     torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("T,out,inn", [(200, 136, 272), (512, 384, 768), (2048, 256, 512)])
+def test_adamw_fp8_moments_delayed_scaling(T, out, inn):
+    """SURVEY.md 8(f) rank 1 (reading S17): e4m3 moments, one scale per tensor,
+    delayed scaling.  Codes within one e4m3 step of the oracle's (the decision x*inv -> e4m3 is taken in fp32 on
+    both sides; they differ only where the fp32 m', v' differ), W as for fp32 moments, the reported amax to 1e-5."""
+    hp = synth.HP_DEFAULT
+    hpt = (hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
+    p = synth.make_problem("f8", T, out, inn, 51)
+    mq, ms = fo.fp8_quantize(p.m.numpy())
+    vq, vs = fo.fp8_quantize(p.v.numpy())
+    Wg = p.W.to(DEV).clone()
+    mg, vg = torch.from_numpy(mq.copy()).to(DEV), torch.from_numpy(vq.copy()).to(DEV)
+    msg, vsg = torch.from_numpy(ms.copy()).to(DEV), torch.from_numpy(vs.copy()).to(DEV)
+    fb.forge_wgrad_adamw(p.X.to(DEV), p.dY.to(DEV), Wg, mg, vg, 10, *hpt, m_scale=msg, v_scale=vsg, moment_dtype=fb.FP8)
+    torch.cuda.synchronize()
+    Wo, mo, vo, mso, vso = synth.bf16_bits(p.W).copy(), mq.copy(), vq.copy(), ms.copy(), vs.copy()
+    G, E = fo.wgrad(synth.bf16_bits(p.dY), synth.bf16_bits(p.X), with_abs=True)
+    Wprev = fo.bf16_to_f64(Wo)
+    fo.adamw_fp8(Wo, mo, vo, mso, vso, G, 10, *hpt)
+    e = T * 2.0 ** -23 * E
+    # W: the fp32-moment criterion of north_star
+    Wr, Wd = fo.bf16_to_f64(Wo), fo.bf16_to_f64(synth.bf16_bits(Wg))
+    ulp = np.maximum(pu.bf16_ulp(Wr), pu.bf16_ulp(Wd)) + 2.0 ** -20 * (np.abs(Wprev) + np.abs(Wr - Wprev))
+    bad = np.where(np.abs(G) > 4 * e, np.abs(Wd - Wr) > ulp, np.abs(Wd - Wr) > 2 * hp["lr"] + ulp)
+    assert not bad.any() and float((synth.bf16_bits(Wg) == Wo).mean()) > 0.99
+    # codes: same sign, magnitude code within 1 (adjacent e4m3 values), almost all identical
+    for got, ref in ((mg.cpu().numpy(), mo), (vg.cpu().numpy(), vo)):
+        dm = np.abs((got & 0x7F).astype(int) - (ref & 0x7F).astype(int))
+        assert dm.max() <= 1 and float((got == ref).mean()) > 0.99
+        assert np.all(((got ^ ref) & 0x80 == 0) | ((got & 0x7F) <= 1) & ((ref & 0x7F) <= 1))
+    # scale in use untouched, amax of this step reported for the next step's scale
+    msn, vsn = msg.cpu().numpy(), vsg.cpu().numpy()
+    assert msn[0] == ms[0] and vsn[0] == vs[0]
+    assert np.isclose(msn[1], mso[1], rtol=1e-4) and np.isclose(vsn[1], vso[1], rtol=1e-4)
+    # missing scales are refused
+    assert fb.forge_wgrad_adamw(p.X.to(DEV), p.dY.to(DEV), Wg, mg, vg, 11, *hpt, moment_dtype=fb.FP8, check=False) == 1
