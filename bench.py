@@ -431,10 +431,10 @@ def run_cuda(args):
         host = make_host_layer(args.moments, 20260622 + 1)
         h2d = sum(sum(v.numel() * v.element_size() for v in d.values()) for d in host)
         d2h = sum(sum(d[k].numel() * d[k].element_size() for k in d if k not in ("X", "dY")) for d in host)
+        host_arr = fb.make_problem_array(host)
+
         def e2e_step(tt):
-            for d in host:
-                fb.forge_wgrad_adamw_host(d["X"], d["dY"], d["W"], d["m"], d["v"], tt, *hpt,
-                                          m_scale=d.get("m_scale"), v_scale=d.get("v_scale"))
+            fb.forge_wgrad_adamw_grouped_host(host, tt, *hpt, mdt, _arr=host_arr)
         e2e_step(1)
         n_e2e = max(1, min(3, args.steps))
         t0 = time.perf_counter()
@@ -443,7 +443,7 @@ def run_cuda(args):
         torch.cuda.synchronize()
         e2e_us = (time.perf_counter() - t0) / n_e2e * 1e6
         line["e2e"] = {"value": e2e_us, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                       "steps": n_e2e, "api": "forge_wgrad_adamw_host x7 (pinned host buffers)"}
+                       "steps": n_e2e, "api": "forge_wgrad_adamw_grouped_host, 7 problems pipelined over 3 streams (pinned host buffers)"}
         del host
         line["baselines_same_gpu"] = time_unfused_baselines(layer, hp, max(3, min(10, args.steps)))
         if world == 1:

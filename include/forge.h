@@ -172,6 +172,15 @@ forge_status_t forge_wgrad_adamw_host(const void *X, const void *dY, void *W, vo
                                       int64_t step, float lr, float beta1, float beta2, float eps, float wd,
                                       forge_moment_dtype_t moment_dtype);
 
+/* The same for a whole group with HOST buffers (every pointer of every problem is a host pointer, ideally pinned):
+ * a three-stage pipeline over the problems -- upload, fused step, download on three streams -- so the copies of
+ * neighbouring problems overlap each other (PCIe is full duplex) and the kernels.  Device scratch is allocated and
+ * freed inside the call; synchronous on return.  FP32 / BF16 / INT8 moments.  A tensor shared by several problems
+ * (q/k/v read one X) is uploaded once per problem. */
+forge_status_t forge_wgrad_adamw_grouped_host(const forge_problem_t *problems, int32_t count, int64_t step, float lr,
+                                             float beta1, float beta2, float eps, float wd,
+                                             forge_moment_dtype_t moment_dtype);
+
 /* TEST-ONLY twin (the paper's "store-G control", App. D): the identical mainloop
  * but the fp32 tile is written to G[out,in] instead of consumed.  Never on the product path. */
 forge_status_t forge_wgrad_store_g(const void *X, const void *dY, float *G,

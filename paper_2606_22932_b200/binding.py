@@ -21,7 +21,7 @@ QBLOCK = 256
 STATUS_NAMES = ["FORGE_OK", "FORGE_ERR_NULL_PTR", "FORGE_ERR_BAD_SHAPE", "FORGE_ERR_ALIGNMENT",
                 "FORGE_ERR_BAD_HYPERPARAM", "FORGE_ERR_BAD_DTYPE", "FORGE_ERR_UNSUPPORTED_ARCH",
                 "FORGE_ERR_CUDA"]
-EXPORTS = ["forge_wgrad_adamw", "forge_wgrad_adamw_grouped", "forge_wgrad_step_grouped", "forge_wgrad_accumulate_grouped", "forge_layer_backward_grouped", "forge_wgrad_adamw_sr_grouped", "forge_wgrad_adamw_host",
+EXPORTS = ["forge_wgrad_adamw", "forge_wgrad_adamw_grouped", "forge_wgrad_step_grouped", "forge_wgrad_accumulate_grouped", "forge_layer_backward_grouped", "forge_wgrad_adamw_sr_grouped", "forge_wgrad_adamw_host", "forge_wgrad_adamw_grouped_host",
            "forge_wgrad_store_g", "forge_adamw_from_g", "forge_workspace_bytes", "forge_launch_count",
            "forge_last_cuda_error", "forge_status_string", "forge_version"]
 
@@ -65,6 +65,8 @@ def lib() -> ctypes.CDLL:
         L.forge_wgrad_adamw.argtypes = [c_void_p] * 7 + [c_int32] * 3 + hp + [ctypes.c_int, c_void_p]
         L.forge_wgrad_adamw_grouped.restype = ctypes.c_int
         L.forge_wgrad_adamw_grouped.argtypes = [ctypes.POINTER(forge_problem_t), c_int32] + hp + [ctypes.c_int, c_void_p]
+        L.forge_wgrad_adamw_grouped_host.restype = ctypes.c_int
+        L.forge_wgrad_adamw_grouped_host.argtypes = [ctypes.POINTER(forge_problem_t), c_int32] + hp + [ctypes.c_int]
         L.forge_wgrad_step_grouped.restype = ctypes.c_int
         L.forge_wgrad_step_grouped.argtypes = [ctypes.POINTER(forge_problem_t), c_int32, ctypes.POINTER(forge_opt_desc_t),
                                                ctypes.c_int, c_void_p]
@@ -205,6 +207,15 @@ def forge_wgrad_adamw_host(X, dY, W, m, v, step, lr, beta1, beta2, eps, wd, m_sc
                                       T, out, inn, int(step), lr, beta1, beta2, eps, wd, moment_dtype_of(m))
     if check:
         _check(st, "forge_wgrad_adamw_host")
+    return st
+
+
+def forge_wgrad_adamw_grouped_host(problems, step, lr, beta1, beta2, eps, wd, moment_dtype, check=True, _arr=None) -> int:
+    """Host-buffer group entry (CPU tensors, ideally pinned): pipelined H2D / fused step / D2H per problem."""
+    arr = make_problem_array(problems) if _arr is None else _arr
+    st = lib().forge_wgrad_adamw_grouped_host(arr, len(arr), int(step), lr, beta1, beta2, eps, wd, moment_dtype)
+    if check:
+        _check(st, "forge_wgrad_adamw_grouped_host")
     return st
 
 

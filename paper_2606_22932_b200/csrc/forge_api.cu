@@ -724,6 +724,105 @@ forge_status_t forge_wgrad_adamw_host(const void *X, const void *dY, void *W, vo
     return FORGE_OK;
 }
 
+forge_status_t forge_wgrad_adamw_grouped_host(const forge_problem_t *problems, int32_t count, int64_t step, float lr,
+                                             float beta1, float beta2, float eps, float wd,
+                                             forge_moment_dtype_t moment_dtype) {
+    if (!problems) return FORGE_ERR_NULL_PTR;
+    if (count < 1) return FORGE_ERR_BAD_SHAPE;
+    const int mdt = static_cast<int>(moment_dtype);
+    if (mdt < 0 || mdt > 2) return FORGE_ERR_BAD_DTYPE;
+    forge_status_t s = validate_hp(step, lr, beta1, beta2, eps, wd);
+    if (s != FORGE_OK) return s;
+    for (int i = 0; i < count; ++i) {
+        s = validate_problem(problems[i], mdt);
+        if (s != FORGE_OK) return s;
+    }
+    const size_t mom = mdt == FORGE_MOMENT_FP32 ? 4 : (mdt == FORGE_MOMENT_BF16 ? 2 : 1);
+    auto up = [](size_t b) { return (b + 255) / 256 * 256; };
+    struct Sizes { size_t bX, bY, bW, bM, bS, off; };
+    Sizes *sz = static_cast<Sizes *>(std::malloc(sizeof(Sizes) * count));
+    forge_problem_t *dp = static_cast<forge_problem_t *>(std::malloc(sizeof(forge_problem_t) * count));
+    if (!sz || !dp) { std::free(sz); std::free(dp); return cuda_fail(cudaErrorMemoryAllocation); }
+    size_t total = 0;
+    for (int i = 0; i < count; ++i) {
+        const forge_problem_t &p = problems[i];
+        const size_t n = static_cast<size_t>(p.out) * p.in;
+        sz[i] = {static_cast<size_t>(p.T) * p.in * 2, static_cast<size_t>(p.T) * p.out * 2, n * 2, n * mom,
+                 mdt == FORGE_MOMENT_INT8 ? n / FORGE_QBLOCK * 4 : 0, total};
+        total += up(sz[i].bX) + up(sz[i].bY) + up(sz[i].bW) + 2 * up(sz[i].bM) + 2 * up(sz[i].bS);
+    }
+    uint8_t *d = nullptr;
+    cudaStream_t s_in = nullptr, s_c = nullptr, s_out = nullptr;
+    cudaEvent_t *ev = static_cast<cudaEvent_t *>(std::calloc(2 * count, sizeof(cudaEvent_t)));
+    cudaError_t e = cudaMalloc(&d, total);
+    auto cleanup = [&]() {
+        if (ev) for (int i = 0; i < 2 * count; ++i) if (ev[i]) cudaEventDestroy(ev[i]);
+        if (s_in) cudaStreamDestroy(s_in);
+        if (s_c) cudaStreamDestroy(s_c);
+        if (s_out) cudaStreamDestroy(s_out);
+        if (d) cudaFree(d);
+        std::free(ev); std::free(sz); std::free(dp);
+    };
+    forge_status_t rc = FORGE_OK;
+#define FORGE_TRY(x) do { if (e == cudaSuccess) e = (x); } while (0)
+    FORGE_TRY(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
+    FORGE_TRY(cudaStreamCreateWithFlags(&s_c, cudaStreamNonBlocking));
+    FORGE_TRY(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
+    for (int i = 0; i < 2 * count && ev; ++i) FORGE_TRY(cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming));
+    // three-stage pipeline over the problems: copy-in (H2D), fused step, copy-out (D2H) on three streams, so the
+    // upload of problem i+1 and the download of problem i-1 overlap the kernel of problem i (PCIe is full duplex)
+    // largest problem first: the download that cannot overlap anything (the last one) is then the smallest
+    int *order = static_cast<int *>(std::malloc(sizeof(int) * count));
+    for (int i = 0; i < count && order; ++i) order[i] = i;
+    for (int i = 0; i < count && order; ++i)
+        for (int j = i + 1; j < count; ++j)
+            if (sz[order[j]].bW > sz[order[i]].bW) { const int t = order[i]; order[i] = order[j]; order[j] = t; }
+    for (int k = 0; k < count && order && e == cudaSuccess && rc == FORGE_OK; ++k) {
+        const int i = order[k];
+        const forge_problem_t &p = problems[i];
+        uint8_t *q = d + sz[i].off;
+        forge_problem_t &g = dp[i];
+        g = p;
+        g.X = q; q += up(sz[i].bX);
+        g.dY = q; q += up(sz[i].bY);
+        g.W = q; q += up(sz[i].bW);
+        g.m = q; q += up(sz[i].bM);
+        g.v = q; q += up(sz[i].bM);
+        g.m_scale = sz[i].bS ? reinterpret_cast<float *>(q) : nullptr; q += up(sz[i].bS);
+        g.v_scale = sz[i].bS ? reinterpret_cast<float *>(q) : nullptr;
+        FORGE_TRY(cudaMemcpyAsync(const_cast<void *>(g.X), p.X, sz[i].bX, cudaMemcpyHostToDevice, s_in));
+        FORGE_TRY(cudaMemcpyAsync(const_cast<void *>(g.dY), p.dY, sz[i].bY, cudaMemcpyHostToDevice, s_in));
+        FORGE_TRY(cudaMemcpyAsync(g.W, p.W, sz[i].bW, cudaMemcpyHostToDevice, s_in));
+        FORGE_TRY(cudaMemcpyAsync(g.m, p.m, sz[i].bM, cudaMemcpyHostToDevice, s_in));
+        FORGE_TRY(cudaMemcpyAsync(g.v, p.v, sz[i].bM, cudaMemcpyHostToDevice, s_in));
+        if (sz[i].bS) {
+            FORGE_TRY(cudaMemcpyAsync(g.m_scale, p.m_scale, sz[i].bS, cudaMemcpyHostToDevice, s_in));
+            FORGE_TRY(cudaMemcpyAsync(g.v_scale, p.v_scale, sz[i].bS, cudaMemcpyHostToDevice, s_in));
+        }
+        FORGE_TRY(cudaEventRecord(ev[2 * i], s_in));
+        FORGE_TRY(cudaStreamWaitEvent(s_c, ev[2 * i], 0));
+        if (e == cudaSuccess)
+            rc = forge_wgrad_adamw_grouped(&g, 1, step, lr, beta1, beta2, eps, wd, moment_dtype, reinterpret_cast<forge_stream_t>(s_c));
+        FORGE_TRY(cudaEventRecord(ev[2 * i + 1], s_c));
+        FORGE_TRY(cudaStreamWaitEvent(s_out, ev[2 * i + 1], 0));
+        FORGE_TRY(cudaMemcpyAsync(p.W, g.W, sz[i].bW, cudaMemcpyDeviceToHost, s_out));
+        FORGE_TRY(cudaMemcpyAsync(p.m, g.m, sz[i].bM, cudaMemcpyDeviceToHost, s_out));
+        FORGE_TRY(cudaMemcpyAsync(p.v, g.v, sz[i].bM, cudaMemcpyDeviceToHost, s_out));
+        if (sz[i].bS) {
+            FORGE_TRY(cudaMemcpyAsync(p.m_scale, g.m_scale, sz[i].bS, cudaMemcpyDeviceToHost, s_out));
+            FORGE_TRY(cudaMemcpyAsync(p.v_scale, g.v_scale, sz[i].bS, cudaMemcpyDeviceToHost, s_out));
+        }
+    }
+    std::free(order);
+    if (s_in) cudaStreamSynchronize(s_in);
+    if (s_c) cudaStreamSynchronize(s_c);
+    if (s_out) FORGE_TRY(cudaStreamSynchronize(s_out));
+#undef FORGE_TRY
+    cleanup();
+    if (rc != FORGE_OK) return rc;
+    return e == cudaSuccess ? FORGE_OK : cuda_fail(e);
+}
+
 size_t forge_workspace_bytes(void) { return 0; }
 uint64_t forge_launch_count(void) { return g_launches.load(); }
 int forge_last_cuda_error(void) { return g_last_cuda_error.load(); }

@@ -333,3 +333,17 @@ def test_layer_backward_dgrad_reads_pre_update_weights_then_fused_step():
     assert fb.forge_layer_backward_grouped(bad, dXs, *hp_args(11), fb.FP32, check=False) == 1
     torch.cuda.synchronize()
     assert torch.equal(probs[0]["W"], W0)
+
+
+def test_grouped_host_entry_matches_device_path_bitwise():
+    """forge_wgrad_adamw_grouped_host (pipelined H2D / step / D2H): same bits as the device-resident grouped call."""
+    ps = [synth.make_problem("a", 200, 136, 264, 61), synth.make_problem("b", 96, 256, 512, 62), synth.make_problem("c", 64, 128, 256, 63)]
+    host = [dict(X=p.X.pin_memory(), dY=p.dY.pin_memory(), W=p.W.clone().pin_memory(), m=p.m.clone().pin_memory(),
+                 v=p.v.clone().pin_memory()) for p in ps]
+    devs = [dict(X=p.X.to(DEV), dY=p.dY.to(DEV), W=p.W.to(DEV).clone(), m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone()) for p in ps]
+    fb.forge_wgrad_adamw_grouped_host(host, *hp_args(10), fb.FP32)
+    fb.forge_wgrad_adamw_grouped(devs, *hp_args(10), fb.FP32)
+    torch.cuda.synchronize()
+    for h, d, p in zip(host, devs, ps):
+        assert torch.equal(h["W"], d["W"].cpu()) and torch.equal(h["m"], d["m"].cpu()) and torch.equal(h["v"], d["v"].cpu())
+        assert not torch.equal(h["W"], p.W)
