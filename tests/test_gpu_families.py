@@ -208,3 +208,109 @@ def test_adamw_fp8_moments_delayed_scaling(T, out, inn):
     assert np.isclose(msn[1], mso[1], rtol=1e-4) and np.isclose(vsn[1], vso[1], rtol=1e-4)
     # missing scales are refused
     assert fb.forge_wgrad_adamw(p.X.to(DEV), p.dY.to(DEV), Wg, mg, vg, 11, *hpt, moment_dtype=fb.FP8, check=False) == 1
+
+
+# ------------------------------------------------------------------ full layer size, sampled rows
+@pytest.fixture(scope="module")
+def layer_cpu():
+    return synth.make_layer(512, seed=synth.BASE_SEED + 1)
+
+
+@pytest.mark.parametrize("family", ["momentum", "lion", "sgd"])
+def test_full_layer_family_grouped_sampled_rows(layer_cpu, family):
+    """The 7 projections of a Llama-3.1-8B layer at full size in ONE grouped launch (the configuration
+    `bench.py --optimizer` times); the oracle is exact on a deterministic sample of rows (rows are independent)."""
+    kw = dict(beta1=0.9, beta2=0.99, eps=1e-8, wd=0.05, momentum=0.9, nesterov=False)
+    lr = 1e-4 if family == "lion" else 1e-2
+    ns = fb.FAMILY_STATES[family]
+    devs = [dict(X=p.X.to(DEV), dY=p.dY.to(DEV), W=p.W.to(DEV).clone(), m=(p.m * 10).to(DEV) if ns else None, v=None)
+            for p in layer_cpu]
+    n0 = fb.forge_launch_count()
+    fb.forge_wgrad_step_grouped(devs, family, 4, lr, **kw)
+    torch.cuda.synchronize()
+    assert fb.forge_launch_count() - n0 == 1
+    for p, d in zip(layer_cpu, devs):
+        dYb, Xb = synth.bf16_bits(p.dY), synth.bf16_bits(p.X)
+        for r0, r1 in pu.sample_rows(p.out):
+            G, E = fo.wgrad(dYb, Xb, rows=(r0, r1), with_abs=True)
+            Wo = synth.bf16_bits(p.W[r0:r1]).copy()
+            Wprev = fo.bf16_to_f64(Wo)
+            so = [(p.m[r0:r1] * 10).numpy().copy()] if ns else []
+            m_before = so[0].astype(np.float64) if ns else None
+            fo.family_step(family, Wo, *(so + [None] * (2 - ns)), G, 4, lr, kw["beta1"], kw["beta2"], kw["eps"], kw["wd"],
+                           kw["momentum"], kw["nesterov"])
+            e = 512 * 2.0 ** -23 * E
+            Wr, Wd = fo.bf16_to_f64(Wo), fo.bf16_to_f64(synth.bf16_bits(d["W"][r0:r1]))
+            ulp = (np.maximum(pu.bf16_ulp(Wr), pu.bf16_ulp(Wd)) + 2.0 ** -20 * (np.abs(Wprev) + np.abs(Wr - Wprev)) + 2 * lr * e)
+            sure = np.abs(G) > 4 * e if family != "lion" else np.abs(0.9 * m_before + 0.1 * G) > 4 * e   # Lion: the sign of c
+            bad = np.where(sure, np.abs(Wd - Wr) > ulp, np.abs(Wd - Wr) > 4 * lr + ulp)
+            assert not bad.any(), f"{family} {p.name}[{r0}:{r1}]: {bad.sum()} W outside tolerance"
+            assert float((synth.bf16_bits(d["W"][r0:r1]) == Wo).mean()) > 0.98
+            if ns:
+                got = d["m"][r0:r1].cpu().numpy().astype(np.float64)
+                assert np.all(np.abs(got - so[0]) <= 2e-4 * np.abs(so[0]) + 4 * e)
+
+
+def test_full_layer_fp8_grouped_sampled_rows(layer_cpu):
+    """fp8 moments at full cfg-1 size, one grouped launch; codes / W / amax against the oracle on sampled rows."""
+    hp = synth.HP_DEFAULT
+    hpt = (hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
+    devs, keep = [], []
+    for p in layer_cpu:
+        mq, ms = fo.fp8_quantize(p.m.numpy())
+        vq, vs = fo.fp8_quantize(p.v.numpy())
+        keep.append((mq, ms, vq, vs))
+        devs.append(dict(X=p.X.to(DEV), dY=p.dY.to(DEV), W=p.W.to(DEV).clone(), m=torch.from_numpy(mq.copy()).to(DEV),
+                         v=torch.from_numpy(vq.copy()).to(DEV), m_scale=torch.from_numpy(ms.copy()).to(DEV),
+                         v_scale=torch.from_numpy(vs.copy()).to(DEV)))
+    n0 = fb.forge_launch_count()
+    fb.forge_wgrad_adamw_grouped(devs, 10, *hpt, fb.FP8)
+    torch.cuda.synchronize()
+    assert fb.forge_launch_count() - n0 == 1
+    for p, d, (mq, ms, vq, vs) in zip(layer_cpu, devs, keep):
+        dYb, Xb = synth.bf16_bits(p.dY), synth.bf16_bits(p.X)
+        amax_rows = 0.0
+        for r0, r1 in pu.sample_rows(p.out):
+            G = fo.wgrad(dYb, Xb, rows=(r0, r1))
+            Wo, mo, vo, mso, vso = synth.bf16_bits(p.W[r0:r1]).copy(), mq[r0:r1].copy(), vq[r0:r1].copy(), ms.copy(), vs.copy()
+            fo.adamw_fp8(Wo, mo, vo, mso, vso, G, 10, *hpt)
+            amax_rows = max(amax_rows, float(mso[1]))
+            assert float((synth.bf16_bits(d["W"][r0:r1]) == Wo).mean()) > 0.99
+            for got, ref in ((d["m"][r0:r1].cpu().numpy(), mo), (d["v"][r0:r1].cpu().numpy(), vo)):
+                assert np.abs((got & 0x7F).astype(int) - (ref & 0x7F).astype(int)).max() <= 1
+                assert float((got == ref).mean()) > 0.99
+        got_amax = float(d["m_scale"].cpu()[1])
+        assert got_amax >= amax_rows * (1 - 1e-5)                  # the tensor-wide amax covers every sampled row
+        assert float(d["m_scale"].cpu()[0]) == float(ms[0])
+
+
+@pytest.mark.parametrize("T,out,inn", [(1, 8, 16), (33, 8, 16), (7, 136, 24)])
+def test_tiny_and_ragged_shapes_new_entries(T, out, inn):
+    """Degenerate sizes through the widened entry points: one token, one 8-row strip, ragged everything."""
+    p = synth.make_problem("t", T, out, inn, 71, sigma_dy=1e-2)
+    G = fo.wgrad(synth.bf16_bits(p.dY), synth.bf16_bits(p.X))
+    X, dY = p.X.to(DEV), p.dY.to(DEV)
+    # momentum
+    W, m = p.W.to(DEV).clone(), (p.m * 10).to(DEV)
+    fb.forge_wgrad_step_grouped([dict(X=X, dY=dY, W=W, m=m, v=None)], "momentum", 2, 1e-2, momentum=0.9)
+    Wo, mo = synth.bf16_bits(p.W).copy(), (p.m * 10).numpy().copy()
+    fo.family_step("momentum", Wo, mo, None, G, 2, 1e-2, momentum=0.9)
+    torch.cuda.synchronize()
+    assert np.abs(synth.bf16_bits(W).astype(int) - Wo.astype(int)).max() <= 1
+    assert np.allclose(m.cpu().numpy(), mo, rtol=1e-5, atol=1e-9)
+    # accumulate
+    B = (p.m * 100).to(DEV)
+    fb.forge_wgrad_accumulate_grouped([dict(X=X, dY=dY, W=None, m=B, v=None)], 0.5)
+    Bo = (p.m * 100).numpy().copy()
+    fo.accumulate(Bo, G, 0.5)
+    torch.cuda.synchronize()
+    assert np.allclose(B.cpu().numpy(), Bo, rtol=1e-5, atol=1e-9)
+    # SR store: always a neighbour of the RNE result
+    Ws, ms_, vs_ = p.W.to(DEV).clone(), p.m.to(DEV).clone(), p.v.to(DEV).clone()
+    Wr, mr, vr = p.W.to(DEV).clone(), p.m.to(DEV).clone(), p.v.to(DEV).clone()
+    hp = synth.HP_DEFAULT
+    hpt = (hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
+    fb.forge_wgrad_adamw_sr_grouped([dict(X=X, dY=dY, W=Ws, m=ms_, v=vs_)], 3, *hpt, fb.FP32, 77)
+    fb.forge_wgrad_adamw_grouped([dict(X=X, dY=dY, W=Wr, m=mr, v=vr)], 3, *hpt, fb.FP32)
+    torch.cuda.synchronize()
+    assert np.abs(synth.bf16_bits(Ws).astype(int) - synth.bf16_bits(Wr).astype(int)).max() <= 1 and torch.equal(ms_, mr)
