@@ -345,8 +345,11 @@ def run_cuda(args):
     hp = synth.HP_DEFAULT
     mdt = MOMENT_ENUM[args.moments]
     layer = make_device_layer(args.moments, 20260622 + 1 + rank, dev, args.workload, args.tokens)
-    nst = fb.FAMILY_STATES[args.optimizer]
-    if args.optimizer != "adamw":                  # keep only the states the family has
+    nst = fb.FAMILY_STATES.get(args.optimizer, 0)
+    if args.optimizer == "storeg":
+        if args.workload in ("layer", "model"):
+            raise SystemExit("--optimizer storeg is the single-projection control: use --workload q|k|v|o|gate|up|down")
+    elif args.optimizer != "adamw":                  # keep only the states the family has
         if args.moments in ("int8", "fp8"):
             raise SystemExit("int8 / fp8 state is implemented for AdamW only")
         for d in layer:
@@ -357,8 +360,12 @@ def run_cuda(args):
     hpt = (hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
     stream = torch.cuda.current_stream()
 
+    G_ctl = torch.empty(layer[0]["W"].shape, dtype=torch.float32, device=dev) if args.optimizer == "storeg" else None
+
     def step(t):
-        if args.optimizer == "adamw":
+        if args.optimizer == "storeg":             # the paper's store-G control: same mainloop, G stored
+            fb.forge_wgrad_store_g(layer[0]["X"], layer[0]["dY"], G_ctl, stream=stream)
+        elif args.optimizer == "adamw":
             fb.forge_wgrad_adamw_grouped(layer, t, *hpt, mdt, stream=stream, _arr=arr)
         else:
             fb.forge_wgrad_step_grouped(layer, args.optimizer, t, hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"],
@@ -391,7 +398,8 @@ def run_cuda(args):
 
     params, in_bytes, flops = layer_counts(args.workload, args.tokens)
     state_b = {"fp32": 8.0, "bf16": 4.0}.get(args.moments, 0.0)
-    alg_bytes = params * (MOMENT_BYTES[args.moments] if args.optimizer == "adamw" else 4.0 + nst * state_b) + in_bytes
+    alg_bytes = params * (MOMENT_BYTES[args.moments] if args.optimizer == "adamw" else
+                          (4.0 if args.optimizer == "storeg" else 4.0 + nst * state_b)) + in_bytes   # store-G: 4 B/element of G out
     hbm_peak, tf_burst, tf_sustained, peak_src = measured_peaks()
     kernel_ms = (evs[0].elapsed_time(evs[-1])) / args.steps       # this rank's average launch duration
     gbs = alg_bytes / (kernel_ms * 1e-3) / 1e9
@@ -463,7 +471,7 @@ def main():
     ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
     ap.add_argument("--workload", choices=["layer", "q", "k", "v", "o", "gate", "up", "down", "model"], default="layer",
                     help="layer = BASELINE.json configs[1] (the metric); a projection name = that problem alone (configs[3]); model = configs[4]")
-    ap.add_argument("--optimizer", default="adamw", choices=["adamw", "sgd", "momentum", "lion", "rmsprop", "adagrad", "adamax", "nadam", "radam"],
+    ap.add_argument("--optimizer", default="adamw", choices=["adamw", "sgd", "momentum", "lion", "rmsprop", "adagrad", "adamax", "nadam", "radam", "storeg"],
                     help="SURVEY.md 8(f) rank 1: the other coordinate-wise families on the same fused mainloop")
     ap.add_argument("--tokens", type=int, default=T_TOKENS, help="T (configs[3] sweeps 512/2048/8192 on gate)")
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, same-GPU baselines and the CPU oracle leg")
