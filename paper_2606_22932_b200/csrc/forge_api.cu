@@ -157,12 +157,14 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
                             uint64_t sr_seed = 0, uint32_t sr_step = 0, uint32_t sr_stream0 = 0) {
     using Cfg = KernelCfg<MDT, BK, ST, SS, CG, CM, CN, P1C, P1S, NST, (MODE == MODE_ACCUM) ? 0 : 1>;
     auto kernel = forge_fused_kernel<MDT, MODE, BK, ST, SS, CG, CM, CN, P1C, P1S, NST>;
-    static std::once_flag once;
-    static cudaError_t attr_err = cudaSuccess;
-    std::call_once(once, [&] {
-        attr_err = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
-    });
-    if (attr_err != cudaSuccess) return cuda_fail(attr_err);
+    // the opt-in shared-memory size is a per-device function attribute: set it once per device, not once per process
+    static std::atomic<uint64_t> attr_done{0};
+    const uint64_t dev_bit = 1ull << (dev.device & 63);
+    if (!(attr_done.load(std::memory_order_acquire) & dev_bit)) {
+        const cudaError_t ae = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
+        if (ae != cudaSuccess) return cuda_fail(ae);
+        attr_done.fetch_or(dev_bit, std::memory_order_release);
+    }
 
     KernelParams P;
     std::memset(&P, 0, sizeof(P));
