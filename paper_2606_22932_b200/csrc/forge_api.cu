@@ -259,12 +259,16 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
         case 2: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 4, 2, 128, 32>(probs, count, hp, dev, stream);
         case 3: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 4, 2, 32, 128>(probs, count, hp, dev, stream);
         case 4: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 2, 4, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 5: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 4, 2, 2, 64, 64>(probs, count, hp, dev, stream);
+        // T > 1024: 128 KB operand ring; the 80 KB left for the state go further as 4 x 20 KB (32 x 64) than as 2 x 40 KB
+        case 5: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 4, 4, 2, 32, 64>(probs, count, hp, dev, stream);
+        case 14: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 4, 2, 2, 64, 64>(probs, count, hp, dev, stream);
         case 6: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
         case 7: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 2, 2, 128, 64>(probs, count, hp, dev, stream);
         case 8: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 8, 2, 64, 32>(probs, count, hp, dev, stream);
         case 9: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 8, 2, 32, 64>(probs, count, hp, dev, stream);
         case 10: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 2, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 12: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 4, 4, 2, 64, 32>(probs, count, hp, dev, stream);
+        case 13: return launch_fused<MDT_FP32, MODE_ADAMW, 128, 2, 2, 2, 64, 64>(probs, count, hp, dev, stream);
         default: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 2, 2, 64, 128>(probs, count, hp, dev, stream);
         }
     case FORGE_MOMENT_BF16:
