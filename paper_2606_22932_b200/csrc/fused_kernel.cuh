@@ -2,13 +2,13 @@
 //
 // Per weight tile (128 rows of `out` x 256 columns of `in`), Algorithm 1:
 //   lines 2-5  G_ij = sum_k dY_k,i^T X_k,j      tcgen05.mma, bf16 x bf16 -> fp32 in tensor memory
-//   line  6    load W_ij, m_ij, v_ij            TMA, CM x CN chunks (default 64 x 64) into a smem ring
+//   line  6    load W_ij, m_ij, v_ij            TMA, CM x CN chunks (64 x 128 with fp32 moments) into a smem ring
 //   lines 7-10 AdamW in fp32 registers          adamw_math.cuh
 //   line  11   store W_ij, m_ij, v_ij           in place in the smem chunk, then TMA store
 // G never leaves the SM.  One CTA owns a tile for the whole token loop, so a
 // partial-K update can never be applied.
 //
-// Warp roles (384 threads -- 512 with int8 moments --, one CTA per SM, persistent over a static tile list):
+// Warp roles (384 threads, one CTA per SM, CTA pairs share a 256 x 256 tile, persistent over a static tile list):
 //   warp 0      operand producer: TMA loads of dY / X token chunks into the mainloop ring
 //   warp 1      MMA issuer: one thread issues tcgen05.mma; accumulators double-buffered in TMEM
 //   warp 2      TMEM allocator + state loader: TMA loads of W/m/v chunks (independent of G, so
@@ -55,12 +55,12 @@ enum : int { MODE_ADAMW = 0, MODE_STORE_G = 1, MODE_FAMILY = 2,      // FAMILY: 
 struct alignas(64) ProblemDesc {
     CUtensorMap map_dY;  // [T, out] bf16, box {64, kBlockK}, SWIZZLE_128B
     CUtensorMap map_X;   // [T, in]  bf16, box {64, kBlockK}, SWIZZLE_128B
-    CUtensorMap map_W;   // [out, in] bf16, box {32, 128}, SWIZZLE_64B
-    CUtensorMap map_m;   // [out, in] moment dtype, box {32, 128}, swizzle = row bytes
+    CUtensorMap map_W;   // [out, in] bf16, box {min(CN, 64), CM}, swizzle = row bytes
+    CUtensorMap map_m;   // [out, in] state dtype, box {min(CN, 128 B worth), CM}, swizzle = row bytes
     CUtensorMap map_v;   //   (MODE_STORE_G: map_m is the fp32 G output)
-    CUtensorMap map_m1;  // INT8 only: the same m / v codes with box {128, 64}, SWIZZLE_128B, for the
-    CUtensorMap map_v1;  //   absmax pass that reads whole 256-column rows
-    float *m_scale;      // INT8 only: [out, in/256]
+    CUtensorMap map_m1;  // INT8 only: the same m / v codes with box {128, 128}, SWIZZLE_128B, for the
+    CUtensorMap map_v1;  //   absmax pass (read-only first-pass ring)
+    float *m_scale;      // INT8: [out, in/256] block absmax; FP8: float[2] = {scale in use, amax out}
     float *v_scale;
     int32_t T, out, in;
     int32_t tiles_n;     // ceil(in / 256)
