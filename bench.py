@@ -33,7 +33,7 @@ MOMENT_ENUM = {"fp32": 0, "bf16": 1, "int8": 2, "fp8": 3}
 T_TOKENS = 512
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed
 # ncu --set full capture (profiles/); None until a capture of the current kernel exists.
-NCU_TRAFFIC_BYTES = {"fp32": 4376165000, "bf16": 2747416000, "int8": 1868895000, "fp8": 1815794000}
+NCU_TRAFFIC_BYTES = {"fp32": 4378000000, "bf16": 2637000000, "int8": 1801000000, "fp8": 1763000000}
 
 
 def measured_peaks():
@@ -99,7 +99,7 @@ class ClockSampler(threading.Thread):
                         self.reasons.add(n)
             except Exception:
                 pass
-            time.sleep(0.02)
+            time.sleep(0.002)
 
     def result(self):
         sm = sorted(self.sm)
@@ -387,6 +387,7 @@ def run_cuda(args):
     for i in range(args.steps):
         step(1 + args.warmup + i)
         evs[i + 1].record(stream)
+    time.sleep(0.004)                              # the launches are asynchronous: let the sampler see the GPU under load
     barrier()
     sampler.stop_flag = True
     launches = fb.forge_launch_count() - launches0
