@@ -427,8 +427,9 @@ forge_status_t dispatch_family(const forge_problem_t *probs, int count, int nst,
         if (forced == 4) return launch_fused<MDT, MODE_FAMILY, 64, 4, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
         if (forced == 5) return launch_fused<MDT, MODE_FAMILY, 64, 3, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
         // measured (momentum, fp32 / bf16 state): 32 x 128 x 4 slots 465 / 376 us, 64 x 64 x 4 483 / 396, 64 x 128 x 2 514 / 417
-        if (MDT == MDT_BF16) return launch_fused<MDT, MODE_FAMILY, 64, 4, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
-        return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
+        if (forced == 6) return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
+        // 128 KB operand ring + 32 x 128 x 4 slots: momentum 439 us (fp32 state), 355 us (bf16); with a 64 KB operand ring 448 / 370
+        return launch_fused<MDT, MODE_FAMILY, 64, 4, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
     }
     if (big) return launch_fused<MDT, MODE_FAMILY, 64, 4, 2, 2, 64, 64, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
     if (MDT == MDT_FP32) return launch_fused<MDT, MODE_FAMILY, 32, 4, 2, 2, 64, 128, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
