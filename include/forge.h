@@ -175,7 +175,8 @@ forge_status_t forge_wgrad_adamw_host(const void *X, const void *dY, void *W, vo
 /* The same for a whole group with HOST buffers (every pointer of every problem is a host pointer, ideally pinned):
  * a three-stage pipeline over the problems -- upload, fused step, download on three streams -- so the copies of
  * neighbouring problems overlap each other (PCIe is full duplex) and the kernels.  Device scratch is allocated and
- * freed inside the call; synchronous on return.  FP32 / BF16 / INT8 moments.  A tensor shared by several problems
+ * freed inside the call; synchronous on return.  All four moment dtypes (INT8: the block scales, FP8: the two
+ * float[2] scale / amax pairs travel with the codes).  A tensor shared by several problems
  * (q/k/v read one X) is uploaded once per problem. */
 forge_status_t forge_wgrad_adamw_grouped_host(const forge_problem_t *problems, int32_t count, int64_t step, float lr,
                                              float beta1, float beta2, float eps, float wd,

@@ -151,12 +151,12 @@ int env_int(const char *name, int dflt) {
 // launch of one fused-kernel instantiation over <= kMaxProblems problems
 // ---------------------------------------------------------------------------------------------
 template <int MDT, int MODE, int BK, int ST, int SS, int CG = 1, int CM = 64, int CN = 64, int P1C = 128, int P1S = 2,
-          int NST = 2>
+          int NST = 2, int NWG = 2>
 forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamWScalars &hp,
                             const DeviceInfo &dev, cudaStream_t stream, const FamilyScalars *fs = nullptr,
                             uint64_t sr_seed = 0, uint32_t sr_step = 0, uint32_t sr_stream0 = 0) {
-    using Cfg = KernelCfg<MDT, BK, ST, SS, CG, CM, CN, P1C, P1S, NST, (MODE == MODE_ACCUM) ? 0 : 1>;
-    auto kernel = forge_fused_kernel<MDT, MODE, BK, ST, SS, CG, CM, CN, P1C, P1S, NST>;
+    using Cfg = KernelCfg<MDT, BK, ST, SS, CG, CM, CN, P1C, P1S, NST, (MODE == MODE_ACCUM) ? 0 : 1, NWG>;
+    auto kernel = forge_fused_kernel<MDT, MODE, BK, ST, SS, CG, CM, CN, P1C, P1S, NST, NWG>;
     // the opt-in shared-memory size is a per-device function attribute: set it once per device, not once per process
     static std::atomic<uint64_t> attr_done{0};
     const uint64_t dev_bit = 1ull << (dev.device & 63);
@@ -219,7 +219,7 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
     if (grid > tiles) grid = tiles;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(grid * CG));
-    cfg.blockDim = dim3(block_threads(MDT));
+    cfg.blockDim = dim3(block_threads(MDT, NWG));
     cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
@@ -269,6 +269,14 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
         case 10: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 2, 2, 64, 64>(probs, count, hp, dev, stream);
         case 12: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 4, 4, 2, 64, 32>(probs, count, hp, dev, stream);
         case 13: return launch_fused<MDT_FP32, MODE_ADAMW, 128, 2, 2, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 15: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 2, 2, 64, 128, 128, 2, 2, 4>(probs, count, hp, dev, stream);
+        case 16: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 2, 2, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 17: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 3, 2, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 18: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 3, 2, 2, 64, 128>(probs, count, hp, dev, stream);
+        case 19: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 2, 2, 2, 64, 128>(probs, count, hp, dev, stream);
+        case 20: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 2, 2, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 21: return launch_fused<MDT_FP32, MODE_ADAMW, 16, 6, 2, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 22: return launch_fused<MDT_FP32, MODE_ADAMW, 16, 4, 2, 2, 128, 64>(probs, count, hp, dev, stream);
         default: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 2, 2, 64, 128>(probs, count, hp, dev, stream);
         }
     case FORGE_MOMENT_BF16:
@@ -285,6 +293,10 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
         case 11: return launch_fused<MDT_BF16, MODE_ADAMW, 64, 3, 4, 2, 64, 64>(probs, count, hp, dev, stream);
         case 12: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 6, 4, 2, 64, 64>(probs, count, hp, dev, stream);
         case 9: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 2, 8, 2, 32, 128>(probs, count, hp, dev, stream);
+        case 13: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 2, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 14: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 3, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 15: return launch_fused<MDT_BF16, MODE_ADAMW, 64, 4, 2, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 16: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 2, 2, 2, 128, 128>(probs, count, hp, dev, stream);
         default: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
         }
     case FORGE_MOMENT_INT8:
@@ -297,7 +309,17 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
         case 8: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 5, 2, 2, 128, 64>(probs, count, hp, dev, stream);
         case 6: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 2, 2, 128, 64, 64, 4>(probs, count, hp, dev, stream);
         case 7: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 4, 2, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
-        default: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 2, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 9: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 3, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
+        case 10: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 4, 3, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
+        case 11: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 3, 2, 128, 64, 64, 4>(probs, count, hp, dev, stream);
+        case 13: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 5, 3, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
+        case 14: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 6, 2, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
+        case 15: return launch_fused<MDT_INT8, MODE_ADAMW, 64, 3, 2, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
+        case 16: return launch_fused<MDT_INT8, MODE_ADAMW, 64, 2, 3, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
+        case 17: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 2, 2, 128, 64>(probs, count, hp, dev, stream);
+        // measured (us / layer): 3 state slots + 80 KB operand ring + 64-column first-pass chunks 420; 3 slots + 48 KB ring 437;
+        // 2 slots 457-489 whatever the operand ring; 4 slots + 48 KB ring 442 (profiles/r01_summary.md)
+        default: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 5, 3, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
         }
     case FORGE_MOMENT_FP8:
         switch (variant) {
@@ -312,6 +334,9 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
         case 10: return launch_fused<MDT_FP8, MODE_ADAMW, 32, 6, 6, 2, 64, 64>(probs, count, hp, dev, stream);
         case 11: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 4, 2, 64, 128>(probs, count, hp, dev, stream);
         case 12: return launch_fused<MDT_FP8, MODE_ADAMW, 32, 4, 6, 2, 64, 64>(probs, count, hp, dev, stream);
+        case 13: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 4, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 14: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 2, 2, 128, 128>(probs, count, hp, dev, stream);
+        case 15: return launch_fused<MDT_FP8, MODE_ADAMW, 32, 4, 4, 2, 128, 64>(probs, count, hp, dev, stream);
         // 8 B/element of state: the T = 512 mainloop needs the deeper operand ring (96 KB) more than the state ring does
         default: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 4, 2, 64, 128>(probs, count, hp, dev, stream);
         }
@@ -737,7 +762,7 @@ forge_status_t forge_wgrad_adamw_grouped_host(const forge_problem_t *problems, i
     if (!problems) return FORGE_ERR_NULL_PTR;
     if (count < 1) return FORGE_ERR_BAD_SHAPE;
     const int mdt = static_cast<int>(moment_dtype);
-    if (mdt < 0 || mdt > 2) return FORGE_ERR_BAD_DTYPE;
+    if (mdt < 0 || mdt > 3) return FORGE_ERR_BAD_DTYPE;
     forge_status_t s = validate_hp(step, lr, beta1, beta2, eps, wd);
     if (s != FORGE_OK) return s;
     for (int i = 0; i < count; ++i) {
@@ -755,7 +780,7 @@ forge_status_t forge_wgrad_adamw_grouped_host(const forge_problem_t *problems, i
         const forge_problem_t &p = problems[i];
         const size_t n = static_cast<size_t>(p.out) * p.in;
         sz[i] = {static_cast<size_t>(p.T) * p.in * 2, static_cast<size_t>(p.T) * p.out * 2, n * 2, n * mom,
-                 mdt == FORGE_MOMENT_INT8 ? n / FORGE_QBLOCK * 4 : 0, total};
+                 mdt == FORGE_MOMENT_INT8 ? n / FORGE_QBLOCK * 4 : (mdt == FORGE_MOMENT_FP8 ? 2 * sizeof(float) : 0), total};
         total += up(sz[i].bX) + up(sz[i].bY) + up(sz[i].bW) + 2 * up(sz[i].bM) + 2 * up(sz[i].bS);
     }
     uint8_t *d = nullptr;

@@ -43,8 +43,9 @@ constexpr int kCtrlWarps = 4;
 #endif
 // int8: warps per TMEM quadrant sharing a row (2 = the two warpgroups; 3 measured slower: 485 vs 461 us/layer)
 constexpr int kI8W = FORGE_INT8_WARPS_PER_QUAD;
-__host__ __device__ constexpr int epi_warps(int mdt) { return mdt == 2 /*MDT_INT8*/ ? 4 * kI8W : 8; }
-__host__ __device__ constexpr int block_threads(int mdt) { return (kCtrlWarps + epi_warps(mdt)) * 32; }
+// nwg = epilogue warpgroups of the floating-point paths (2, or 4 when a chunk has four 32-column sub-blocks)
+__host__ __device__ constexpr int epi_warps(int mdt, int nwg = 2) { return mdt == 2 /*MDT_INT8*/ ? 4 * kI8W : 4 * nwg; }
+__host__ __device__ constexpr int block_threads(int mdt, int nwg = 2) { return (kCtrlWarps + epi_warps(mdt, nwg)) * 32; }
 // L2 eviction priority of the state stream (W, m, v loads and the in-place stores).  Measured on the cfg-1 layer:
 // evict_first for both 762 us, normal for both 729 us (fp32 moments; bf16 484 -> 459 us): the store that follows
 // the load of the same lines a few microseconds later should still find them in L2.
@@ -95,8 +96,9 @@ enum : int { DBG_NO_MAINLOOP = 1, DBG_NO_STATE = 2, DBG_NO_EPILOGUE = 4 };
 // and 64 x 128 x 2 slots 0.90 (profiles/r01_summary.md) -- longer contiguous runs per DRAM page and
 // fewer pages open at once matter more than bytes in flight.
 template <int MDT, int kBlockK, int kStages, int kStateStages, int CG = 1, int CM_ = 64, int CN_ = 64, int P1C_ = 128, int P1S_ = 2,
-          int NST_ = 2, int HASW_ = 1>
+          int NST_ = 2, int HASW_ = 1, int NWG_ = 2>
 struct KernelCfg {
+    static constexpr int NWG = NWG_;                        // epilogue warpgroups (fp paths)
     static constexpr int HASW = HASW_;                      // the chunk image carries W (not in MODE_ACCUM)
     static constexpr int NST = NST_;                        // state tensors besides W in a chunk (AdamW: m, v)
     static constexpr int kMomBytes = (MDT == MDT_FP32) ? 4 : (MDT == MDT_BF16 ? 2 : 1);   // int8 and fp8: 1
@@ -107,7 +109,8 @@ struct KernelCfg {
     static constexpr int CM = CM_, CN = CN_;
     static constexpr int RB = BLOCK_M / CM, CB = BLOCK_N / CN, CHUNKS = RB * CB;
     static constexpr int SUBS = CN / SUB;                   // 32-column sub-blocks per chunk row
-    static constexpr int WGS = SUBS >= 2 ? 2 : 1;           // warpgroups that share one chunk
+    static constexpr int WGS = SUBS >= NWG ? NWG : (SUBS >= 2 ? 2 : 1);   // warpgroups that share one chunk
+    static_assert(NWG == 2 || (NWG == 4 && SUBS >= 4 && MDT != MDT_INT8), "four epilogue warpgroups need four sub-blocks per chunk row");
     // chunks ci and ci + PERIOD are consumed by the same warps
     static constexpr int PERIOD = RB * (SUBS >= 2 ? 1 : 2);
     static constexpr int DONE_COUNT = (CM / SUB) * (MDT == MDT_INT8 ? kI8W : WGS) * 32;
@@ -574,11 +577,11 @@ __device__ __forceinline__ void int8_loader(const KernelParams &P, uint32_t rank
 // ---------------------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------------------
-template <int MDT, int MODE, int kBlockK, int kStages, int kStateStages, int CG, int CM, int CN, int P1C, int P1S, int NST>
-__global__ void __launch_bounds__(block_threads(MDT), 1)
+template <int MDT, int MODE, int kBlockK, int kStages, int kStateStages, int CG, int CM, int CN, int P1C, int P1S, int NST, int NWG>
+__global__ void __launch_bounds__(block_threads(MDT, NWG), 1)
 forge_fused_kernel(const __grid_constant__ KernelParams P) {
     constexpr int HASW = (MODE == MODE_ACCUM) ? 0 : 1;
-    using Cfg = KernelCfg<MDT, kBlockK, kStages, kStateStages, CG, CM, CN, P1C, P1S, NST, HASW>;
+    using Cfg = KernelCfg<MDT, kBlockK, kStages, kStateStages, CG, CM, CN, P1C, P1S, NST, HASW, NWG>;
     static_assert(MODE != MODE_ADAMW_SR || (MDT != MDT_INT8 && MDT != MDT_FP8), "the SR store is implemented for fp32 / bf16 moments");
     static_assert(MDT != MDT_FP8 || MODE == MODE_ADAMW, "fp8 moments are implemented for AdamW");
     static_assert(MODE == MODE_FAMILY || MODE == MODE_ACCUM || NST == 2, "AdamW and the store-G twin use the two-state chunk image");
@@ -615,7 +618,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         }
         for (int i = 0; i < 2; ++i) {
             mbar_init(bar_tm_full + 8 * i, 1);
-            mbar_init(bar_tm_empty + 8 * i, epi_warps(MDT) * CG);   // one arrival per epilogue warp of the pair
+            mbar_init(bar_tm_empty + 8 * i, epi_warps(MDT, NWG) * CG);   // one arrival per epilogue warp of the pair
         }
         for (int i = 0; i < kStateStages; ++i) {
             mbar_init(bar_st_full + 8 * i, 1);
@@ -624,7 +627,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         }
         for (int i = 0; i < Cfg::P1_STAGES; ++i) {
             mbar_init(bar_p1_full + 8 * i, 1);
-            mbar_init(bar_p1_empty + 8 * i, epi_warps(MDT) * 32);     // every epilogue thread reads its part of the chunk
+            mbar_init(bar_p1_empty + 8 * i, epi_warps(MDT, NWG) * 32);     // every epilogue thread reads its part of the chunk
         }
         mbar_fence_init();
     }
@@ -806,7 +809,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
     } else {
         // ================= epilogue warpgroups (Alg. 1 lines 7-10 on the TMEM tile) ==============
         const int ew = warp - kCtrlWarps;
-        const int wg = ew >> 2;                       // warpgroup 0/1
+        const int wg = ew >> 2;                       // warpgroup 0 .. NWG-1
         const uint32_t quad = warp & 3;               // TMEM lane quadrant this warp may read
         const uint32_t row_t = quad * 32 + lane;      // row of the tile == TMEM lane
         const uint32_t rb = row_t / CM, row = row_t % CM;   // this warp's row block, row inside the chunk

@@ -370,3 +370,25 @@ def test_every_mode_is_bitwise_repeatable_on_a_ragged_group(mode):
             ref = snap
         else:
             assert all(torch.equal(x, y) for a, b in zip(ref, snap) for x, y in zip(a, b)), mode
+
+
+def test_grouped_host_entry_fp8_matches_device_path_bitwise():
+    """forge_wgrad_adamw_grouped_host with FP8 moments: codes, W and both scale / amax pairs equal the device-resident call."""
+    hp = synth.HP_DEFAULT
+    hpt = (hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
+    ps = [synth.make_problem("a", 200, 136, 272, 71), synth.make_problem("b", 96, 256, 512, 72)]
+    host, devs = [], []
+    for p in ps:
+        mq, ms = fo.fp8_quantize(p.m.numpy())
+        vq, vs = fo.fp8_quantize(p.v.numpy())
+        t = dict(X=p.X, dY=p.dY, W=p.W.clone(), m=torch.from_numpy(mq.copy()), v=torch.from_numpy(vq.copy()),
+                 m_scale=torch.from_numpy(ms.copy()), v_scale=torch.from_numpy(vs.copy()))
+        host.append({k: x.clone().pin_memory() for k, x in t.items()})
+        devs.append({k: x.to(DEV).clone() for k, x in t.items()})
+    fb.forge_wgrad_adamw_grouped_host(host, 10, *hpt, fb.FP8)
+    fb.forge_wgrad_adamw_grouped(devs, 10, *hpt, fb.FP8)
+    torch.cuda.synchronize()
+    for h, d, p in zip(host, devs, ps):
+        for k in ("W", "m", "v", "m_scale", "v_scale"):
+            assert torch.equal(h[k], d[k].cpu()), k
+        assert not torch.equal(h["W"], p.W) and float(h["m_scale"][1]) > 0.0
