@@ -202,6 +202,9 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
         if (!ok) return cuda_fail(cudaErrorInvalidValue);
         d.m_scale = p.m_scale;
         d.v_scale = p.v_scale;
+        d.pW = static_cast<char *>(p.W);
+        d.pM = static_cast<char *>(p.m);
+        d.pV = static_cast<char *>(p.v);
         d.T = p.T;
         d.out = p.out;
         d.in = p.in;
@@ -244,14 +247,27 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
 // FORGE_CFG selects the other instantiations for tuning sweeps and the determinism tests only.
 int pick_variant(int maxT) {
     const int forced = env_int("FORGE_CFG", -1);   // debug only
-    return forced >= 0 ? forced : (maxT > 1024 ? 5 : 0);
+    // T >= 4096 (fp32 / bf16 moments): the ring-less direct state path, all shared memory to the operand ring
+    return forced >= 0 ? forced : (maxT >= 4096 ? 30 : (maxT > 1024 ? 5 : 0));
+}
+
+// The direct state path (variants >= 30) moves 16 columns per thread with 32-byte accesses: every row must be a
+// whole number of such vectors and every base 32-byte aligned; anything else takes the TMA ring.
+bool direct_ok(const forge_problem_t *probs, int count) {
+    for (int i = 0; i < count; ++i) {
+        const forge_problem_t &p = probs[i];
+        const uintptr_t bits = reinterpret_cast<uintptr_t>(p.W) | reinterpret_cast<uintptr_t>(p.m) | reinterpret_cast<uintptr_t>(p.v);
+        if (p.in % 16 != 0 || bits % 32 != 0) return false;
+    }
+    return true;
 }
 
 forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, const AdamWScalars &hp,
                               const DeviceInfo &dev, cudaStream_t stream) {
     int maxT = 0;
     for (int i = 0; i < count; ++i) maxT = probs[i].T > maxT ? probs[i].T : maxT;
-    const int variant = pick_variant(maxT);
+    int variant = pick_variant(maxT);
+    if (variant >= 30 && (!direct_ok(probs, count) || mdt > FORGE_MOMENT_BF16)) variant = maxT > 1024 ? 5 : 0;
     switch (mdt) {
     case FORGE_MOMENT_FP32:
         switch (variant) {
@@ -270,6 +286,12 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
         case 12: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 4, 4, 2, 64, 32>(probs, count, hp, dev, stream);
         case 13: return launch_fused<MDT_FP32, MODE_ADAMW, 128, 2, 2, 2, 64, 64>(probs, count, hp, dev, stream);
         case 15: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 2, 2, 64, 128, 128, 2, 2, 4>(probs, count, hp, dev, stream);
+        case 30: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 6, 0, 2, 64, 128>(probs, count, hp, dev, stream);
+        case 31: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 4, 0, 2, 64, 128>(probs, count, hp, dev, stream);
+        case 32: return launch_fused<MDT_FP32, MODE_ADAMW, 128, 3, 0, 2, 64, 128>(probs, count, hp, dev, stream);
+        case 33: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 7, 0, 2, 64, 128>(probs, count, hp, dev, stream);
+        case 34: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 12, 0, 2, 64, 128>(probs, count, hp, dev, stream);
+        case 35: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 5, 0, 2, 64, 128>(probs, count, hp, dev, stream);
         case 16: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 2, 2, 2, 128, 64>(probs, count, hp, dev, stream);
         case 17: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 3, 2, 2, 128, 64>(probs, count, hp, dev, stream);
         case 18: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 3, 2, 2, 64, 128>(probs, count, hp, dev, stream);
@@ -294,6 +316,7 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
         case 12: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 6, 4, 2, 64, 64>(probs, count, hp, dev, stream);
         case 9: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 2, 8, 2, 32, 128>(probs, count, hp, dev, stream);
         case 13: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 2, 2, 128, 64>(probs, count, hp, dev, stream);
+        case 30: return launch_fused<MDT_BF16, MODE_ADAMW, 64, 6, 0, 2, 64, 64>(probs, count, hp, dev, stream);
         case 14: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 3, 2, 128, 64>(probs, count, hp, dev, stream);
         case 15: return launch_fused<MDT_BF16, MODE_ADAMW, 64, 4, 2, 2, 128, 64>(probs, count, hp, dev, stream);
         case 16: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 2, 2, 2, 128, 128>(probs, count, hp, dev, stream);

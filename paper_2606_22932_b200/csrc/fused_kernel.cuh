@@ -71,6 +71,7 @@ struct alignas(64) ProblemDesc {
     int32_t tiles_n;     // ceil(in / 256)
     int32_t tile_begin;  // first linear tile index of this problem
     uint32_t sr_inner;   // MODE_ADAMW_SR: fmix32(seed_hi ^ step ^ stream) of this problem
+    char *pW, *pM, *pV;  // raw bases of W, m, v: the direct (ring-less) state path only
 };
 
 struct alignas(64) KernelParams {
@@ -240,6 +241,57 @@ __device__ __forceinline__ void epi_sub_fp(const AdamWScalars &hp, const uint32_
 struct Fp8Row {
     float bm, bv, inv_m, inv_v;    // beta * scale (dequantisation folded into the moment update), 1 / scale
 };
+// Direct state path (kStateStages == 0, tensor-bound shapes).  At large T the mainloop's operand traffic alone
+// takes most of the shared-memory bandwidth (per MMA of 128 clocks each SM reads 8 KB of operands and TMA writes
+// 8 KB), and the state ring adds four more passes over 20 B/element (TMA in, ld.shared, st.shared, TMA out):
+// measured at T = 8192 the ring costs 114 us on a 650 us mainloop.  Here each thread owns one row of the tile and
+// moves its 16 columns per step with 32-byte global accesses, registers only; step s + 1 is loaded before step s
+// is computed.  Same arithmetic and rounding as epi_sub_fp.
+template <int MDT>
+struct DirectRegs {
+    static constexpr int MV = (MDT == MDT_FP32) ? 2 : 1;   // 32-byte vectors of m (and of v) per 16 columns
+    uint32_t w[8], m[MV][8], v[MV][8];
+};
+template <int MDT>
+__device__ __forceinline__ void direct_load(DirectRegs<MDT> &r, const char *Wp, const char *Mp, const char *Vp) {
+    ldg256(Wp, r.w);
+#pragma unroll
+    for (int i = 0; i < DirectRegs<MDT>::MV; ++i) {
+        ldg256(Mp + 32 * i, r.m[i]);
+        ldg256(Vp + 32 * i, r.v[i]);
+    }
+}
+template <int MDT>
+__device__ __forceinline__ void direct_step(const AdamWScalars &hp, const uint32_t (&g)[16], DirectRegs<MDT> &r,
+                                            char *Wp, char *Mp, char *Vp) {
+#pragma unroll
+    for (int e = 0; e < 8; ++e) {               // coordinate pairs (2e, 2e + 1)
+        f32x2 w = bf16x2_to_f32x2(r.w[e]), m, v;
+        if constexpr (MDT == MDT_FP32) {
+            m = pk2u(r.m[e / 4][(2 * e) % 8], r.m[e / 4][(2 * e) % 8 + 1]);
+            v = pk2u(r.v[e / 4][(2 * e) % 8], r.v[e / 4][(2 * e) % 8 + 1]);
+        } else {
+            m = bf16x2_to_f32x2(r.m[0][e]);
+            v = bf16x2_to_f32x2(r.v[0][e]);
+        }
+        adamw_update2(hp, pk2u(g[2 * e], g[2 * e + 1]), w, m, v);
+        r.w[e] = f32x2_to_bf16x2(w);
+        if constexpr (MDT == MDT_FP32) {
+            r.m[e / 4][(2 * e) % 8] = lo2u(m); r.m[e / 4][(2 * e) % 8 + 1] = hi2u(m);
+            r.v[e / 4][(2 * e) % 8] = lo2u(v); r.v[e / 4][(2 * e) % 8 + 1] = hi2u(v);
+        } else {
+            r.m[0][e] = f32x2_to_bf16x2(m);
+            r.v[0][e] = f32x2_to_bf16x2(v);
+        }
+    }
+    stg256(Wp, r.w);
+#pragma unroll
+    for (int i = 0; i < DirectRegs<MDT>::MV; ++i) {
+        stg256(Mp + 32 * i, r.m[i]);
+        stg256(Vp + 32 * i, r.v[i]);
+    }
+}
+
 template <class Cfg>
 __device__ __forceinline__ void epi_sub_fp8(const AdamWScalars &hp, const Fp8Row &R, const uint32_t (&g)[32],
                                             const SubAddr<Cfg> &a, uint32_t row, float &pm, float &pv) {
@@ -588,6 +640,9 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
     static_assert(MODE != MODE_ACCUM || NST == 1, "accumulate-into-state has exactly one state tensor");
     static_assert((MODE != MODE_FAMILY && MODE != MODE_ACCUM) || MDT != MDT_INT8, "int8 state is implemented for AdamW only");
     constexpr int CHUNKS = Cfg::CHUNKS;
+    constexpr bool DIRECT = (kStateStages == 0);      // no state ring: the epilogue moves W, m, v itself (direct_step)
+    constexpr uint32_t SSN = DIRECT ? 1 : kStateStages;
+    static_assert(!DIRECT || (MODE == MODE_ADAMW && (MDT == MDT_FP32 || MDT == MDT_BF16)), "the direct state path is AdamW, fp32 / bf16 moments");
     const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;   // rank 0 = the pair's leader
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -723,13 +778,13 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         if constexpr (MDT == MDT_INT8) {
             if (lane == 0 && !(P.debug & DBG_NO_STATE))
                 int8_loader<Cfg, kStateStages, CG>(P, rank, first_tile, tile_step, sST, bar_st_full, bar_st_empty, i8);
-        } else if (MODE != MODE_STORE_G && lane == 0 && !(P.debug & DBG_NO_STATE)) {
+        } else if (!DIRECT && MODE != MODE_STORE_G && lane == 0 && !(P.debug & DBG_NO_STATE)) {
             uint32_t ci = 0;  // running chunk counter
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step) {
                 const TileCoord tc = decode_tile<CG>(P, tile, rank);
                 const ProblemDesc &pd = P.prob[tc.p];
                 for (int c = 0; c < CHUNKS; ++c, ++ci) {
-                    const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
+                    const uint32_t s = ci % SSN, ph = (ci / SSN) & 1u;
                     mbar_wait(bar_st_empty + 8 * s, ph ^ 1u);
                     const uint32_t full = bar_st_full + 8 * s;
                     mbar_expect_tx(full, Cfg::ST_TX_BYTES);
@@ -756,7 +811,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         }
     } else if (warp == 3) {
         // ================= state storer (Alg. 1 line 11: store W_ij, m_ij, v_ij) ================
-        if (lane == 0) {
+        if (!DIRECT && lane == 0) {
             // One store group may stay in flight while the next chunk is stored (look-ahead 1): the
             // ~0.8 us a TMA store needs before its shared-memory source is reusable is then hidden
             // behind the next chunk instead of serialising the ring.  A slot is released as soon as
@@ -767,7 +822,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                 const TileCoord tc = decode_tile<CG>(P, tile, rank);
                 const ProblemDesc &pd = P.prob[tc.p];
                 for (int c = 0; c < CHUNKS; ++c, ++ci) {
-                    const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
+                    const uint32_t s = ci % SSN, ph = (ci / SSN) & 1u;
                     if (held >= 0 && !mbar_test_wait(bar_st_done + 8 * s, ph)) {
                         tma_store_wait_read<0>();
                         mbar_arrive(bar_st_empty + 8 * held);
@@ -837,11 +892,35 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                 f8.inv_m = fp8_inv_scale(sm);
                 f8.inv_v = fp8_inv_scale(sv);
             }
-            if constexpr (MDT != MDT_INT8) {
+            if constexpr (DIRECT) {
+                // each warpgroup takes one 128-column half of the tile, each thread its row, 16 columns per step
+                const TileCoord tc = decode_tile<CG>(P, tile, rank);
+                const ProblemDesc &pd = P.prob[tc.p];
+                constexpr int MB = Cfg::kMomBytes;
+                const int grow = tc.tm * BLOCK_M + static_cast<int>(row_t);
+                const int col0 = tc.tn * BLOCK_N + wg * (BLOCK_N / 2);
+                const bool row_ok = grow < pd.out && !(P.debug & DBG_NO_STATE);
+                const size_t e0 = static_cast<size_t>(row_ok ? grow : 0) * pd.in + col0;
+                char *Wp = pd.pW + e0 * 2, *Mp = pd.pM + e0 * MB, *Vp = pd.pV + e0 * MB;
+                constexpr int STEPS = BLOCK_N / 2 / 16;
+                DirectRegs<MDT> R[2];
+                if (row_ok && col0 < pd.in) direct_load<MDT>(R[0], Wp, Mp, Vp);
+#pragma unroll
+                for (int st = 0; st < STEPS; ++st) {
+                    uint32_t g[16];
+                    tmem_ld_32x32b_x16(taddr + wg * (BLOCK_N / 2) + st * 16, g);
+                    const bool ok = row_ok && col0 + st * 16 < pd.in;
+                    if (st + 1 < STEPS && row_ok && col0 + (st + 1) * 16 < pd.in)
+                        direct_load<MDT>(R[(st + 1) & 1], Wp + (st + 1) * 32, Mp + (st + 1) * 16 * MB, Vp + (st + 1) * 16 * MB);
+                    tmem_ld_wait();
+                    if (ok && !(P.debug & DBG_NO_EPILOGUE))
+                        direct_step<MDT>(hp, g, R[st & 1], Wp + st * 32, Mp + st * 16 * MB, Vp + st * 16 * MB);
+                }
+            } else if constexpr (MDT != MDT_INT8) {
                 for (int cb = 0; cb < Cfg::CB; ++cb) {
                     if (Cfg::SUBS < 2 && (cb & 1) != wg) continue;
                     const uint32_t ci = titer * CHUNKS + cb * Cfg::RB + rb;
-                    const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
+                    const uint32_t s = ci % SSN, ph = (ci / SSN) & 1u;
                     const uint32_t base = sST + s * Cfg::ST_STAGE;
                     if (MODE != MODE_STORE_G && !(P.debug & DBG_NO_STATE)) mbar_wait(bar_st_full + 8 * s, ph);
                     else mbar_wait(bar_st_empty + 8 * s, ph ^ 1u);

@@ -183,6 +183,25 @@ def test_fused_equals_store_g_twin_plus_same_update_bitwise(moment, T):
         assert torch.equal(d1[k].view(torch.uint8), d2[k].view(torch.uint8)), f"{moment}: {k} differs from the unfused twin"
 
 
+@pytest.mark.parametrize("moment", ["fp32", "bf16"])
+@pytest.mark.parametrize("out,inn", [(640, 768), (600, 528), (200, 264)])
+def test_direct_state_path_at_large_T_equals_store_g_twin_bitwise(moment, out, inn):
+    """T >= 4096 takes the ring-less direct epilogue (32-byte global accesses, thread = row) when every row is a
+    whole number of 16-column vectors; (200, 264) is not and falls back to the TMA ring.  Ragged row blocks, several
+    column tiles; bit-identical to the store-G twin plus the same update either way."""
+    p = synth.make_problem("x", 4096, out, inn, seed=17)
+    d1, _ = gpu_state(p, moment)
+    d2 = {k: v.clone() for k, v in d1.items()}
+    fb.forge_wgrad_adamw(d1["X"], d1["dY"], d1["W"], d1["m"], d1["v"], 5, **HP)
+    G = torch.empty(out, inn, device=DEV)
+    fb.forge_wgrad_store_g(d2["X"], d2["dY"], G)
+    fb.forge_adamw_from_g(G, d2["W"], d2["m"], d2["v"], 5, **HP)
+    torch.cuda.synchronize()
+    for k in d1:
+        assert torch.equal(d1[k].view(torch.uint8), d2[k].view(torch.uint8)), f"{moment}: {k} differs from the unfused twin"
+    assert not torch.equal(d1["W"], p.W.to(DEV))
+
+
 def test_store_g_matches_oracle_gradient():
     p = synth.make_problem("x", 300, 264, 520, seed=9)
     G = torch.empty(264, 520, device=DEV)
