@@ -8,7 +8,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB_PATH = os.path.join(_HERE, "libforge_b200.so")
 SOURCES = ["forge_api.cu"]
-HEADERS = ["fused_kernel.cuh", "elementwise_kernel.cuh", "adamw_math.cuh", "ptx.cuh"]
+HEADERS = ["fused_kernel.cuh", "elementwise_kernel.cuh", "adamw_math.cuh", "family_math.cuh", "ptx.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--compiler-options", "-fPIC", "-shared", "-lcublas"]
 
