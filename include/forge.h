@@ -77,7 +77,10 @@ typedef enum {
 /* CUDA stream handle; identical to cudaStream_t / CUstream.  NULL is the legacy default stream. */
 typedef struct CUstream_st *forge_stream_t;
 
-/* One linear layer's problem.  Layouts are row-major and dense (leading dimension = row length):
+/* One linear layer's problem.  Layouts are row-major; the state tensors are dense (leading dimension = row
+ * length), the two operands may be strided views -- the q / k / v slices of one fused-QKV output gradient, the gate /
+ * up halves of a fused MLP projection -- through ldx / lddy (row pitch in ELEMENTS; 0 means dense; otherwise
+ * >= the row length and a multiple of 8, else FORGE_ERR_BAD_SHAPE; the host-buffer entries take dense operands only):
  *   X  [T, in]   bf16, read only          dY [T, out]  bf16, read only
  *   W  [out, in] bf16, updated in place   m, v [out, in] in the moment dtype, updated in place
  *   m_scale, v_scale [out, in/256] fp32, INT8 mode only (must be NULL otherwise), in place.
@@ -92,6 +95,7 @@ typedef struct {
     float *m_scale;
     float *v_scale;
     int32_t T, out, in;
+    int64_t ldx, lddy;
 } forge_problem_t;
 
 /* Fused weight gradient + AdamW step for one layer (Algorithm 1).

@@ -36,7 +36,7 @@ class ForgeError(RuntimeError):
 class forge_problem_t(ctypes.Structure):
     _fields_ = [("X", c_void_p), ("dY", c_void_p), ("W", c_void_p), ("m", c_void_p), ("v", c_void_p),
                 ("m_scale", c_void_p), ("v_scale", c_void_p),
-                ("T", c_int32), ("out", c_int32), ("in_", c_int32)]
+                ("T", c_int32), ("out", c_int32), ("in_", c_int32), ("ldx", c_int64), ("lddy", c_int64)]
 
 
 class forge_opt_desc_t(ctypes.Structure):
@@ -141,6 +141,12 @@ def make_problem_array(problems):
         arr[i].v_scale = None if vs is None else vs.data_ptr()
         arr[i].T, arr[i].in_ = X.shape
         arr[i].out = dY.shape[1]
+        # operands may be column slices of a wider tensor (fused QKV / gate-up): row pitch in elements, 0 = dense
+        for t, name in ((X, "X"), (dY, "dY")):
+            if t.dim() != 2 or (t.shape[1] > 1 and t.stride(1) != 1):
+                raise ValueError(f"{name} must be a 2-D tensor with unit column stride")
+        arr[i].ldx = 0 if X.is_contiguous() else X.stride(0)
+        arr[i].lddy = 0 if dY.is_contiguous() else dY.stride(0)
     return arr
 
 

@@ -51,11 +51,11 @@ EncodeTiledFn get_encode_fn() {
 
 // 2D row-major tensor [rows, cols] of `esize`-byte elements; box {box_cols, box_rows}.
 bool encode_2d(CUtensorMap *map, CUtensorMapDataType dt, int esize, const void *base, uint64_t rows,
-               uint64_t cols, uint32_t box_cols, uint32_t box_rows, CUtensorMapSwizzle swz) {
+               uint64_t cols, uint32_t box_cols, uint32_t box_rows, CUtensorMapSwizzle swz, uint64_t pitch_elems = 0) {
     EncodeTiledFn fn = get_encode_fn();
     if (!fn) return false;
     cuuint64_t dims[2] = {cols, rows};
-    cuuint64_t strides[1] = {cols * static_cast<uint64_t>(esize)};
+    cuuint64_t strides[1] = {(pitch_elems ? pitch_elems : cols) * static_cast<uint64_t>(esize)};
     cuuint32_t box[2] = {box_cols, box_rows};
     cuuint32_t estr[2] = {1, 1};
     CUresult r = fn(map, dt, 2, const_cast<void *>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -107,8 +107,13 @@ forge_status_t validate_problem(const forge_problem_t &p, int mdt) {
     forge_status_t s = validate_state(p.W, p.m, p.v, p.m_scale, p.v_scale, p.out, p.in, mdt);
     if (s != FORGE_OK) return s;
     if (p.T < 1) return FORGE_ERR_BAD_SHAPE;
+    if (p.ldx != 0 && (p.ldx < p.in || p.ldx % 8 != 0)) return FORGE_ERR_BAD_SHAPE;
+    if (p.lddy != 0 && (p.lddy < p.out || p.lddy % 8 != 0)) return FORGE_ERR_BAD_SHAPE;
     if (!aligned16(p.X) || !aligned16(p.dY)) return FORGE_ERR_ALIGNMENT;
     return FORGE_OK;
+}
+bool dense_operands(const forge_problem_t &p) {
+    return (p.ldx == 0 || p.ldx == p.in) && (p.lddy == 0 || p.lddy == p.out);
 }
 
 // Alg. 1 line 9 bias terms and the folded constants, computed in double from the float
@@ -179,8 +184,10 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
         const forge_problem_t &p = probs[i];
         ProblemDesc &d = P.prob[i];
         bool ok = true;
-        ok &= encode_2d(&d.map_dY, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.dY, p.T, p.out, 64, BK, CU_TENSOR_MAP_SWIZZLE_128B);
-        ok &= encode_2d(&d.map_X, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.X, p.T, p.in, 64, BK, CU_TENSOR_MAP_SWIZZLE_128B);
+        ok &= encode_2d(&d.map_dY, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.dY, p.T, p.out, 64, BK, CU_TENSOR_MAP_SWIZZLE_128B,
+                        static_cast<uint64_t>(p.lddy));
+        ok &= encode_2d(&d.map_X, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.X, p.T, p.in, 64, BK, CU_TENSOR_MAP_SWIZZLE_128B,
+                        static_cast<uint64_t>(p.ldx));
         if (MODE != MODE_STORE_G) {
             if (MODE != MODE_ACCUM)
                 ok &= encode_2d(&d.map_W, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.W, p.out, p.in, Cfg::W_BOX_COLS, CM,
@@ -521,6 +528,7 @@ forge_status_t forge_wgrad_adamw(const void *X, const void *dY, void *W, void *m
                                  float beta1, float beta2, float eps, float wd,
                                  forge_moment_dtype_t moment_dtype, forge_stream_t stream) {
     forge_problem_t p;
+    std::memset(&p, 0, sizeof(p));
     p.X = X; p.dY = dY; p.W = W; p.m = m; p.v = v; p.m_scale = m_scale; p.v_scale = v_scale;
     p.T = T; p.out = out; p.in = in;
     return forge_wgrad_adamw_grouped(&p, 1, step, lr, beta1, beta2, eps, wd, moment_dtype, stream);
@@ -666,7 +674,7 @@ forge_status_t forge_layer_backward_grouped(const forge_problem_t *problems, voi
     for (int i = 0; i < count; ++i) {
         const forge_problem_t &p = problems[i];
         cublasStatus_t cs = cublasGemmEx(handle, CUBLAS_OP_N, CUBLAS_OP_N, p.in, p.T, p.out, &one, p.W, CUDA_R_16BF, p.in,
-                                         p.dY, CUDA_R_16BF, p.out, &zero, dX[i], CUDA_R_16BF, p.in, CUBLAS_COMPUTE_32F,
+                                         p.dY, CUDA_R_16BF, p.lddy ? p.lddy : p.out, &zero, dX[i], CUDA_R_16BF, p.in, CUBLAS_COMPUTE_32F,
                                          CUBLAS_GEMM_DEFAULT);
         if (cs != CUBLAS_STATUS_SUCCESS) return cuda_fail(cudaErrorUnknown);
     }
@@ -735,6 +743,7 @@ forge_status_t forge_wgrad_adamw_host(const void *X, const void *dY, void *W, vo
     const int mdt = static_cast<int>(moment_dtype);
     if (mdt < 0 || mdt > 2) return FORGE_ERR_BAD_DTYPE;
     forge_problem_t hp_;
+    std::memset(&hp_, 0, sizeof(hp_));
     hp_.X = X; hp_.dY = dY; hp_.W = W; hp_.m = m; hp_.v = v; hp_.m_scale = m_scale; hp_.v_scale = v_scale;
     hp_.T = T; hp_.out = out; hp_.in = in;
     forge_status_t s = validate_hp(step, lr, beta1, beta2, eps, wd);
@@ -791,6 +800,7 @@ forge_status_t forge_wgrad_adamw_grouped_host(const forge_problem_t *problems, i
     for (int i = 0; i < count; ++i) {
         s = validate_problem(problems[i], mdt);
         if (s != FORGE_OK) return s;
+        if (!dense_operands(problems[i])) return FORGE_ERR_BAD_SHAPE;   // host buffers are copied as dense blocks
     }
     const size_t mom = mdt == FORGE_MOMENT_FP32 ? 4 : (mdt == FORGE_MOMENT_BF16 ? 2 : 1);
     auto up = [](size_t b) { return (b + 255) / 256 * 256; };

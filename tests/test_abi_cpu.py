@@ -41,9 +41,10 @@ def test_version_strings_workspace(lib):
 
 
 def test_struct_layout_matches_header():
-    # 7 pointers + 3 int32, padded to pointer alignment
-    assert ctypes.sizeof(fb.forge_problem_t) == 7 * 8 + 16
+    # 7 pointers + 3 int32 padded to 8 + the two operand pitches (ldx, lddy)
+    assert ctypes.sizeof(fb.forge_problem_t) == 7 * 8 + 16 + 16
     assert fb.forge_problem_t.T.offset == 56 and fb.forge_problem_t.in_.offset == 64
+    assert fb.forge_problem_t.ldx.offset == 72 and fb.forge_problem_t.lddy.offset == 80
 
 
 def _call(lib, X=0x1000, dY=0x2000, W=0x3000, m=0x4000, v=0x5000, ms=None, vs=None, T=128, out=384, inn=256,
@@ -79,6 +80,14 @@ def test_argument_validation_happens_before_any_cuda_call(lib):
     assert lib.forge_wgrad_adamw_grouped(arr, 0, *HP, 0, None) == BAD_SHAPE
     arr[1].out = 7
     assert lib.forge_wgrad_adamw_grouped(arr, 2, *HP, 0, None) == BAD_SHAPE
+    # operand pitches: 0 = dense; otherwise >= the row length and a multiple of 8 elements
+    arr[1].out = 384
+    for ldx, lddy in ((255, 0), (260, 0), (0, 380), (0, 388)):
+        arr[1].ldx, arr[1].lddy = ldx, lddy
+        assert lib.forge_wgrad_adamw_grouped(arr, 2, *HP, 0, None) == BAD_SHAPE
+    arr[1].ldx, arr[1].lddy = 512, 1152                       # valid strided views are refused by the host-buffer entry only
+    assert lib.forge_wgrad_adamw_grouped_host(arr, 2, *HP, 0) == BAD_SHAPE
+    arr[1].ldx, arr[1].lddy = 0, 0
     # test-only twins validate too
     assert lib.forge_wgrad_store_g(None, 0x2000, 0x3000, 128, 384, 256, None) == NULL_PTR
     assert lib.forge_adamw_from_g(None, 0x3000, 0x4000, 0x5000, None, None, 384, 256, *HP, 0, None) == NULL_PTR

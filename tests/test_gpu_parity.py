@@ -202,6 +202,37 @@ def test_direct_state_path_at_large_T_equals_store_g_twin_bitwise(moment, out, i
     assert not torch.equal(d1["W"], p.W.to(DEV))
 
 
+@pytest.mark.parametrize("moment", ["fp32", "int8"])
+def test_strided_operand_views_fused_qkv_bitwise_and_dgrad(moment):
+    """ldx / lddy (include/forge.h): q, k, v read column slices of ONE fused dY[T, 512+256+256] and a column slice of a
+    wider X; the result must be bit-identical to the same call on dense copies of the slices, and the dgrad of
+    forge_layer_backward_grouped must read the strided dY too."""
+    T, inn, outs = 200, 512, (512, 256, 256)
+    wide_x = torch.randn(T, inn + 64, generator=torch.Generator().manual_seed(5)).to(torch.bfloat16).to(DEV)
+    fused_dy = (torch.randn(T, sum(outs), generator=torch.Generator().manual_seed(6)) * 1e-2).to(torch.bfloat16).to(DEV)
+    X = wide_x[:, 32:32 + inn]
+    views, dense, c0 = [], [], 0
+    for i, o in enumerate(outs):
+        p = synth.make_problem(f"p{i}", T, o, inn, seed=30 + i)
+        d, _ = gpu_state(p, moment)
+        dY = fused_dy[:, c0:c0 + o]
+        c0 += o
+        views.append(dict(d, X=X, dY=dY))
+        dense.append({k: v.clone() for k, v in dict(d, X=X.contiguous(), dY=dY.contiguous()).items()})
+    assert not views[1]["dY"].is_contiguous() and not X.is_contiguous()
+    mdt = {"fp32": fb.FP32, "int8": fb.INT8}[moment]
+    dXv = [torch.empty(T, inn, dtype=torch.bfloat16, device=DEV) for _ in outs]
+    dXd = [torch.empty(T, inn, dtype=torch.bfloat16, device=DEV) for _ in outs]
+    fb.forge_layer_backward_grouped(views, dXv, *hp_args(7), mdt)
+    fb.forge_layer_backward_grouped(dense, dXd, *hp_args(7), mdt)
+    torch.cuda.synchronize()
+    for a, b, xa, xb in zip(views, dense, dXv, dXd):
+        for k in ("W", "m", "v") + (("m_scale", "v_scale") if moment == "int8" else ()):
+            assert torch.equal(a[k].view(torch.uint8), b[k].view(torch.uint8)), k
+        assert torch.equal(xa, xb)
+    assert (dXv[0].float().abs() > 0).any()
+
+
 def test_store_g_matches_oracle_gradient():
     p = synth.make_problem("x", 300, 264, 520, seed=9)
     G = torch.empty(264, 520, device=DEV)
