@@ -370,10 +370,19 @@ def run_cuda(args):
             rot.append((lk, fb.make_problem_array(lk)))
 
     G_ctl = torch.empty(layer[0]["W"].shape, dtype=torch.float32, device=dev) if args.optimizer == "storeg" else None
+    dp_plan = dp_pool = None
+    if args.schedule == "bucket":                    # the data-parallel bucket-transient schedule
+        if args.optimizer != "adamw" or args.moments == "fp8" or args.distinct_layers > 1:
+            raise SystemExit("--schedule bucket: AdamW with fp32 / bf16 / int8 moments")
+        from paper_2606_22932_b200 import dp
+        dp_plan = dp.BucketPlan([tuple(d["W"].shape) for d in layer], args.bucket_mb << 20, slots=2)
+        dp_pool = [torch.empty(dp_plan.slot_elems, dtype=torch.float32, device=dev) for _ in range(dp_plan.slots)]
 
     def step(t):
         if args.optimizer == "storeg":             # the paper's store-G control: same mainloop, G stored
             fb.forge_wgrad_store_g(layer[0]["X"], layer[0]["dY"], G_ctl, stream=stream)
+        elif dp_plan is not None:                      # store-G into the rotating bucket, (all-reduce,) update from it
+            dp.bucket_step_adamw(layer, t, hpt, dp_plan, dp_pool, group=None)
         elif args.optimizer == "adamw":
             lk, ak = rot[t % len(rot)]
             fb.forge_wgrad_adamw_grouped(lk, t, *hpt, mdt, stream=stream, _arr=ak)
@@ -446,10 +455,14 @@ def run_cuda(args):
                                     f"{args.optimizer} with {nst} {args.moments} state tensor(s)"),
                        "moments": args.moments, "params_per_layer": params, "tokens": args.tokens,
                        "distinct_layers": len(rot),
+                       "schedule": ("fused" if dp_plan is None else
+                                    f"dp bucket-transient: {len(dp_plan.buckets)} buckets, {dp_plan.transient_bytes >> 20} MiB of fp32 "
+                                    f"gradient in flight, all-reduce over {world} rank(s)"),
                        "l2": "working set 4.4 GB/layer >> 126 MB L2, no flush needed",
                        "parallelism": f"replicated layers x{world}, no collective"},
             "roofline": roofline, "gpu_launches": int(launches), "clocks": sampler.result(),
-            "dw_bytes_allocated": 0, "library_workspace_bytes": fb.forge_workspace_bytes()}
+            "dw_bytes_allocated": 0 if dp_plan is None else dp_plan.transient_bytes,
+            "library_workspace_bytes": fb.forge_workspace_bytes()}
 
     if rank == 0 and ((not args.no_extras and is_headline) or args.sustained):
         # ---- the same launch under SUSTAINED load: about 1.2 s of back-to-back launches, the last third timed.
@@ -518,6 +531,9 @@ def main():
     ap.add_argument("--tokens", type=int, default=T_TOKENS, help="T (configs[3] sweeps 512/2048/8192 on gate)")
     ap.add_argument("--distinct-layers", type=int, default=1,
                     help="rotate the timed loop over N resident layers (default 1: the same layer re-stepped)")
+    ap.add_argument("--schedule", choices=["fused", "bucket"], default="fused",
+                    help="bucket = the data-parallel schedule of dp.py (gradient through a rotating fp32 bucket)")
+    ap.add_argument("--bucket-mb", type=int, default=256)
     ap.add_argument("--sustained", action="store_true", help="add the sustained-load leg even with --no-extras / other workloads")
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, same-GPU baselines and the CPU oracle leg")
     args = ap.parse_args()

@@ -186,15 +186,25 @@ forge_status_t forge_wgrad_adamw_grouped_host(const forge_problem_t *problems, i
                                              float beta1, float beta2, float eps, float wd,
                                              forge_moment_dtype_t moment_dtype);
 
-/* TEST-ONLY twin (the paper's "store-G control", App. D): the identical mainloop
- * but the fp32 tile is written to G[out,in] instead of consumed.  Never on the product path. */
+/* The two halves of the fused call, for the one case that cannot fuse: data / context parallelism with a nonlinear
+ * update (Prop. 2(ii)).  There the gradient tiles stream into a small rotating fp32 bucket, the bucket is
+ * all-reduced, and the update is applied from the reduced bucket ("bucket-transient schedule"; 304);
+ * paper_2606_22932_b200/dp.py drives that schedule.  They are also the paper's "store-G control" (PAPER.md:334-345
+ * App. D) and its standalone optimizer kernel (86), and the tests use them as twins of the fused kernel:
+ * never on the single-GPU / weight-sharded product path, which materialises no gradient.
+ *
+ * forge_wgrad_store_g[_grouped]: the identical mainloop, the fp32 tile is written to G[out,in] (dense, problem.m =
+ * G for the grouped form; W, v and the scales must be NULL; ldx / lddy honoured, so a row range of a layer is a problem
+ * of its own with a column slice of dY).  A later micro-batch adds to the same bucket with
+ * forge_wgrad_accumulate_grouped(mu = 1). */
 forge_status_t forge_wgrad_store_g(const void *X, const void *dY, float *G,
                                    int32_t T, int32_t out, int32_t in, forge_stream_t stream);
+forge_status_t forge_wgrad_store_g_grouped(const forge_problem_t *problems, int32_t count, forge_stream_t stream);
 
-/* TEST/BENCH-ONLY unfused optimizer pass (the paper's standalone "FORGE optimizer kernel",
- * PAPER.md:354; 86): applies the same per-element update function as the fused epilogue to a
- * materialised fp32 G[out,in].  forge_wgrad_store_g + this must be bit-identical to
- * forge_wgrad_adamw ("the operands are bit-identical and so are the results"). */
+/* forge_adamw_from_g: applies the same per-element update function as the fused epilogue to a materialised fp32
+ * G[out,in] (any contiguous row range of a layer: out is then the number of rows passed).  forge_wgrad_store_g + this
+ * is bit-identical to forge_wgrad_adamw ("the operands are bit-identical and so are the results").
+ * FP32 / BF16 / INT8 moments. */
 forge_status_t forge_adamw_from_g(const float *G, void *W, void *m, void *v,
                                   float *m_scale, float *v_scale, int32_t out, int32_t in,
                                   int64_t step, float lr, float beta1, float beta2, float eps, float wd,

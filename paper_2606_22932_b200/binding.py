@@ -22,7 +22,7 @@ STATUS_NAMES = ["FORGE_OK", "FORGE_ERR_NULL_PTR", "FORGE_ERR_BAD_SHAPE", "FORGE_
                 "FORGE_ERR_BAD_HYPERPARAM", "FORGE_ERR_BAD_DTYPE", "FORGE_ERR_UNSUPPORTED_ARCH",
                 "FORGE_ERR_CUDA"]
 EXPORTS = ["forge_wgrad_adamw", "forge_wgrad_adamw_grouped", "forge_wgrad_step_grouped", "forge_wgrad_accumulate_grouped", "forge_layer_backward_grouped", "forge_wgrad_adamw_sr_grouped", "forge_wgrad_adamw_host", "forge_wgrad_adamw_grouped_host",
-           "forge_wgrad_store_g", "forge_adamw_from_g", "forge_workspace_bytes", "forge_launch_count",
+           "forge_wgrad_store_g", "forge_wgrad_store_g_grouped", "forge_adamw_from_g", "forge_workspace_bytes", "forge_launch_count",
            "forge_last_cuda_error", "forge_status_string", "forge_version"]
 
 
@@ -82,6 +82,8 @@ def lib() -> ctypes.CDLL:
         L.forge_wgrad_adamw_host.argtypes = [c_void_p] * 7 + [c_int32] * 3 + hp + [ctypes.c_int]
         L.forge_wgrad_store_g.restype = ctypes.c_int
         L.forge_wgrad_store_g.argtypes = [c_void_p] * 3 + [c_int32] * 3 + [c_void_p]
+        L.forge_wgrad_store_g_grouped.restype = ctypes.c_int
+        L.forge_wgrad_store_g_grouped.argtypes = [ctypes.POINTER(forge_problem_t), c_int32, c_void_p]
         L.forge_adamw_from_g.restype = ctypes.c_int
         L.forge_adamw_from_g.argtypes = [c_void_p] * 6 + [c_int32] * 2 + hp + [ctypes.c_int, c_void_p]
         L.forge_workspace_bytes.restype = ctypes.c_size_t
@@ -226,7 +228,7 @@ def forge_wgrad_adamw_grouped_host(problems, step, lr, beta1, beta2, eps, wd, mo
 
 
 def forge_wgrad_store_g(X, dY, G, stream=None, check=True) -> int:
-    """TEST-ONLY store-G twin: G[out,in] fp32 = dY^T X."""
+    """Store-G: G[out,in] fp32 = dY^T X; the DP bucket producer and the fused kernel's test twin."""
     T, inn = X.shape
     out = dY.shape[1]
     st = lib().forge_wgrad_store_g(_ptr(X), _ptr(dY), _ptr(G), T, out, inn, _stream(stream))
@@ -235,9 +237,18 @@ def forge_wgrad_store_g(X, dY, G, stream=None, check=True) -> int:
     return st
 
 
+def forge_wgrad_store_g_grouped(problems, stream=None, check=True, _arr=None) -> int:
+    """include/forge.h forge_wgrad_store_g_grouped: problems carry X, dY and m = the fp32 G slice (dp.py buckets)."""
+    arr = make_problem_array(problems) if _arr is None else _arr
+    st = lib().forge_wgrad_store_g_grouped(arr, len(arr), _stream(stream))
+    if check:
+        _check(st, "forge_wgrad_store_g_grouped")
+    return st
+
+
 def forge_adamw_from_g(G, W, m, v, step, lr, beta1, beta2, eps, wd, m_scale=None, v_scale=None, stream=None,
                        check=True) -> int:
-    """TEST/BENCH-ONLY unfused optimizer pass over a materialised fp32 G."""
+    """The update from a materialised fp32 G: dp.py's reduced bucket, and the fused kernel's test twin."""
     out, inn = W.shape
     st = lib().forge_adamw_from_g(_ptr(G), _ptr(W), _ptr(m), _ptr(v), _ptr(m_scale), _ptr(v_scale), out, inn,
                                   int(step), lr, beta1, beta2, eps, wd, moment_dtype_of(m), _stream(stream))

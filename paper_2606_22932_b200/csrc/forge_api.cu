@@ -682,26 +682,45 @@ forge_status_t forge_layer_backward_grouped(const forge_problem_t *problems, voi
     return forge_wgrad_adamw_grouped(problems, count, step, lr, beta1, beta2, eps, wd, moment_dtype, stream);
 }
 
-forge_status_t forge_wgrad_store_g(const void *X, const void *dY, float *G, int32_t T, int32_t out, int32_t in,
-                                   forge_stream_t stream) {
-    if (!X || !dY || !G) return FORGE_ERR_NULL_PTR;
-    if (T < 1 || out < 8 || in < 8 || (out % 8) || (in % 8)) return FORGE_ERR_BAD_SHAPE;
-    if (!aligned16(X) || !aligned16(dY) || !aligned16(G)) return FORGE_ERR_ALIGNMENT;
+forge_status_t forge_wgrad_store_g_grouped(const forge_problem_t *problems, int32_t count, forge_stream_t stream) {
+    if (!problems) return FORGE_ERR_NULL_PTR;
+    if (count < 1) return FORGE_ERR_BAD_SHAPE;
+    int maxT = 0;
+    for (int i = 0; i < count; ++i) {
+        const forge_problem_t &p = problems[i];
+        if (!p.X || !p.dY || !p.m) return FORGE_ERR_NULL_PTR;
+        if (p.W || p.v || p.m_scale || p.v_scale) return FORGE_ERR_BAD_DTYPE;   // a gradient has no state besides G
+        if (p.T < 1 || p.out < 8 || p.in < 8 || (p.out % 8) || (p.in % 8)) return FORGE_ERR_BAD_SHAPE;
+        if (p.ldx != 0 && (p.ldx < p.in || p.ldx % 8 != 0)) return FORGE_ERR_BAD_SHAPE;
+        if (p.lddy != 0 && (p.lddy < p.out || p.lddy % 8 != 0)) return FORGE_ERR_BAD_SHAPE;
+        if (!aligned16(p.X) || !aligned16(p.dY) || !aligned16(p.m)) return FORGE_ERR_ALIGNMENT;
+        maxT = p.T > maxT ? p.T : maxT;
+    }
     DeviceInfo dev;
     forge_status_t s = device_info(dev);
     if (s != FORGE_OK) return s;
+    AdamWScalars hp;
+    std::memset(&hp, 0, sizeof(hp));
+    // The accumulator sums the tokens in ascending order 16 at a time whatever the token-chunk length and the CTA
+    // grouping, so store-G + forge_adamw_from_g is bit-identical to the fused call of any instantiation
+    const int variant = pick_variant(maxT);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    for (int i = 0; i < count; i += kMaxProblems) {
+        const int n = (count - i) < kMaxProblems ? (count - i) : kMaxProblems;
+        if (variant == 1) s = launch_fused<MDT_FP32, MODE_STORE_G, 64, 3, 2, 1, 64, 64>(problems + i, n, hp, dev, st);
+        else if (variant == 4 || variant == 5) s = launch_fused<MDT_FP32, MODE_STORE_G, 64, 4, 2, 2, 64, 64>(problems + i, n, hp, dev, st);
+        else s = launch_fused<MDT_FP32, MODE_STORE_G, 32, 4, 2, 2, 64, 128>(problems + i, n, hp, dev, st);
+        if (s != FORGE_OK) return s;
+    }
+    return FORGE_OK;
+}
+
+forge_status_t forge_wgrad_store_g(const void *X, const void *dY, float *G, int32_t T, int32_t out, int32_t in,
+                                   forge_stream_t stream) {
     forge_problem_t p;
     std::memset(&p, 0, sizeof(p));
     p.X = X; p.dY = dY; p.m = G; p.T = T; p.out = out; p.in = in;
-    AdamWScalars hp;
-    std::memset(&hp, 0, sizeof(hp));
-    // same token-chunk length and CTA grouping as the fused variant chosen for this T: identical
-    // summation order, so store-G + forge_adamw_from_g is bit-identical to the fused call
-    const int variant = pick_variant(T);
-    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-    if (variant == 1) return launch_fused<MDT_FP32, MODE_STORE_G, 64, 3, 2, 1, 64, 64>(&p, 1, hp, dev, st);
-    if (variant == 4 || variant == 5) return launch_fused<MDT_FP32, MODE_STORE_G, 64, 4, 2, 2, 64, 64>(&p, 1, hp, dev, st);
-    return launch_fused<MDT_FP32, MODE_STORE_G, 32, 4, 2, 2, 64, 128>(&p, 1, hp, dev, st);
+    return forge_wgrad_store_g_grouped(&p, 1, stream);
 }
 
 forge_status_t forge_adamw_from_g(const float *G, void *W, void *m, void *v, float *m_scale, float *v_scale,

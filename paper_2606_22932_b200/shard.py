@@ -25,13 +25,13 @@ def shard_rows(out: int, world: int, rank: int, align: int = ROW_ALIGN) -> tuple
 
 def shard_problem(d: dict, world: int, rank: int) -> dict | None:
     """Row shard of one problem dict (keys X, dY, W, m, v[, m_scale, v_scale]); None if empty.
-    W/m/v/scales are row slices (views, updated in place); dY's column slice is copied contiguous
-    because the ABI takes dense tensors only."""
+    W/m/v/scales are row slices (views, updated in place); dY's column slice is a view too (the ABI takes its
+    row pitch, include/forge.h lddy)."""
     out = d["W"].shape[0]
     r0, r1 = shard_rows(out, world, rank)
     if r1 <= r0:
         return None
-    s = {"X": d["X"], "dY": d["dY"][:, r0:r1].contiguous()}
+    s = {"X": d["X"], "dY": d["dY"][:, r0:r1]}
     for k in ("W", "m", "v", "m_scale", "v_scale"):
         if d.get(k) is not None:
             s[k] = d[k][r0:r1]

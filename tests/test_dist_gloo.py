@@ -93,5 +93,6 @@ def test_shard_problem_views_alias_the_state():
     s = shard.shard_problem(d, 2, 1)
     assert s["rows"] == (128, 256)
     assert s["W"].data_ptr() == p.W[128:].data_ptr() and s["m_scale"].shape == (128, 2)
-    assert s["dY"].is_contiguous() and s["dY"].shape == (16, 128)
+    # dY is a column-slice VIEW (row pitch = the full out, passed to the ABI as lddy), not a copy
+    assert s["dY"].shape == (16, 128) and s["dY"].stride() == (256, 1) and s["dY"].data_ptr() == p.dY[:, 128:].data_ptr()
     assert shard.shard_problem(d, 4, 3) is None           # 2 row blocks over 4 ranks: ranks 2,3 empty

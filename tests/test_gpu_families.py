@@ -392,3 +392,66 @@ def test_grouped_host_entry_fp8_matches_device_path_bitwise():
         for k in ("W", "m", "v", "m_scale", "v_scale"):
             assert torch.equal(h[k], d[k].cpu()), k
         assert not torch.equal(h["W"], p.W) and float(h["m_scale"][1]) > 0.0
+
+
+# ------------------------------------------------------------------ DP schedules ------
+@pytest.mark.parametrize("moment", ["fp32", "int8"])
+def test_dp_bucket_schedule_single_rank_is_bitwise_the_fused_step(moment):
+    """dp.bucket_step_adamw with the library's own steps (store-G into a rotating bucket -> update from the bucket),
+    buckets that cut problems into row ranges and mix pieces of two problems: at world size 1 and one micro-batch it
+    must be bit-identical to the fused call (Prop. 1 bucket-wise)."""
+    from paper_2606_22932_b200 import dp
+    hp = synth.HP_DEFAULT
+    hpt = (hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
+    shapes = [(384, 512), (200, 256), (640, 768)]
+    fused, bucketed = [], []
+    for i, (o, c) in enumerate(shapes):
+        p = synth.make_problem(f"dp{i}", 300, o, c, 90 + i)
+        d = dict(X=p.X.to(DEV), dY=p.dY.to(DEV), W=p.W.to(DEV).clone())
+        if moment == "fp32":
+            d.update(m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone())
+        else:
+            mq, ms, vq, vs = fo.quantize(p.m.numpy(), p.v.numpy())
+            d.update(m=torch.from_numpy(mq.copy()).to(DEV), v=torch.from_numpy(vq.copy()).to(DEV),
+                     m_scale=torch.from_numpy(ms.copy()).to(DEV), v_scale=torch.from_numpy(vs.copy()).to(DEV))
+        fused.append(d)
+        bucketed.append({k: (t if k in ("X", "dY") else t.clone()) for k, t in d.items()})
+    plan = dp.BucketPlan(shapes, 4 * 256 * 768, slots=2)
+    assert len(plan.buckets) >= 3 and any(len(b) > 1 for b in plan.buckets)
+    pool = [torch.full((plan.slot_elems,), float("nan"), device=DEV) for _ in range(plan.slots)]
+    dp.bucket_step_adamw(bucketed, 10, hpt, plan, pool)
+    fb.forge_wgrad_adamw_grouped(fused, 10, *hpt, fb.FP32 if moment == "fp32" else fb.INT8)
+    torch.cuda.synchronize()
+    for a, b in zip(bucketed, fused):
+        for k in a:
+            assert torch.equal(a[k].view(torch.uint8), b[k].view(torch.uint8)), k
+    assert plan.transient_bytes < sum(o * c for o, c in shapes) * 4
+
+
+def test_dp_micro_batch_accumulation_and_reduce_into_state_against_the_oracle():
+    """Two micro-batches summed in the fp32 bucket (store-G, then accumulate with mu = 1) before the update, and the
+    single-rank reduce-into-state B <- mu*B + dY^T X; both against the oracle on all tokens."""
+    from paper_2606_22932_b200 import dp
+    hp = synth.HP_DEFAULT
+    hpt = (hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
+    T, o, c = 256, 384, 512
+    p = synth.make_problem("mb", T, o, c, 99)
+    d = dict(X=[p.X[:96].to(DEV), p.X[96:].to(DEV)], dY=[p.dY[:96].to(DEV), p.dY[96:].to(DEV)],
+             W=p.W.to(DEV).clone(), m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone())
+    plan = dp.BucketPlan([(o, c)], 4 * 128 * c, slots=2)
+    pool = [torch.empty(plan.slot_elems, device=DEV) for _ in range(plan.slots)]
+    dp.bucket_step_adamw([d], 10, hpt, plan, pool)
+    B = dict(X=p.X.to(DEV), dY=p.dY.to(DEV), m=p.m.to(DEV).clone())
+    dp.reduce_into_state([B], 0.9)
+    torch.cuda.synchronize()
+    G, E = fo.wgrad(synth.bf16_bits(p.dY), synth.bf16_bits(p.X), with_abs=True)
+    Wo, mo, vo = synth.bf16_bits(p.W).copy(), p.m.numpy().copy(), p.v.numpy().copy()
+    fo.adamw_fp32(Wo, mo, vo, G, 10, *hpt)
+    e = T * 2.0 ** -23 * E
+    mg, vg = d["m"].cpu().numpy().astype(np.float64), d["v"].cpu().numpy().astype(np.float64)
+    assert (np.abs(mg - mo) <= 1e-4 * np.abs(mo) + (1 - hp["beta1"]) * e).all()
+    assert (np.abs(vg - vo) <= 1e-4 * vo + (1 - hp["beta2"]) * (2 * np.abs(G) * e + e * e)).all()
+    assert float((synth.bf16_bits(d["W"].cpu()) == Wo).mean()) > 0.99
+    Bo = p.m.numpy().copy()
+    fo.accumulate(Bo, G, 0.9)
+    assert (np.abs(B["m"].cpu().numpy().astype(np.float64) - Bo) <= e + 2.0 ** -22 * np.abs(Bo)).all()
