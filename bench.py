@@ -202,8 +202,8 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": us, "unit": UNIT, "n_gpus": args.gpus,
             "steps": len(times), "warmup": args.warmup, "ms_per_step": us / 1e3, "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "configs[1]: Llama-3.1-8B layer, 7 projections, T=512, fp32 m/v",
-                       "moments": "fp32", "params_per_layer": layer_counts()[0]},
+            "config": {"workload": "configs[1]: Llama-3.1-8B layer, 7 projections in one grouped launch, T=512",
+                       "moments": "fp32", "params_per_layer": layer_counts()[0], "tokens": T_TOKENS},
             "cpu_baseline": {"value": us, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
             "e2e": {"value": us, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
