@@ -254,8 +254,9 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
 // FORGE_CFG selects the other instantiations for tuning sweeps and the determinism tests only.
 int pick_variant(int maxT) {
     const int forced = env_int("FORGE_CFG", -1);   // debug only
-    // T >= 4096 (fp32 / bf16 moments): the ring-less direct state path, all shared memory to the operand ring
-    return forced >= 0 ? forced : (maxT >= 4096 ? 30 : (maxT > 1024 ? 5 : 0));
+    // T >= 8192 (fp32 / bf16 moments): the ring-less direct state path, all shared memory to the operand ring
+    // (gate_proj: T = 8192 direct 741-770 us vs ring 770-784; T = 4096 direct 469 vs ring 446; T = 2048 320 vs 274)
+    return forced >= 0 ? forced : (maxT >= 8192 ? 30 : (maxT > 1024 ? 5 : 0));
 }
 
 // The direct state path (variants >= 30) moves 16 columns per thread with 32-byte accesses: every row must be a

@@ -186,10 +186,10 @@ def test_fused_equals_store_g_twin_plus_same_update_bitwise(moment, T):
 @pytest.mark.parametrize("moment", ["fp32", "bf16"])
 @pytest.mark.parametrize("out,inn", [(640, 768), (600, 528), (200, 264)])
 def test_direct_state_path_at_large_T_equals_store_g_twin_bitwise(moment, out, inn):
-    """T >= 4096 takes the ring-less direct epilogue (32-byte global accesses, thread = row) when every row is a
+    """T >= 8192 takes the ring-less direct epilogue (32-byte global accesses, thread = row) when every row is a
     whole number of 16-column vectors; (200, 264) is not and falls back to the TMA ring.  Ragged row blocks, several
     column tiles; bit-identical to the store-G twin plus the same update either way."""
-    p = synth.make_problem("x", 4096, out, inn, seed=17)
+    p = synth.make_problem("x", 8192, out, inn, seed=17)
     d1, _ = gpu_state(p, moment)
     d2 = {k: v.clone() for k, v in d1.items()}
     fb.forge_wgrad_adamw(d1["X"], d1["dY"], d1["W"], d1["m"], d1["v"], 5, **HP)
