@@ -82,9 +82,10 @@ struct alignas(64) KernelParams {
     int32_t total_tiles;
     uint32_t sr_seed_lo; // MODE_ADAMW_SR
     int32_t debug;       // ablation switches for profiling ONLY (results are wrong when set):
-                         // 1 = no operand loads / MMA, 2 = no state loads / stores, 4 = no epilogue math
+                         // 1 = no operand loads / MMA, 2 = no state loads / stores, 4 = no epilogue math,
+                         // 8 = no state stores (direct path only)
 };
-enum : int { DBG_NO_MAINLOOP = 1, DBG_NO_STATE = 2, DBG_NO_EPILOGUE = 4 };
+enum : int { DBG_NO_MAINLOOP = 1, DBG_NO_STATE = 2, DBG_NO_EPILOGUE = 4, DBG_NO_STORE = 8 /* direct path only */ };
 
 // CG = 1: one CTA per 128x256 tile.  CG = 2: a CTA pair (cluster of 2, tcgen05 cta_group::2) shares
 // a 256x256 tile: each CTA stages its own 128 rows of A = dY^T and only HALF of B = X (128 of the
@@ -263,7 +264,7 @@ __device__ __forceinline__ void direct_load(DirectRegs<MDT> &r, const char *Wp, 
 }
 template <int MDT>
 __device__ __forceinline__ void direct_step(const AdamWScalars &hp, const uint32_t (&g)[16], DirectRegs<MDT> &r,
-                                            char *Wp, char *Mp, char *Vp) {
+                                            char *Wp, char *Mp, char *Vp, bool no_store = false) {
 #pragma unroll
     for (int e = 0; e < 8; ++e) {               // coordinate pairs (2e, 2e + 1)
         f32x2 w = bf16x2_to_f32x2(r.w[e]), m, v;
@@ -284,6 +285,7 @@ __device__ __forceinline__ void direct_step(const AdamWScalars &hp, const uint32
             r.v[0][e] = f32x2_to_bf16x2(v);
         }
     }
+    if (no_store) return;                       // profiling ablation only
     stg256(Wp, r.w);
 #pragma unroll
     for (int i = 0; i < DirectRegs<MDT>::MV; ++i) {
@@ -914,7 +916,8 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                         direct_load<MDT>(R[(st + 1) & 1], Wp + (st + 1) * 32, Mp + (st + 1) * 16 * MB, Vp + (st + 1) * 16 * MB);
                     tmem_ld_wait();
                     if (ok && !(P.debug & DBG_NO_EPILOGUE))
-                        direct_step<MDT>(hp, g, R[st & 1], Wp + st * 32, Mp + st * 16 * MB, Vp + st * 16 * MB);
+                        direct_step<MDT>(hp, g, R[st & 1], Wp + st * 32, Mp + st * 16 * MB, Vp + st * 16 * MB,
+                                         (P.debug & DBG_NO_STORE) != 0);
                 }
             } else if constexpr (MDT != MDT_INT8) {
                 for (int cb = 0; cb < Cfg::CB; ++cb) {
