@@ -177,8 +177,9 @@ forge_status_t forge_wgrad_adamw_host(const void *X, const void *dY, void *W, vo
                                       forge_moment_dtype_t moment_dtype);
 
 /* The same for a whole group with HOST buffers (every pointer of every problem is a host pointer, ideally pinned):
- * a three-stage pipeline over the problems -- upload, fused step, download on three streams -- so the copies of
- * neighbouring problems overlap each other (PCIe is full duplex) and the kernels.  Device scratch is allocated and
+ * a three-stage pipeline -- upload, fused step, download on three streams -- over ~64 MB row slices of each problem's
+ * state (whole tile rows: the result is bit-identical to the device-resident call), so the download of one slice
+ * overlaps the upload of the next (PCIe is full duplex) and the kernels.  Device scratch is allocated and
  * freed inside the call; synchronous on return.  All four moment dtypes (INT8: the block scales, FP8: the two
  * float[2] scale / amax pairs travel with the codes).  A tensor shared by several problems
  * (q/k/v read one X) is uploaded once per problem. */

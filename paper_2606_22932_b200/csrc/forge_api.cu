@@ -836,12 +836,28 @@ forge_status_t forge_wgrad_adamw_grouped_host(const forge_problem_t *problems, i
                  mdt == FORGE_MOMENT_INT8 ? n / FORGE_QBLOCK * 4 : (mdt == FORGE_MOMENT_FP8 ? 2 * sizeof(float) : 0), total};
         total += up(sz[i].bX) + up(sz[i].bY) + up(sz[i].bW) + 2 * up(sz[i].bM) + 2 * up(sz[i].bS);
     }
+    // Row chunks: a problem's state goes up, is stepped and comes down in slices of about 64 MB (whole 256-row tile
+    // rows, so the tiles -- and the bits -- are those of the unchunked call), each slice a sub-problem that reads a
+    // column slice of the resident dY through lddy.  The download of slice c overlaps the upload of slice c + 1
+    // (PCIe is full duplex); without the slicing the first upload and the last download (0.6 GB each for gate_proj)
+    // overlap nothing.
+    const bool i8 = mdt == FORGE_MOMENT_INT8, f8 = mdt == FORGE_MOMENT_FP8;
+    const int slice_mb = env_int("FORGE_HOST_SLICE_MB", 64);   // tuning only; 0 = one slice per problem
+    auto chunk_rows = [&](const forge_problem_t &p) {
+        if (slice_mb <= 0) return static_cast<int>(p.out);
+        const size_t row_bytes = static_cast<size_t>(p.in) * (2 + 2 * mom);
+        size_t rows = ((static_cast<size_t>(slice_mb) << 20) / row_bytes + 255) / 256 * 256;
+        if (rows < 256) rows = 256;
+        return static_cast<int>(rows < static_cast<size_t>(p.out) ? rows : static_cast<size_t>(p.out));
+    };
+    int nev = 0;
+    for (int i = 0; i < count; ++i) nev += 2 * ((problems[i].out + chunk_rows(problems[i]) - 1) / chunk_rows(problems[i]));
     uint8_t *d = nullptr;
     cudaStream_t s_in = nullptr, s_c = nullptr, s_out = nullptr;
-    cudaEvent_t *ev = static_cast<cudaEvent_t *>(std::calloc(2 * count, sizeof(cudaEvent_t)));
+    cudaEvent_t *ev = static_cast<cudaEvent_t *>(std::calloc(nev, sizeof(cudaEvent_t)));
     cudaError_t e = cudaMalloc(&d, total);
     auto cleanup = [&]() {
-        if (ev) for (int i = 0; i < 2 * count; ++i) if (ev[i]) cudaEventDestroy(ev[i]);
+        if (ev) for (int i = 0; i < nev; ++i) if (ev[i]) cudaEventDestroy(ev[i]);
         if (s_in) cudaStreamDestroy(s_in);
         if (s_c) cudaStreamDestroy(s_c);
         if (s_out) cudaStreamDestroy(s_out);
@@ -849,19 +865,20 @@ forge_status_t forge_wgrad_adamw_grouped_host(const forge_problem_t *problems, i
         std::free(ev); std::free(sz); std::free(dp);
     };
     forge_status_t rc = FORGE_OK;
+    if (!ev) e = cudaErrorMemoryAllocation;
 #define FORGE_TRY(x) do { if (e == cudaSuccess) e = (x); } while (0)
     FORGE_TRY(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
     FORGE_TRY(cudaStreamCreateWithFlags(&s_c, cudaStreamNonBlocking));
     FORGE_TRY(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
-    for (int i = 0; i < 2 * count && ev; ++i) FORGE_TRY(cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming));
-    // three-stage pipeline over the problems: copy-in (H2D), fused step, copy-out (D2H) on three streams, so the
-    // upload of problem i+1 and the download of problem i-1 overlap the kernel of problem i (PCIe is full duplex)
+    for (int i = 0; i < nev && ev; ++i) FORGE_TRY(cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming));
+    // three-stage pipeline over the slices: copy-in (H2D), fused step, copy-out (D2H) on three streams;
     // largest problem first: the download that cannot overlap anything (the last one) is then the smallest
     int *order = static_cast<int *>(std::malloc(sizeof(int) * count));
     for (int i = 0; i < count && order; ++i) order[i] = i;
     for (int i = 0; i < count && order; ++i)
         for (int j = i + 1; j < count; ++j)
             if (sz[order[j]].bW > sz[order[i]].bW) { const int t = order[i]; order[i] = order[j]; order[j] = t; }
+    int evi = 0;
     for (int k = 0; k < count && order && e == cudaSuccess && rc == FORGE_OK; ++k) {
         const int i = order[k];
         const forge_problem_t &p = problems[i];
@@ -877,23 +894,48 @@ forge_status_t forge_wgrad_adamw_grouped_host(const forge_problem_t *problems, i
         g.v_scale = sz[i].bS ? reinterpret_cast<float *>(q) : nullptr;
         FORGE_TRY(cudaMemcpyAsync(const_cast<void *>(g.X), p.X, sz[i].bX, cudaMemcpyHostToDevice, s_in));
         FORGE_TRY(cudaMemcpyAsync(const_cast<void *>(g.dY), p.dY, sz[i].bY, cudaMemcpyHostToDevice, s_in));
-        FORGE_TRY(cudaMemcpyAsync(g.W, p.W, sz[i].bW, cudaMemcpyHostToDevice, s_in));
-        FORGE_TRY(cudaMemcpyAsync(g.m, p.m, sz[i].bM, cudaMemcpyHostToDevice, s_in));
-        FORGE_TRY(cudaMemcpyAsync(g.v, p.v, sz[i].bM, cudaMemcpyHostToDevice, s_in));
-        if (sz[i].bS) {
+        if (f8) {                                   // one {scale, amax} pair per tensor, shared by the slices
             FORGE_TRY(cudaMemcpyAsync(g.m_scale, p.m_scale, sz[i].bS, cudaMemcpyHostToDevice, s_in));
             FORGE_TRY(cudaMemcpyAsync(g.v_scale, p.v_scale, sz[i].bS, cudaMemcpyHostToDevice, s_in));
         }
-        FORGE_TRY(cudaEventRecord(ev[2 * i], s_in));
-        FORGE_TRY(cudaStreamWaitEvent(s_c, ev[2 * i], 0));
-        if (e == cudaSuccess)
-            rc = forge_wgrad_adamw_grouped(&g, 1, step, lr, beta1, beta2, eps, wd, moment_dtype, reinterpret_cast<forge_stream_t>(s_c));
-        FORGE_TRY(cudaEventRecord(ev[2 * i + 1], s_c));
-        FORGE_TRY(cudaStreamWaitEvent(s_out, ev[2 * i + 1], 0));
-        FORGE_TRY(cudaMemcpyAsync(p.W, g.W, sz[i].bW, cudaMemcpyDeviceToHost, s_out));
-        FORGE_TRY(cudaMemcpyAsync(p.m, g.m, sz[i].bM, cudaMemcpyDeviceToHost, s_out));
-        FORGE_TRY(cudaMemcpyAsync(p.v, g.v, sz[i].bM, cudaMemcpyDeviceToHost, s_out));
-        if (sz[i].bS) {
+        const int crow = chunk_rows(p);
+        const size_t sblk = static_cast<size_t>(p.in) / FORGE_QBLOCK;     // int8: scales per row
+        for (int r0 = 0; r0 < p.out && e == cudaSuccess && rc == FORGE_OK; r0 += crow, evi += 2) {
+            const int rows = (p.out - r0) < crow ? (p.out - r0) : crow;
+            const size_t e0 = static_cast<size_t>(r0) * p.in, n = static_cast<size_t>(rows) * p.in;
+            forge_problem_t c = g;
+            c.out = rows;
+            c.ldx = 0;
+            c.lddy = p.out;
+            c.dY = static_cast<const uint8_t *>(g.dY) + static_cast<size_t>(r0) * 2;
+            c.W = static_cast<uint8_t *>(g.W) + e0 * 2;
+            c.m = static_cast<uint8_t *>(g.m) + e0 * mom;
+            c.v = static_cast<uint8_t *>(g.v) + e0 * mom;
+            if (i8) { c.m_scale = g.m_scale + r0 * sblk; c.v_scale = g.v_scale + r0 * sblk; }
+            uint8_t *hW = static_cast<uint8_t *>(p.W) + e0 * 2, *hM = static_cast<uint8_t *>(p.m) + e0 * mom,
+                    *hV = static_cast<uint8_t *>(p.v) + e0 * mom;
+            FORGE_TRY(cudaMemcpyAsync(c.W, hW, n * 2, cudaMemcpyHostToDevice, s_in));
+            FORGE_TRY(cudaMemcpyAsync(c.m, hM, n * mom, cudaMemcpyHostToDevice, s_in));
+            FORGE_TRY(cudaMemcpyAsync(c.v, hV, n * mom, cudaMemcpyHostToDevice, s_in));
+            if (i8) {
+                FORGE_TRY(cudaMemcpyAsync(c.m_scale, p.m_scale + r0 * sblk, rows * sblk * 4, cudaMemcpyHostToDevice, s_in));
+                FORGE_TRY(cudaMemcpyAsync(c.v_scale, p.v_scale + r0 * sblk, rows * sblk * 4, cudaMemcpyHostToDevice, s_in));
+            }
+            FORGE_TRY(cudaEventRecord(ev[evi], s_in));
+            FORGE_TRY(cudaStreamWaitEvent(s_c, ev[evi], 0));
+            if (e == cudaSuccess)
+                rc = forge_wgrad_adamw_grouped(&c, 1, step, lr, beta1, beta2, eps, wd, moment_dtype, reinterpret_cast<forge_stream_t>(s_c));
+            FORGE_TRY(cudaEventRecord(ev[evi + 1], s_c));
+            FORGE_TRY(cudaStreamWaitEvent(s_out, ev[evi + 1], 0));
+            FORGE_TRY(cudaMemcpyAsync(hW, c.W, n * 2, cudaMemcpyDeviceToHost, s_out));
+            FORGE_TRY(cudaMemcpyAsync(hM, c.m, n * mom, cudaMemcpyDeviceToHost, s_out));
+            FORGE_TRY(cudaMemcpyAsync(hV, c.v, n * mom, cudaMemcpyDeviceToHost, s_out));
+            if (i8) {
+                FORGE_TRY(cudaMemcpyAsync(p.m_scale + r0 * sblk, c.m_scale, rows * sblk * 4, cudaMemcpyDeviceToHost, s_out));
+                FORGE_TRY(cudaMemcpyAsync(p.v_scale + r0 * sblk, c.v_scale, rows * sblk * 4, cudaMemcpyDeviceToHost, s_out));
+            }
+        }
+        if (f8) {                                   // after the last slice's kernel: s_out already waits for it
             FORGE_TRY(cudaMemcpyAsync(p.m_scale, g.m_scale, sz[i].bS, cudaMemcpyDeviceToHost, s_out));
             FORGE_TRY(cudaMemcpyAsync(p.v_scale, g.v_scale, sz[i].bS, cudaMemcpyDeviceToHost, s_out));
         }

@@ -455,3 +455,47 @@ def test_dp_micro_batch_accumulation_and_reduce_into_state_against_the_oracle():
     Bo = p.m.numpy().copy()
     fo.accumulate(Bo, G, 0.9)
     assert (np.abs(B["m"].cpu().numpy().astype(np.float64) - Bo) <= e + 2.0 ** -22 * np.abs(Bo)).all()
+
+
+@pytest.mark.parametrize("moment", ["fp32", "int8", "fp8"])
+def test_grouped_host_entry_row_slices_are_bitwise_the_device_call(moment):
+    """forge_wgrad_adamw_grouped_host streams a problem's state in ~64 MB row slices (several slices and a ragged last
+    one here: 2400 rows of 8192 columns); the slices are whole tile rows reading a column slice of the resident dY, so
+    the result equals the device-resident call bit for bit, scales / amax included."""
+    hp = synth.HP_DEFAULT
+    hpt = (hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
+    p = synth.make_problem("big", 64, 2400, 8192, 81)
+    t = dict(X=p.X, dY=p.dY, W=p.W.clone())
+    if moment == "fp32":
+        t.update(m=p.m.clone(), v=p.v.clone())
+    elif moment == "int8":
+        mq, ms, vq, vs = fo.quantize(p.m.numpy(), p.v.numpy())
+        t.update(m=torch.from_numpy(mq.copy()), v=torch.from_numpy(vq.copy()), m_scale=torch.from_numpy(ms.copy()),
+                 v_scale=torch.from_numpy(vs.copy()))
+    else:
+        mq, ms = fo.fp8_quantize(p.m.numpy())
+        vq, vs = fo.fp8_quantize(p.v.numpy())
+        t.update(m=torch.from_numpy(mq.copy()), v=torch.from_numpy(vq.copy()), m_scale=torch.from_numpy(ms.copy()),
+                 v_scale=torch.from_numpy(vs.copy()))
+    small = synth.make_problem("small", 64, 136, 272, 82)       # a second, single-slice problem in the same call
+    t2 = dict(X=small.X, dY=small.dY, W=small.W.clone())
+    if moment == "fp32":
+        t2.update(m=small.m.clone(), v=small.v.clone())
+    elif moment == "int8":
+        t2 = None                                               # int8 needs in % 256 == 0
+    else:
+        mq, ms = fo.fp8_quantize(small.m.numpy())
+        vq, vs = fo.fp8_quantize(small.v.numpy())
+        t2.update(m=torch.from_numpy(mq.copy()), v=torch.from_numpy(vq.copy()), m_scale=torch.from_numpy(ms.copy()),
+                  v_scale=torch.from_numpy(vs.copy()))
+    ts = [t] + ([t2] if t2 is not None else [])
+    host = [{k: x.clone().pin_memory() for k, x in d.items()} for d in ts]
+    devs = [{k: x.to(DEV).clone() for k, x in d.items()} for d in ts]
+    mdt = {"fp32": fb.FP32, "int8": fb.INT8, "fp8": fb.FP8}[moment]
+    fb.forge_wgrad_adamw_grouped_host(host, 10, *hpt, mdt)
+    fb.forge_wgrad_adamw_grouped(devs, 10, *hpt, mdt)
+    torch.cuda.synchronize()
+    for h, d, src in zip(host, devs, ts):
+        for k in h:
+            assert torch.equal(h[k].view(torch.uint8), d[k].cpu().view(torch.uint8)), k
+        assert not torch.equal(h["W"], src["W"])
