@@ -98,6 +98,10 @@ typedef struct {
     int64_t ldx, lddy;
 } forge_problem_t;
 
+/* Environment: FORGE_POWER_STATE=boost|capped overrides the library's own estimate of whether a launch will run under
+ * the board's power cap (it picks between two bit-identical instantiations of the fp32-moment kernel; DESIGN.md section
+ * 6).  FORGE_CFG / FORGE_GRID / FORGE_ABLATE / FORGE_HOST_SLICE_MB are tuning and profiling switches (profiles/). */
+
 /* Fused weight gradient + AdamW step for one layer (Algorithm 1).
  * `step` is the 1-based index t of the update being applied (bias terms 1-beta^t); step < 1,
  * lr < 0 or non-finite, beta outside [0,1), eps < 0, wd < 0 -> FORGE_ERR_BAD_HYPERPARAM. */

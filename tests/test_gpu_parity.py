@@ -261,6 +261,28 @@ def test_result_independent_of_grid_size_and_repeatable():
             assert torch.equal(outs[0][k], d[k])
 
 
+def test_power_state_variants_are_bit_identical():
+    """The fp32 path switches chunk shape when the library expects the launch to run under the board's power cap
+    (forge_api.cu expect_power_cap); FORGE_POWER_STATE forces either side.  Same bits, grouped launch, ragged shapes."""
+    ps = [synth.make_problem("a", 512, 640, 768, 21), synth.make_problem("b", 200, 136, 264, 22), synth.make_problem("c", 512, 1024, 1536, 23)]
+    outs = []
+    for state in ("boost", "capped", None):
+        if state:
+            os.environ["FORGE_POWER_STATE"] = state
+        else:
+            os.environ.pop("FORGE_POWER_STATE", None)
+        devs = [dict(X=p.X.to(DEV), dY=p.dY.to(DEV), W=p.W.to(DEV).clone(), m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone()) for p in ps]
+        fb.forge_wgrad_adamw_grouped(devs, *hp_args(4), fb.FP32)
+        torch.cuda.synchronize()
+        outs.append(devs)
+    os.environ.pop("FORGE_POWER_STATE", None)
+    for devs in outs[1:]:
+        for a, b in zip(outs[0], devs):
+            for k in ("W", "m", "v"):
+                assert torch.equal(a[k], b[k]), k
+    assert not torch.equal(outs[0][0]["W"], ps[0].W.to(DEV))
+
+
 # ------------------------------------------------------------------------------ properties ---
 def test_lr_zero_keeps_w_and_inputs_untouched_moments_move():
     p = synth.make_problem("x", 256, 256, 512, seed=13)
