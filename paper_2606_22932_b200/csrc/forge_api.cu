@@ -537,7 +537,11 @@ forge_status_t dispatch_family(const forge_problem_t *probs, int count, int nst,
         return launch_fused<MDT, MODE_FAMILY, 64, 4, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
     }
     if (big) return launch_fused<MDT, MODE_FAMILY, 64, 4, 2, 2, 64, 64, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
-    if (MDT == MDT_FP32) return launch_fused<MDT, MODE_FAMILY, 32, 4, 2, 2, 64, 128, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
+    if (MDT == MDT_FP32) {      // two fp32 states: AdamW's byte count, and AdamW's two instantiations by power state
+        if (expect_power_cap(dev.device, estimate_ms(probs, count, FORGE_MOMENT_FP32)) && forced < 0)
+            return launch_fused<MDT, MODE_FAMILY, 32, 3, 2, 2, 128, 64, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
+        return launch_fused<MDT, MODE_FAMILY, 32, 4, 2, 2, 64, 128, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
+    }
     return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 64, 64, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
 }
 
