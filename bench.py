@@ -437,7 +437,7 @@ def run_cuda(args):
     else:
         roofline = {"bound": "tensor", "achieved": tfs, "peak": tf_peak, "unit": "TFLOP/s", "frac": tfs / tf_peak,
                     "peak_kind": tf_kind, "burst_peak": tf_burst, "sustained_peak": tf_sustained}
-    is_headline = args.workload == "layer" and args.tokens == T_TOKENS and args.optimizer == "adamw"
+    is_headline = args.workload == "layer" and args.tokens == T_TOKENS and args.optimizer == "adamw" and dp_plan is None
     roofline.update({"traffic": NCU_TRAFFIC_BYTES[args.moments] if is_headline else None, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": alg_bytes, "flops_per_launch": flops,
                      "roofline_us": max(t_hbm_us, t_tensor_us), "hbm_term_us": t_hbm_us, "tensor_term_us": t_tensor_us,
