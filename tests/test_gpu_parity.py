@@ -261,6 +261,44 @@ def test_result_independent_of_grid_size_and_repeatable():
             assert torch.equal(outs[0][k], d[k])
 
 
+def test_randomised_shapes_strides_and_dispatch_paths_equal_the_twin_bitwise():
+    """40 seeded random cases over T (1 ... 9000: ring, large-T ring, direct path), ragged out / in, the three moment dtypes,
+    strided operand views and both power-state instantiations: the fused call must equal store-G + the same update bit
+    for bit.  (The gradient itself is checked against the oracle by the tests above.)"""
+    import random
+    rnd = random.Random(20260622)
+    for it in range(40):
+        moment = rnd.choice(["fp32", "bf16", "int8"])
+        T = rnd.choice([1, 7, 33, 100, 512, 777, 2048, 4096, 8192, 8200]) if rnd.random() < 0.7 else rnd.randint(1, 3000)
+        out = 8 * rnd.randint(1, 120)
+        inn = 256 * rnd.randint(1, 4) if moment == "int8" else (16 * rnd.randint(1, 64) if moment == "bf16" or rnd.random() < 0.7 else 8 * rnd.randint(1, 128))
+        if T >= 4096:
+            out, inn = min(out, 520), min(inn, 768)
+        p = synth.make_problem("f", T, out, inn, seed=5000 + it)
+        d1, _ = gpu_state(p, moment)
+        X, dY = d1["X"], d1["dY"]
+        if rnd.random() < 0.4:                              # column slices of wider tensors: ldx / lddy
+            wx = torch.zeros(T, inn + 24, dtype=torch.bfloat16, device=DEV)
+            wy = torch.zeros(T, out + 40, dtype=torch.bfloat16, device=DEV)
+            wx[:, 8:8 + inn], wy[:, 16:16 + out] = X, dY
+            d1["X"], d1["dY"] = wx[:, 8:8 + inn], wy[:, 16:16 + out]
+        d2 = {k: (v if k in ("X", "dY") else v.clone()) for k, v in d1.items()}
+        if rnd.random() < 0.3:
+            os.environ["FORGE_POWER_STATE"] = "capped"
+        try:
+            fb.forge_wgrad_adamw_grouped([d1], *hp_args(5), {"fp32": fb.FP32, "bf16": fb.BF16, "int8": fb.INT8}[moment])
+        finally:
+            os.environ.pop("FORGE_POWER_STATE", None)
+        G = torch.full((out, inn), float("nan"), device=DEV)
+        fb.forge_wgrad_store_g(X, dY, G)
+        fb.forge_adamw_from_g(G, d2["W"], d2["m"], d2["v"], 5, m_scale=d2.get("m_scale"), v_scale=d2.get("v_scale"), **HP)
+        torch.cuda.synchronize()
+        assert not torch.isnan(G).any()
+        for k in d1:
+            if k not in ("X", "dY"):
+                assert torch.equal(d1[k].view(torch.uint8), d2[k].view(torch.uint8)), (it, moment, T, out, inn, k)
+
+
 def test_power_state_variants_are_bit_identical():
     """The fp32 path switches chunk shape when the library expects the launch to run under the board's power cap
     (forge_api.cu expect_power_cap); FORGE_POWER_STATE forces either side.  Same bits, grouped launch, ragged shapes."""
