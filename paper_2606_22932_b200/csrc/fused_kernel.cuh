@@ -85,7 +85,8 @@ struct alignas(64) KernelParams {
                          // 1 = no operand loads / MMA, 2 = no state loads / stores, 4 = no epilogue math,
                          // 8 = no state stores (direct path only)
 };
-enum : int { DBG_NO_MAINLOOP = 1, DBG_NO_STATE = 2, DBG_NO_EPILOGUE = 4, DBG_NO_STORE = 8 /* direct path only */ };
+enum : int { DBG_NO_MAINLOOP = 1, DBG_NO_STATE = 2, DBG_NO_EPILOGUE = 4, DBG_NO_STORE = 8 /* direct path only */,
+              DBG_NO_A = 16 /* CTA pairs: dY chunks loaded for the first ring pass only (operand traffic halved) */ };
 
 // CG = 1: one CTA per 128x256 tile.  CG = 2: a CTA pair (cluster of 2, tcgen05 cta_group::2) shares
 // a 256x256 tile: each CTA stages its own 128 rows of A = dY^T and only HALF of B = X (128 of the
@@ -726,10 +727,11 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                                         kb * kBlockK, kEvictLast);
                     } else {
                         // both CTAs' bytes are counted on the LEADER's full barrier
-                        if (rank == 0) mbar_expect_tx(bar_ml_full + 8 * s, 2 * Cfg::ML_STAGE);
+                        const bool no_a = (P.debug & DBG_NO_A) && it >= kStages;
+                        if (rank == 0) mbar_expect_tx(bar_ml_full + 8 * s, 2 * (Cfg::ML_STAGE - (no_a ? Cfg::A_STAGE : 0)));
                         const uint32_t full = mapa_shared(bar_ml_full + 8 * s, 0);
 #pragma unroll
-                        for (int i = 0; i < BLOCK_M / 64; ++i)
+                        for (int i = 0; i < (no_a ? 0 : BLOCK_M / 64); ++i)
                             tma_load_2d_cg2(a + i * kBlockK * 128, &pd.map_dY, full, tc.tm * BLOCK_M + i * 64,
                                             kb * kBlockK, kEvictLast);
 #pragma unroll
