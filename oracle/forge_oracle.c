@@ -186,38 +186,39 @@ void forge_oracle_adamw_bf16(uint16_t *W, uint16_t *m, uint16_t *v, const double
 
 #define FORGE_ORACLE_QBLOCK 256   /* BASELINE.json: 256-element blocks along `in` (reading S4) */
 
-/* App. B: per-block absmax a, scale s = a/127, q(x) = s*round(x/s).
- * The decision that produces an integer code is taken in the kernel's precision (S7):
- *   xf = fp32(x);  a = max|xf|;  inv = fp32(127/a);  code = rint(xf * inv), where the product of the
- *   two fp32 values is EXACT (it fits a double) and is rounded once, to the nearest integer, ties
- *   to even; clamped to [-127,127].
- * An all-zero block stores a = 0 and codes 0. */
+/* App. B: "m blockwise symmetric int8 ... a block with absolute maximum a has scale
+ * s = a/127 and round-to-nearest quantization q(x) = s*round(x/s)".  Written out in fp64 from the fp64
+ * moments: a = max|x| over the block, stored as fp32 (north_star: "fp32 absmax scale"); s = a/127 with
+ * that stored a; code = rint(x/s) (S7: ties to even), clamped to [-127,127] (the fp32 rounding of a can
+ * put |x/s| a hair above 127).  An all-zero block stores a = 0 and codes 0. */
 void forge_oracle_quant_m_block(const double *x, int n, int8_t *code, float *scale)
 {
-    float a = 0.0f;
-    for (int i = 0; i < n; ++i) { float f = fabsf((float)x[i]); if (f > a) a = f; }
+    double amax = 0.0;
+    for (int i = 0; i < n; ++i) { double f = fabs(x[i]); if (f > amax) amax = f; }
+    float a = (float)amax;
     *scale = a;
     if (!(a > 0.0f)) { for (int i = 0; i < n; ++i) code[i] = 0; return; }
-    volatile float inv = 127.0f / a;
+    double s = (double)a / 127.0;
     for (int i = 0; i < n; ++i) {
-        double r = rint((double)(float)x[i] * (double)inv);
+        double r = rint(x[i] / s);
         if (r > 127.0) r = 127.0;
         if (r < -127.0) r = -127.0;
         code[i] = (int8_t)r;
     }
 }
 
-/* v >= 0: unsigned linear code in [0,255], scale a/255 (S5); "v is floored away from zero"
+/* v >= 0: unsigned linear code in [0,255], s = a/255 (S5); "v is floored away from zero"
  * (PAPER.md:316): in a block with a > 0 every code is at least 1 (S6). */
 void forge_oracle_quant_v_block(const double *x, int n, uint8_t *code, float *scale)
 {
-    float a = 0.0f;
-    for (int i = 0; i < n; ++i) { float f = fabsf((float)x[i]); if (f > a) a = f; }
+    double amax = 0.0;
+    for (int i = 0; i < n; ++i) { double f = fabs(x[i]); if (f > amax) amax = f; }
+    float a = (float)amax;
     *scale = a;
     if (!(a > 0.0f)) { for (int i = 0; i < n; ++i) code[i] = 0; return; }
-    volatile float inv = 255.0f / a;
+    double s = (double)a / 255.0;
     for (int i = 0; i < n; ++i) {
-        double r = rint((double)(float)x[i] * (double)inv);
+        double r = rint(x[i] / s);
         if (r > 255.0) r = 255.0;
         if (r < 1.0) r = 1.0;
         code[i] = (uint8_t)r;

@@ -157,10 +157,11 @@ void forge_oracle_accumulate(void *B, int state_bf16, const double *G, size_t n,
 /* ---------------------------------------------------------------- stochastic-rounding store --
  * The paper's "SR-store" recipe (1287-1296: "the bf16 weight is the only copy, committed by
  * stochastic rounding"; microcheck PAPER.md:1450 "dead zone, unbiasedness").  The paper gives no generator,
- * so both sides implement the same counter-based one (reading S16): 16 random bits per weight
- * element from (seed, step, stream, row, col) through the murmur3 finaliser; the decision is taken in the
- * kernel's precision: x = fp32(W'), out = (bits(x) + r16) >> 16, i.e. round away from zero with probability
- * (low 16 bits) / 65536 -- unbiased on the fp32 value.  Inf / NaN take the RNE path. */
+ * so both sides implement the same counter-based one (reading S16): 16 random bits r16 per weight
+ * element from (seed, step, stream, row, col) through the murmur3 finaliser, u = r16 / 65536 uniform on [0,1).
+ * The rounding itself is the textbook rule on the fp64 value W': with lo, hi its two bf16 neighbours (lo toward
+ * zero) and frac = (|W'| - lo) / (hi - lo), the store takes hi iff u >= 1 - frac, i.e. with probability frac
+ * (to the 2^-16 resolution of u) -- unbiased.  Inf / NaN take the RNE path. */
 static uint32_t fmix32(uint32_t h)
 {
     h ^= h >> 16; h *= 0x85EBCA6Bu; h ^= h >> 13; h *= 0xC2B2AE35u; h ^= h >> 16;
@@ -174,11 +175,23 @@ uint32_t forge_oracle_sr_bits(uint64_t seed, long step, uint32_t stream, uint32_
 }
 uint16_t forge_oracle_bf16_sr_from_double(double x, uint32_t r16)
 {
-    float f = (float)x;                                   /* the kernel's arithmetic type */
+    if (isnan(x) || isinf(x) || x == 0.0) return forge_oracle_bf16_from_double(x);
+    uint16_t sign = signbit(x) ? 0x8000u : 0u;
+    double a = fabs(x);
+    int e;
+    (void)frexp(a, &e);
+    int p = e - 1;
+    if (p < -126) p = -126;
+    double ulp = ldexp(1.0, p - 7);                        /* spacing of bf16 numbers around |x| */
+    double q = a / ulp;                                   /* exact (power of two) */
+    double fl = floor(q), frac = q - fl;                  /* exact */
+    if ((double)r16 + frac * 65536.0 >= 65536.0) fl += 1.0;
+    double r = fl * ulp;
+    if (r >= ldexp(1.0, 128)) return (uint16_t)(sign | 0x7F80u);
+    float rf = (float)r;                                  /* exact: r is a bf16 value */
     uint32_t b;
-    __builtin_memcpy(&b, &f, 4);
-    if ((b & 0x7F800000u) == 0x7F800000u) return forge_oracle_bf16_from_double(x);
-    return (uint16_t)((b + r16) >> 16);
+    __builtin_memcpy(&b, &rf, 4);
+    return (uint16_t)(sign | (uint16_t)(b >> 16));
 }
 
 /* AdamW (Algorithm 1) with fp32 moments and the SR store of W; W is [out, in]. */
@@ -207,13 +220,11 @@ void forge_oracle_adamw_fp32_sr(uint16_t *W, float *m, float *v, const double *G
  * codes of x / s with one fp32 scale s per tensor; DELAYED scaling: the scale in use was derived by the caller
  * from the amax the previous step reported (s = amax_prev / 448); this step reports its own amax of m', v'
  * for the next one.  Values beyond 448 s saturate (round-to-nearest-even, satfinite -- the hardware cvt).
- * The code decision is taken in the kernel's precision: code = e4m3(fp32(fp32(x) * fp32(1/s))). */
-uint8_t forge_oracle_e4m3_from_float(float t)
+ * code = e4m3(x / s) evaluated in fp64 from the fp64 moment and the stored fp32 scale; s = 0 stores code 0. */
+uint8_t forge_oracle_e4m3_from_double(double t)
 {
-    uint32_t b;
-    __builtin_memcpy(&b, &t, 4);
-    uint8_t sign = (uint8_t)((b >> 24) & 0x80u);
-    double a = fabs((double)t);
+    uint8_t sign = signbit(t) ? 0x80u : 0u;
+    double a = fabs(t);
     if (t != t) return (uint8_t)(sign | 0x7Fu);            /* NaN */
     if (a > 448.0) return (uint8_t)(sign | 0x7Eu);         /* satfinite (includes Inf) */
     if (a < 0.015625) {                                    /* below the smallest normal 2^-6: subnormal grid 2^-9 */
@@ -229,6 +240,7 @@ uint8_t forge_oracle_e4m3_from_float(float t)
     if (code > 0x7E) code = 0x7E;
     return (uint8_t)(sign | (uint8_t)code);
 }
+uint8_t forge_oracle_e4m3_from_float(float t) { return forge_oracle_e4m3_from_double((double)t); }
 double forge_oracle_e4m3_to_double(uint8_t c)
 {
     double s = (c & 0x80u) ? -1.0 : 1.0;
@@ -237,17 +249,16 @@ double forge_oracle_e4m3_to_double(uint8_t c)
     if (e == 0) return s * (double)q * 0.001953125;        /* q * 2^-9 */
     return s * (1.0 + (double)q / 8.0) * ldexp(1.0, e - 7);
 }
-static float fp8_inv_scale(float s) { volatile float r = (s > 0.0f) ? 1.0f / s : 0.0f; return r; }
+static double fp8_scaled(double x, float s) { return s > 0.0f ? x / (double)s : 0.0; }
 
-/* quantise one fp32 tensor: scale = amax / 448, codes as above */
+/* quantise one fp32 tensor: scale = amax / 448 stored as fp32, codes as above */
 void forge_oracle_fp8_quantize(const float *x, size_t n, uint8_t *code, float *scale)
 {
-    float amax = 0.0f;
-    for (size_t i = 0; i < n; ++i) { float a = fabsf(x[i]); if (a > amax) amax = a; }
-    volatile float s = amax / 448.0f;
+    double amax = 0.0;
+    for (size_t i = 0; i < n; ++i) { double a = fabs((double)x[i]); if (a > amax) amax = a; }
+    float s = (float)(amax / 448.0);
     *scale = s;
-    float inv = fp8_inv_scale(s);
-    for (size_t i = 0; i < n; ++i) { volatile float t = x[i] * inv; code[i] = forge_oracle_e4m3_from_float(t); }
+    for (size_t i = 0; i < n; ++i) code[i] = forge_oracle_e4m3_from_double(fp8_scaled((double)x[i], s));
 }
 
 /* AdamW (Algorithm 1) with e4m3 moments.  m_scale / v_scale: [0] = scale in use (read),
@@ -257,7 +268,6 @@ void forge_oracle_adamw_fp8(uint16_t *W, uint8_t *mq, uint8_t *vq, float *m_scal
 {
     const double b1 = beta1, b2 = beta2, bc1 = 1.0 - pow(b1, (double)step), bc2 = 1.0 - pow(b2, (double)step);
     const double sm = (double)m_scale[0], sv = (double)v_scale[0];
-    const float inv_m = fp8_inv_scale(m_scale[0]), inv_v = fp8_inv_scale(v_scale[0]);
     float am = m_scale[1], av = v_scale[1];
 #pragma omp parallel for schedule(static) reduction(max : am, av)
     for (size_t i = 0; i < n; ++i) {
@@ -266,9 +276,8 @@ void forge_oracle_adamw_fp8(uint16_t *W, uint8_t *mq, uint8_t *vq, float *m_scal
         double v1 = b2 * (forge_oracle_e4m3_to_double(vq[i]) * sv) + (1.0 - b2) * G[i] * G[i];
         double w1 = (1.0 - (double)lr * (double)wd) * w - (double)lr * (m1 / bc1) / (sqrt(v1 / bc2) + (double)eps);
         W[i] = forge_oracle_bf16_from_double(w1);
-        volatile float tm = (float)m1 * inv_m, tv = (float)v1 * inv_v;
-        mq[i] = forge_oracle_e4m3_from_float(tm);
-        vq[i] = forge_oracle_e4m3_from_float(tv);
+        mq[i] = forge_oracle_e4m3_from_double(fp8_scaled(m1, m_scale[0]));
+        vq[i] = forge_oracle_e4m3_from_double(fp8_scaled(v1, v_scale[0]));
         float fm = fabsf((float)m1), fv = fabsf((float)v1);
         if (fm > am) am = fm;
         if (fv > av) av = fv;

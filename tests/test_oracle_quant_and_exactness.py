@@ -83,6 +83,7 @@ def test_int8_step_consistent_with_fp32_step_on_dequantised_state():
     v = np.abs(rng.standard_normal((out, inn)) * 1e-6).astype(F)
     G = rng.standard_normal((out, inn)) * 1e-2
     mq, ms, vq, vs = fo.quantize(m, v)
+    mq_in, ms_in, vq_in, vs_in = mq.copy(), ms.copy(), vq.copy(), vs.copy()
     md0, vd0 = fo.dequantize_m(mq, ms), fo.dequantize_v(vq, vs)
     W1 = W0.copy()
     Wd1, md1, vd1 = fo.adamw_int8(W1, mq, vq, ms, vs, G, 10, *HP, debug=True)
@@ -96,6 +97,48 @@ def test_int8_step_consistent_with_fp32_step_on_dequantised_state():
     assert np.array_equal(mq, mq2) and np.array_equal(vq, vq2)
     assert np.array_equal(ms, ms2) and np.array_equal(vs, vs2)
     assert np.array_equal(W1, fo.f64_to_bf16(Wd1))
+    # and against an independent scale-index restatement: dequantise with numpy indexing, one coordinate at a time
+    bc1, bc2 = 1 - b1 ** 10, 1 - b2 ** 10
+    for (p_, q_) in [(0, 0), (3, 255), (3, 256), (7, 511), (5, 300)]:
+        mm = float(mq_in[p_, q_]) * (float(ms_in[p_, q_ // 256]) / 127.0)
+        vv = float(vq_in[p_, q_]) * (float(vs_in[p_, q_ // 256]) / 255.0)
+        m1 = b1 * mm + (1 - b1) * G[p_, q_]
+        v1 = b2 * vv + (1 - b2) * G[p_, q_] ** 2
+        w1 = (1 - lr * wd) * fo.bf16_to_f64(W0)[p_, q_] - lr * (m1 / bc1) / (np.sqrt(v1 / bc2) + eps)
+        assert abs(Wd1[p_, q_] - w1) <= 4e-16 * max(abs(w1), 1e-300) + 1e-18
+
+
+def test_int8_weight_equals_fp32_oracle_on_dequantised_state_bitwise():
+    """Pin of W' (and the unrounded m', v') of ``adamw_int8``: with block maxima 127 * 2^-20 (m) and 255 * 2^-30
+    (v) the steps a/127 and a/255 are powers of two, every dequantised moment is an fp32 number, and the
+    fp32-moment oracle -- pinned on its own against torch.optim.AdamW and the step-1 closed form -- can be fed
+    the dequantised state exactly.  Both must then agree on W bit for bit and on the fp64 W', m', v' exactly
+    (same update, only the storage differs).  A wrong scale index, a swapped m / v scale or a
+    missing dequantisation step fails here."""
+    rng = np.random.default_rng(131)
+    out, inn = 6, 768
+    W0 = rand_bf16(rng, (out, inn), 0.02)
+    am, av = 127.0 * 2.0 ** -20, 255.0 * 2.0 ** -30
+    m = np.clip(rng.standard_normal((out, inn)) * 3e-5, -0.99 * am, 0.99 * am)
+    v = np.clip(np.abs(rng.standard_normal((out, inn))) * 6e-8, 0, 0.99 * av)
+    # different maxima per block so that a wrong block index shows: block b of row p gets am * 2^-(p+b)
+    for p_ in range(out):
+        for b_ in range(inn // 256):
+            k = 2.0 ** -((p_ + b_) % 4)
+            m[p_, b_ * 256:(b_ + 1) * 256] *= k; v[p_, b_ * 256:(b_ + 1) * 256] *= k
+            m[p_, b_ * 256 + (7 * p_ + b_) % 256] = -am * k if (p_ + b_) % 2 else am * k
+            v[p_, b_ * 256 + (11 * p_ + 3 * b_) % 256] = av * k
+    G = rng.standard_normal((out, inn)) * 1e-2
+    mq, ms, vq, vs = fo.quantize(m, v)
+    md0, vd0 = fo.dequantize_m(mq, ms), fo.dequantize_v(vq, vs)
+    mf, vf = md0.astype(F), vd0.astype(F)
+    assert np.array_equal(mf.astype(np.float64), md0) and np.array_equal(vf.astype(np.float64), vd0)
+    assert len(np.unique(ms)) == 4 and len(np.unique(vs)) == 4
+    W1, Wf = W0.copy(), W0.copy()
+    Wd1, md1, vd1 = fo.adamw_int8(W1, mq, vq, ms, vs, G, 10, *HP, debug=True)
+    Wdf, mdf, vdf = fo.adamw_fp32(Wf, mf, vf, G, 10, *HP, debug=True)
+    assert np.array_equal(W1, Wf)
+    assert np.array_equal(Wd1, Wdf) and np.array_equal(md1, mdf) and np.array_equal(vd1, vdf)
 
 
 def test_prop1_tile_by_tile_equals_one_shot_bitwise():
