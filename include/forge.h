@@ -21,12 +21,21 @@
  *     PAPER.md:74 Alg. 1 line 1; PAPER.md:296 Remark 2).
  *   - a weight with more than one backward consumer (tied embedding / LM head) must not be passed
  *     (PAPER.md:296).
- *   - W, m, v, scales do not overlap each other or X, dY; problems of one group have disjoint state.
+ * Aliasing (enforced): inside one call no updated tensor (W, m, v, scales, dX, G) may overlap any other tensor the
+ * call touches, within a problem or across the problems of a group; read-only operands may be shared (q / k / v read
+ * one X).  A violation returns FORGE_ERR_BAD_SHAPE before anything is enqueued.
  *
- * Error behaviour: every argument of every problem is validated before anything is enqueued, so a
- * non-OK return means no state was touched.  No exceptions cross this boundary.  NaN/Inf in the
- * inputs propagate by IEEE rules.  There is no CPU or library fallback: a device that is not
- * compute capability 10.x returns FORGE_ERR_UNSUPPORTED_ARCH.
+ * Error behaviour: every argument of every problem is validated, every tensor map of every launch the call needs is
+ * encoded and every kernel attribute is set BEFORE the first launch is enqueued, so a status other than FORGE_ERR_CUDA
+ * means no state was touched.  FORGE_ERR_CUDA can only come from a launch itself; when the call needed several
+ * launches (more than 8 problems, or forge_layer_backward_grouped's dgrad + update) the earlier ones have then been
+ * enqueued.  No exceptions cross this boundary.  NaN/Inf in the inputs propagate by IEEE rules (to the rows / columns
+ * of G they enter and nowhere else).  There is no CPU or library fallback: a device that is not compute capability
+ * 10.x returns FORGE_ERR_UNSUPPORTED_ARCH.
+ *
+ * Environment: the library reads no environment variable.  The tuning / profiling switches FORGE_CFG, FORGE_GRID,
+ * FORGE_ABLATE and FORGE_HOST_SLICE_MB exist only in the separate -DFORGE_PROFILING build (libforge_b200_prof.so)
+ * that the commands quoted under profiles/ load.
  */
 #ifndef FORGE_H_
 #define FORGE_H_
@@ -98,10 +107,6 @@ typedef struct {
     int64_t ldx, lddy;
 } forge_problem_t;
 
-/* Environment: FORGE_POWER_STATE=boost|capped overrides the library's own estimate of whether a launch will run under
- * the board's power cap (it picks between two bit-identical instantiations of the fp32-moment kernel; DESIGN.md section
- * 6).  FORGE_CFG / FORGE_GRID / FORGE_ABLATE / FORGE_HOST_SLICE_MB are tuning and profiling switches (profiles/). */
-
 /* Fused weight gradient + AdamW step for one layer (Algorithm 1).
  * `step` is the 1-based index t of the update being applied (bias terms 1-beta^t); step < 1,
  * lr < 0 or non-finite, beta outside [0,1), eps < 0, wd < 0 -> FORGE_ERR_BAD_HYPERPARAM. */
@@ -152,13 +157,14 @@ forge_status_t forge_wgrad_adamw_sr_grouped(const forge_problem_t *problems, int
                                            forge_moment_dtype_t moment_dtype, uint64_t seed, forge_stream_t stream);
 
 /* One layer's backward for the linear weights in ONE call (Alg. 1 line 1 + lines 2-11): first the
- * input gradients dX[i][T,in] = dY_i . W_i (bf16, fp32 accumulate; a plain library GEMM -- cuBLAS, as in the paper)
- * from the PRE-update weights, then, stream-ordered behind every one of them, the fused weight-gradient + AdamW
- * step that overwrites W in place.  This closes the ordering hazard forge_wgrad_adamw leaves to the caller
- * (296 Remark 2).  dX is a HOST array of `count` device pointers, one output per problem (the
- * caller sums the dX of projections that share an input).  cuBLAS keeps its own small workspace; no
- * gradient-shaped buffer is allocated.  Validation and errors as forge_wgrad_adamw_grouped; nothing is enqueued
- * on a non-OK return. */
+ * input gradients dX[i][T,in] = dY_i . W_i (bf16 output, fp32 accumulation in tensor memory) from the PRE-update
+ * weights -- a hand-written tcgen05 kernel (csrc/dgrad_kernel.cuh; A = dY K-major, B = W MN-major, CTA pairs, tiles of
+ * all problems assigned longest-first), one launch per 8 problems -- then, stream-ordered behind it, the fused
+ * weight-gradient + AdamW launch that overwrites W in place.  This closes the ordering hazard forge_wgrad_adamw leaves
+ * to the caller (296 Remark 2).  dX is a HOST array of `count` device pointers, one dense [T,in] output
+ * per problem (the caller sums the dX of projections that share an input); it may not overlap any other tensor of the
+ * call.  No library GEMM and no gradient-shaped buffer is involved.  Validation and errors as
+ * forge_wgrad_adamw_grouped. */
 forge_status_t forge_layer_backward_grouped(const forge_problem_t *problems, void *const *dX, int32_t count,
                                             int64_t step, float lr, float beta1, float beta2, float eps, float wd,
                                             forge_moment_dtype_t moment_dtype, forge_stream_t stream);
@@ -221,6 +227,10 @@ size_t forge_workspace_bytes(void);
 uint64_t forge_launch_count(void);
 /* Detail of the last CUDA error seen by this library (cudaError_t value), 0 if none. */
 int forge_last_cuda_error(void);
+/* Name and template arguments of the kernel instantiation the most recent launch of this library used, as a profiler
+ * prints it (e.g. "forge_fused_kernel<0, 0, 32, 4, 2, 2, 64, 128, 128, 2, 2, 2>"); "" before the first launch.
+ * bench.py uses it to match its launches with the committed ncu captures under profiles/. */
+const char *forge_last_kernel(void);
 const char *forge_status_string(forge_status_t status);
 int forge_version(void);
 

@@ -23,7 +23,7 @@ STATUS_NAMES = ["FORGE_OK", "FORGE_ERR_NULL_PTR", "FORGE_ERR_BAD_SHAPE", "FORGE_
                 "FORGE_ERR_CUDA"]
 EXPORTS = ["forge_wgrad_adamw", "forge_wgrad_adamw_grouped", "forge_wgrad_step_grouped", "forge_wgrad_accumulate_grouped", "forge_layer_backward_grouped", "forge_wgrad_adamw_sr_grouped", "forge_wgrad_adamw_host", "forge_wgrad_adamw_grouped_host",
            "forge_wgrad_store_g", "forge_wgrad_store_g_grouped", "forge_adamw_from_g", "forge_workspace_bytes", "forge_launch_count",
-           "forge_last_cuda_error", "forge_status_string", "forge_version"]
+           "forge_last_cuda_error", "forge_last_kernel", "forge_status_string", "forge_version"]
 
 
 class ForgeError(RuntimeError):
@@ -49,16 +49,28 @@ FAMILIES = {"adamw": 0, "sgd": 1, "momentum": 2, "lion": 3, "rmsprop": 4, "adagr
 FAMILY_STATES = {"adamw": 2, "sgd": 0, "momentum": 1, "lion": 1, "rmsprop": 1, "adagrad": 1, "adamax": 2, "nadam": 2, "radam": 2}
 
 _lib = None
+_libs = {}
+_profiling = False
+
+
+def use_profiling_library(on: bool) -> None:
+    """Route every call of this module through libforge_b200_prof.so (the -DFORGE_PROFILING build: FORGE_CFG /
+    FORGE_GRID / FORGE_ABLATE are honoured there and nowhere else).  For profiles/ commands and two tests only."""
+    global _lib, _profiling
+    _profiling = bool(on)
+    _lib = None
 
 
 def lib() -> ctypes.CDLL:
     """Load libforge_b200.so (built in-tree by build.build()); raises if it cannot be loaded."""
     global _lib
+    if _lib is None and _profiling in _libs:
+        _lib = _libs[_profiling]
     if _lib is None:
-        path = _build.LIB_PATH
+        path = _build.PROF_LIB_PATH if _profiling else _build.LIB_PATH
         if not os.path.exists(path):
-            raise FileNotFoundError(f"{path} not built: run `python -m paper_2606_22932_b200.build` "
-                                    "(there is no fallback path)")
+            raise FileNotFoundError(f"{path} not built: run `python -m paper_2606_22932_b200.build"
+                                    f"{' --profiling' if _profiling else ''}` (there is no fallback path)")
         L = ctypes.CDLL(path)
         hp = [c_int64, c_float, c_float, c_float, c_float, c_float]
         L.forge_wgrad_adamw.restype = ctypes.c_int
@@ -89,9 +101,11 @@ def lib() -> ctypes.CDLL:
         L.forge_workspace_bytes.restype = ctypes.c_size_t
         L.forge_launch_count.restype = ctypes.c_uint64
         L.forge_last_cuda_error.restype = ctypes.c_int
+        L.forge_last_kernel.restype = ctypes.c_char_p
         L.forge_status_string.restype = ctypes.c_char_p
         L.forge_status_string.argtypes = [ctypes.c_int]
         L.forge_version.restype = ctypes.c_int
+        _libs[_profiling] = L
         _lib = L
     return _lib
 

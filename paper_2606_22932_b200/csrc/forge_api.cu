@@ -1,19 +1,21 @@
 // forge_api.cu -- the C ABI of include/forge.h: argument validation, host-side scalars, tensor-map
 // construction and kernel launches.  Allocates no device memory (except the scratch of the
 // explicitly host-buffer entry point forge_wgrad_adamw_host, freed before it returns).
+#include <algorithm>
 #include <atomic>
-#include <chrono>
 #include <cmath>
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
 #include <mutex>
+#include <string>
+#include <vector>
 
-#include <cublas_v2.h>
 #include <cuda.h>
 #include <cuda_runtime.h>
 
 #include "../../include/forge.h"
+#include "dgrad_kernel.cuh"
 #include "elementwise_kernel.cuh"
 #include "fused_kernel.cuh"
 
@@ -23,6 +25,7 @@ using namespace forge;
 
 std::atomic<uint64_t> g_launches{0};
 std::atomic<int> g_last_cuda_error{0};
+std::atomic<const char *> g_last_kernel{""};     // signature of the instantiation the last launch used (forge_last_kernel)
 
 forge_status_t cuda_fail(cudaError_t e) {
     g_last_cuda_error.store(static_cast<int>(e));
@@ -103,18 +106,68 @@ forge_status_t validate_state(const void *W, const void *m, const void *v, const
     return FORGE_OK;
 }
 
-forge_status_t validate_problem(const forge_problem_t &p, int mdt) {
+// the two GEMM operands: pointers, token count, pitches, alignment (every entry point goes through this)
+forge_status_t validate_operands(const forge_problem_t &p) {
     if (!p.X || !p.dY) return FORGE_ERR_NULL_PTR;
-    forge_status_t s = validate_state(p.W, p.m, p.v, p.m_scale, p.v_scale, p.out, p.in, mdt);
-    if (s != FORGE_OK) return s;
-    if (p.T < 1) return FORGE_ERR_BAD_SHAPE;
+    if (p.T < 1 || p.out < 8 || p.in < 8 || (p.out % 8) != 0 || (p.in % 8) != 0) return FORGE_ERR_BAD_SHAPE;
     if (p.ldx != 0 && (p.ldx < p.in || p.ldx % 8 != 0)) return FORGE_ERR_BAD_SHAPE;
     if (p.lddy != 0 && (p.lddy < p.out || p.lddy % 8 != 0)) return FORGE_ERR_BAD_SHAPE;
     if (!aligned16(p.X) || !aligned16(p.dY)) return FORGE_ERR_ALIGNMENT;
     return FORGE_OK;
 }
+forge_status_t validate_problem(const forge_problem_t &p, int mdt) {
+    if (!p.X || !p.dY) return FORGE_ERR_NULL_PTR;
+    forge_status_t s = validate_state(p.W, p.m, p.v, p.m_scale, p.v_scale, p.out, p.in, mdt);
+    if (s != FORGE_OK) return s;
+    return validate_operands(p);
+}
 bool dense_operands(const forge_problem_t &p) {
     return (p.ldx == 0 || p.ldx == p.in) && (p.lddy == 0 || p.lddy == p.out);
+}
+
+// Aliasing (forge.h "Caller's obligations"): inside one call no updated tensor may overlap any other tensor the call
+// touches -- overlapping state inside a group is a silent race between CTAs.  Read-only operands may be shared
+// (q / k / v read one X).  Sort-and-sweep over the byte intervals, O(n log n) in the number of tensors.
+struct Interval {
+    uintptr_t lo, hi;
+    bool written;
+};
+void add_interval(std::vector<Interval> &iv, const void *p, size_t bytes, bool written) {
+    if (p && bytes) iv.push_back({reinterpret_cast<uintptr_t>(p), reinterpret_cast<uintptr_t>(p) + bytes, written});
+}
+size_t moment_bytes(int mdt) { return mdt == FORGE_MOMENT_FP32 ? 4 : (mdt == FORGE_MOMENT_BF16 ? 2 : 1); }
+// every tensor of a problem: operands read-only, everything else written (absent tensors are NULL and skipped)
+void add_problem_intervals(std::vector<Interval> &iv, const forge_problem_t &p, int mdt, size_t m_elem_bytes) {
+    const size_t n = static_cast<size_t>(p.out) * p.in;
+    const size_t ldx = p.ldx ? p.ldx : p.in, lddy = p.lddy ? p.lddy : p.out;
+    add_interval(iv, p.X, ((static_cast<size_t>(p.T) - 1) * ldx + p.in) * 2, false);
+    add_interval(iv, p.dY, ((static_cast<size_t>(p.T) - 1) * lddy + p.out) * 2, false);
+    add_interval(iv, p.W, n * 2, true);
+    add_interval(iv, p.m, n * m_elem_bytes, true);
+    add_interval(iv, p.v, n * m_elem_bytes, true);
+    const size_t sb = mdt == FORGE_MOMENT_INT8 ? n / FORGE_QBLOCK * 4 : (mdt == FORGE_MOMENT_FP8 ? 2 * sizeof(float) : 0);
+    add_interval(iv, p.m_scale, sb, true);
+    add_interval(iv, p.v_scale, sb, true);
+}
+forge_status_t check_disjoint(std::vector<Interval> &iv) {
+    std::sort(iv.begin(), iv.end(), [](const Interval &a, const Interval &b) { return a.lo < b.lo; });
+    uintptr_t end_any = 0, end_written = 0;
+    for (const Interval &x : iv) {
+        if (x.lo < end_written || (x.written && x.lo < end_any)) return FORGE_ERR_BAD_SHAPE;
+        end_any = std::max(end_any, x.hi);
+        if (x.written) end_written = std::max(end_written, x.hi);
+    }
+    return FORGE_OK;
+}
+forge_status_t validate_disjoint(const forge_problem_t *probs, int count, int mdt, size_t m_elem_bytes,
+                                 void *const *extra_out = nullptr, const size_t *extra_bytes = nullptr) {
+    std::vector<Interval> iv;
+    iv.reserve(static_cast<size_t>(count) * 8);
+    for (int i = 0; i < count; ++i) {
+        add_problem_intervals(iv, probs[i], mdt, m_elem_bytes);
+        if (extra_out) add_interval(iv, extra_out[i], extra_bytes[i], true);
+    }
+    return check_disjoint(iv);
 }
 
 // Alg. 1 line 9 bias terms and the folded constants, computed in double from the float
@@ -136,6 +189,7 @@ AdamWScalars make_scalars(int64_t step, float lr, float b1, float b2, float eps,
 
 struct DeviceInfo {
     int device = -1, sm_count = 0, cc_major = 0;
+    bool dry = false;   // encode every tensor map and set every function attribute, launch nothing (see for_each_launch)
 };
 forge_status_t device_info(DeviceInfo &d) {
     cudaError_t e = cudaGetDevice(&d.device);
@@ -148,9 +202,31 @@ forge_status_t device_info(DeviceInfo &d) {
     return FORGE_OK;
 }
 
+// The tuning / ablation switches FORGE_CFG, FORGE_GRID, FORGE_ABLATE, FORGE_HOST_SLICE_MB exist only in the
+// -DFORGE_PROFILING build (libforge_b200_prof.so, loaded by the profiles/ commands and two tests).  The product
+// library reads no environment variable: nothing left over in a shell can change a launch or a result.
+#ifdef FORGE_PROFILING
 int env_int(const char *name, int dflt) {
     const char *s = std::getenv(name);
     return s ? std::atoi(s) : dflt;
+}
+#else
+constexpr int env_int(const char *, int dflt) { return dflt; }
+#endif
+
+// A group of more than kMaxProblems problems takes several launches.  All of them are prepared (tensor maps encoded,
+// function attributes set) in a dry pass BEFORE the first one is enqueued, so that the only failure left once state
+// has been touched is a launch failure itself.  f(first, n, dev) prepares or launches problems [first, first + n).
+template <class F>
+forge_status_t for_each_launch(int count, DeviceInfo dev, F f) {
+    for (int pass = (count > kMaxProblems ? 0 : 1); pass < 2; ++pass) {
+        dev.dry = (pass == 0);
+        for (int i = 0; i < count; i += kMaxProblems) {
+            const forge_status_t s = f(i, std::min(count - i, kMaxProblems), dev);
+            if (s != FORGE_OK) return s;
+        }
+    }
+    return FORGE_OK;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -223,11 +299,12 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
     }
     P.total_tiles = tiles;
     P.sr_seed_lo = static_cast<uint32_t>(sr_seed);
-    P.debug = env_int("FORGE_ABLATE", 0);          // profiling ablations only (profiles/): results are wrong when set
+    P.debug = env_int("FORGE_ABLATE", 0);          // FORGE_PROFILING build only (constant 0 otherwise)
     int grid = dev.sm_count / CG;                  // persistent: one CTA (or CTA pair) per SM (pair)
-    const int forced = env_int("FORGE_GRID", 0);   // debug/determinism tests only
+    const int forced = env_int("FORGE_GRID", 0);   // FORGE_PROFILING build only: determinism test across grid sizes
     if (forced > 0) grid = (forced + CG - 1) / CG;
     if (grid > tiles) grid = tiles;
+    if (dev.dry) return FORGE_OK;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(grid * CG));
     cfg.blockDim = dim3(block_threads(MDT, NWG));
@@ -244,6 +321,13 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
     if (e == cudaSuccess) e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
     g_launches.fetch_add(1);
+    static const std::string sig = [] {
+        const int a[12] = {MDT, MODE, BK, ST, SS, CG, CM, CN, P1C, P1S, NST, NWG};
+        std::string t = "forge_fused_kernel<";
+        for (int i = 0; i < 12; ++i) t += std::to_string(a[i]) + (i < 11 ? ", " : ">");
+        return t;
+    }();
+    g_last_kernel.store(sig.c_str());
     return FORGE_OK;
 }
 
@@ -251,62 +335,13 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
 // PAPER.md:706-710 App. H; here the choice is fixed per moment dtype and token count):
 //   small T : HBM-bound -> short token chunks, state ring as deep as shared memory allows
 //   large T : tensor-bound -> 64-token chunks, 4-stage operand ring, shallow state ring
+//   T >= 8192 (fp32 / bf16 moments): the ring-less direct state path, all shared memory to the operand ring
+//   (gate_proj: T = 8192 direct 741-770 us vs ring 770-784; T = 4096 direct 469 vs ring 446; T = 2048 320 vs 274)
 // Template arguments: <moments, mode, token chunk, operand stages, state stages, CTA group, chunk rows, chunk cols>.
-// FORGE_CFG selects the other instantiations for tuning sweeps and the determinism tests only.
-int pick_variant(int maxT) {
-    const int forced = env_int("FORGE_CFG", -1);   // debug only
-    // T >= 8192 (fp32 / bf16 moments): the ring-less direct state path, all shared memory to the operand ring
-    // (gate_proj: T = 8192 direct 741-770 us vs ring 770-784; T = 4096 direct 469 vs ring 446; T = 2048 320 vs 274)
-    return forced >= 0 ? forced : (maxT >= 8192 ? 30 : (maxT > 1024 ? 5 : 0));
-}
+enum : int { V_SMALL_T = 0, V_LARGE_T = 5, V_DIRECT = 30 };
+int pick_variant(int maxT) { return maxT >= 8192 ? V_DIRECT : (maxT > 1024 ? V_LARGE_T : V_SMALL_T); }
 
-// Power state.  K back-to-back launches of tens of milliseconds run at the boost clock; after about 0.1 s of continuous
-// load the board reaches its power cap and the SM clock falls by 13-25 % (profiles/r01_summary.md, "Power state").  With
-// fp32 moments the two chunk shapes trade places across that line: 64 x 128 chunks give 730 us / layer at the boost
-// clock and 790 under the cap, 128 x 64 chunks (3 operand stages) 752 and 741.  The library cannot see the clock, so it
-// keeps a simple model of its own load per device: every launch adds its estimated duration to a "heat" that idle time
-// (no launch of ours queued) removes one for one; above kHotMs the launch is expected to execute under the cap.  The
-// instantiations are bit-identical (same token order in the accumulator, same per-element arithmetic), so the switch
-// is invisible in the results.  FORGE_POWER_STATE=boost|capped overrides the model (other GPU work is invisible to it).
-constexpr double kHotMs = 70.0, kHeatMaxMs = 400.0;
-struct LoadModel {
-    std::mutex mu;
-    double busy_until_ms = 0.0, heat_ms = 0.0;
-};
-LoadModel g_load[64];
-
-bool expect_power_cap(int device, double est_ms) {
-    const char *forced = std::getenv("FORGE_POWER_STATE");
-    const double now = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now().time_since_epoch()).count();
-    LoadModel &L = g_load[device & 63];
-    std::lock_guard<std::mutex> lock(L.mu);
-    if (now > L.busy_until_ms) {
-        L.heat_ms -= now - L.busy_until_ms;
-        if (L.heat_ms < 0.0) L.heat_ms = 0.0;
-        L.busy_until_ms = now;
-    }
-    const bool hot = L.heat_ms > kHotMs;            // the state this launch will START in
-    L.busy_until_ms += est_ms;
-    L.heat_ms = L.heat_ms + est_ms < kHeatMaxMs ? L.heat_ms + est_ms : kHeatMaxMs;
-    if (forced && forced[0] == 'b') return false;
-    if (forced && forced[0] == 'c') return true;
-    return hot;
-}
-
-// estimated duration of one grouped launch: the slower of its HBM and tensor terms at 90 % of nominal rates
-double estimate_ms(const forge_problem_t *probs, int count, int mdt) {
-    const double state_b = mdt == FORGE_MOMENT_FP32 ? 20.0 : (mdt == FORGE_MOMENT_BF16 ? 12.0 : 8.0);
-    double bytes = 0.0, flops = 0.0;
-    for (int i = 0; i < count; ++i) {
-        const double n = static_cast<double>(probs[i].out) * probs[i].in;
-        bytes += n * state_b + 2.0 * probs[i].T * (static_cast<double>(probs[i].out) + probs[i].in);
-        flops += 2.0 * n * probs[i].T;
-    }
-    const double t_hbm = bytes / 5.8e9, t_tc = flops / 1.3e12;      // ms
-    return t_hbm > t_tc ? t_hbm : t_tc;
-}
-
-// The direct state path (variants >= 30) moves 16 columns per thread with 32-byte accesses: every row must be a
+// The direct state path moves 16 columns per thread with 32-byte accesses: every row must be a
 // whole number of such vectors and every base 32-byte aligned; anything else takes the TMA ring.
 bool direct_ok(const forge_problem_t *probs, int count) {
     for (int i = 0; i < count; ++i) {
@@ -317,109 +352,43 @@ bool direct_ok(const forge_problem_t *probs, int count) {
     return true;
 }
 
-forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, const AdamWScalars &hp,
-                              const DeviceInfo &dev, cudaStream_t stream) {
+int max_tokens(const forge_problem_t *probs, int count) {
     int maxT = 0;
     for (int i = 0; i < count; ++i) maxT = probs[i].T > maxT ? probs[i].T : maxT;
-    int variant = pick_variant(maxT);
-    if (variant >= 30 && (!direct_ok(probs, count) || mdt > FORGE_MOMENT_BF16)) variant = maxT > 1024 ? 5 : 0;
-    const bool capped = expect_power_cap(dev.device, estimate_ms(probs, count, mdt));
-    if (capped && variant == 0 && mdt == FORGE_MOMENT_FP32 && env_int("FORGE_CFG", -1) < 0) variant = 17;
+    return maxT;
+}
+
+forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, const AdamWScalars &hp,
+                              const DeviceInfo &dev, cudaStream_t stream) {
+    int variant = pick_variant(max_tokens(probs, count));
+    if (variant == V_DIRECT && (!direct_ok(probs, count) || mdt > FORGE_MOMENT_BF16)) variant = V_LARGE_T;
+#ifdef FORGE_PROFILING
+    if (env_int("FORGE_CFG", -1) >= 0) {
+        variant = env_int("FORGE_CFG", -1);
+        switch (mdt) {
+#include "profiling_variants.inc"
+        default: break;
+        }
+    }
+#endif
     switch (mdt) {
     case FORGE_MOMENT_FP32:
-        switch (variant) {
-        case 1: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 3, 2, 1, 64, 64>(probs, count, hp, dev, stream);
-        case 2: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 4, 2, 128, 32>(probs, count, hp, dev, stream);
-        case 3: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 4, 2, 32, 128>(probs, count, hp, dev, stream);
-        case 4: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 2, 4, 2, 64, 64>(probs, count, hp, dev, stream);
         // T > 1024: 128 KB operand ring; the 80 KB left for the state go further as 4 x 20 KB (32 x 64) than as 2 x 40 KB
-        case 5: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 4, 4, 2, 32, 64>(probs, count, hp, dev, stream);
-        case 14: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 4, 2, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 6: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 7: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 2, 2, 128, 64>(probs, count, hp, dev, stream);
-        case 8: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 8, 2, 64, 32>(probs, count, hp, dev, stream);
-        case 9: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 8, 2, 32, 64>(probs, count, hp, dev, stream);
-        case 10: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 2, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 12: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 4, 4, 2, 64, 32>(probs, count, hp, dev, stream);
-        case 13: return launch_fused<MDT_FP32, MODE_ADAMW, 128, 2, 2, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 15: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 2, 2, 64, 128, 128, 2, 2, 4>(probs, count, hp, dev, stream);
-        case 30: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 6, 0, 2, 64, 128>(probs, count, hp, dev, stream);
-        case 31: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 4, 0, 2, 64, 128>(probs, count, hp, dev, stream);
-        case 32: return launch_fused<MDT_FP32, MODE_ADAMW, 128, 3, 0, 2, 64, 128>(probs, count, hp, dev, stream);
-        case 33: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 7, 0, 2, 64, 128>(probs, count, hp, dev, stream);
-        case 34: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 12, 0, 2, 64, 128>(probs, count, hp, dev, stream);
-        case 35: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 5, 0, 2, 64, 128>(probs, count, hp, dev, stream);
-        case 16: return launch_fused<MDT_FP32, MODE_ADAMW, 64, 2, 2, 2, 128, 64>(probs, count, hp, dev, stream);
-        case 17: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 3, 2, 2, 128, 64>(probs, count, hp, dev, stream);
-        case 18: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 3, 2, 2, 64, 128>(probs, count, hp, dev, stream);
-        case 19: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 2, 2, 2, 64, 128>(probs, count, hp, dev, stream);
-        case 20: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 2, 2, 2, 128, 64>(probs, count, hp, dev, stream);
-        case 21: return launch_fused<MDT_FP32, MODE_ADAMW, 16, 6, 2, 2, 128, 64>(probs, count, hp, dev, stream);
-        case 22: return launch_fused<MDT_FP32, MODE_ADAMW, 16, 4, 2, 2, 128, 64>(probs, count, hp, dev, stream);
-        default: return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 2, 2, 64, 128>(probs, count, hp, dev, stream);
-        }
+        if (variant == V_DIRECT) return launch_fused<MDT_FP32, MODE_ADAMW, 64, 6, 0, 2, 64, 128>(probs, count, hp, dev, stream);
+        if (variant == V_LARGE_T) return launch_fused<MDT_FP32, MODE_ADAMW, 64, 4, 4, 2, 32, 64>(probs, count, hp, dev, stream);
+        return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 2, 2, 64, 128>(probs, count, hp, dev, stream);
     case FORGE_MOMENT_BF16:
-        switch (variant) {
-        case 1: return launch_fused<MDT_BF16, MODE_ADAMW, 64, 3, 2, 1, 64, 64>(probs, count, hp, dev, stream);
-        case 2: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 6, 2, 128, 32>(probs, count, hp, dev, stream);
-        case 3: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 2, 4, 2, 64, 128>(probs, count, hp, dev, stream);
-        case 4: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 2, 4, 2, 32, 256>(probs, count, hp, dev, stream);
-        case 5: return launch_fused<MDT_BF16, MODE_ADAMW, 64, 4, 2, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 6: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 6, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 7: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 2, 2, 64, 128>(probs, count, hp, dev, stream);
-        case 8: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 4, 2, 32, 128>(probs, count, hp, dev, stream);
-        case 10: return launch_fused<MDT_BF16, MODE_ADAMW, 64, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 11: return launch_fused<MDT_BF16, MODE_ADAMW, 64, 3, 4, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 12: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 6, 4, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 9: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 2, 8, 2, 32, 128>(probs, count, hp, dev, stream);
-        case 13: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 2, 2, 128, 64>(probs, count, hp, dev, stream);
-        case 30: return launch_fused<MDT_BF16, MODE_ADAMW, 64, 6, 0, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 14: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 3, 2, 128, 64>(probs, count, hp, dev, stream);
-        case 15: return launch_fused<MDT_BF16, MODE_ADAMW, 64, 4, 2, 2, 128, 64>(probs, count, hp, dev, stream);
-        case 16: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 2, 2, 2, 128, 128>(probs, count, hp, dev, stream);
-        default: return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
-        }
+        if (variant == V_DIRECT) return launch_fused<MDT_BF16, MODE_ADAMW, 64, 6, 0, 2, 64, 64>(probs, count, hp, dev, stream);
+        if (variant == V_LARGE_T) return launch_fused<MDT_BF16, MODE_ADAMW, 64, 4, 2, 2, 64, 64>(probs, count, hp, dev, stream);
+        return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
     case FORGE_MOMENT_INT8:
-        switch (variant) {
-        case 1: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 2, 2, 1, 128, 64>(probs, count, hp, dev, stream);
-        case 2: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 3, 2, 128, 64>(probs, count, hp, dev, stream);
-        case 3: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 4, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
-        case 4: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 2, 4, 2, 128, 64, 64, 3>(probs, count, hp, dev, stream);
-        case 5: return launch_fused<MDT_INT8, MODE_ADAMW, 64, 2, 2, 2, 128, 64>(probs, count, hp, dev, stream);
-        case 8: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 5, 2, 2, 128, 64>(probs, count, hp, dev, stream);
-        case 6: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 2, 2, 128, 64, 64, 4>(probs, count, hp, dev, stream);
-        case 7: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 4, 2, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
-        case 9: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 3, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
-        case 10: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 4, 3, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
-        case 11: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 3, 2, 128, 64, 64, 4>(probs, count, hp, dev, stream);
-        case 13: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 5, 3, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
-        case 14: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 6, 2, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
-        case 15: return launch_fused<MDT_INT8, MODE_ADAMW, 64, 3, 2, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
-        case 16: return launch_fused<MDT_INT8, MODE_ADAMW, 64, 2, 3, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
-        case 17: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 3, 2, 2, 128, 64>(probs, count, hp, dev, stream);
         // measured (us / layer): 3 state slots + 80 KB operand ring + 64-column first-pass chunks 420; 3 slots + 48 KB ring 437;
         // 2 slots 457-489 whatever the operand ring; 4 slots + 48 KB ring 442 (profiles/r01_summary.md)
-        default: return launch_fused<MDT_INT8, MODE_ADAMW, 32, 5, 3, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
-        }
+        if (variant == V_LARGE_T) return launch_fused<MDT_INT8, MODE_ADAMW, 64, 2, 2, 2, 128, 64>(probs, count, hp, dev, stream);
+        return launch_fused<MDT_INT8, MODE_ADAMW, 32, 5, 3, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
     case FORGE_MOMENT_FP8:
-        switch (variant) {
-        case 1: return launch_fused<MDT_FP8, MODE_ADAMW, 32, 4, 4, 2, 64, 128>(probs, count, hp, dev, stream);
-        case 2: return launch_fused<MDT_FP8, MODE_ADAMW, 32, 4, 8, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 3: return launch_fused<MDT_FP8, MODE_ADAMW, 32, 4, 4, 2, 32, 128>(probs, count, hp, dev, stream);
-        case 5: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 6: return launch_fused<MDT_FP8, MODE_ADAMW, 32, 8, 4, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 7: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 6, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 8: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 8, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 9: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 4, 6, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 10: return launch_fused<MDT_FP8, MODE_ADAMW, 32, 6, 6, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 11: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 4, 2, 64, 128>(probs, count, hp, dev, stream);
-        case 12: return launch_fused<MDT_FP8, MODE_ADAMW, 32, 4, 6, 2, 64, 64>(probs, count, hp, dev, stream);
-        case 13: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 4, 2, 128, 64>(probs, count, hp, dev, stream);
-        case 14: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 2, 2, 128, 128>(probs, count, hp, dev, stream);
-        case 15: return launch_fused<MDT_FP8, MODE_ADAMW, 32, 4, 4, 2, 128, 64>(probs, count, hp, dev, stream);
         // 8 B/element of state: the T = 512 mainloop needs the deeper operand ring (96 KB) more than the state ring does
-        default: return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 4, 2, 64, 128>(probs, count, hp, dev, stream);
-        }
+        return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 4, 2, 64, 128>(probs, count, hp, dev, stream);
     default:
         return FORGE_ERR_BAD_DTYPE;
     }
@@ -507,42 +476,107 @@ FamilyScalars make_family(const forge_opt_desc_t &o) {
 template <int MDT>
 forge_status_t dispatch_family(const forge_problem_t *probs, int count, int nst, const FamilyScalars &fs,
                                const DeviceInfo &dev, cudaStream_t stream) {
-    int maxT = 0;
-    for (int i = 0; i < count; ++i) maxT = probs[i].T > maxT ? probs[i].T : maxT;
     AdamWScalars hp;
     std::memset(&hp, 0, sizeof(hp));
-    const bool big = maxT > 1024;
-    const int forced = env_int("FORGE_CFG", -1);   // tuning sweeps only
+    const bool big = max_tokens(probs, count) > 1024;
     if (nst == 0) {
         if (big) return launch_fused<MDT, MODE_FAMILY, 64, 4, 4, 2, 64, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
-        if (forced == 1) return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 128, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
-        if (forced == 2) return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 64, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
-        if (forced == 3) return launch_fused<MDT, MODE_FAMILY, 32, 4, 2, 2, 128, 256, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
-        if (forced == 4) return launch_fused<MDT, MODE_FAMILY, 64, 4, 6, 2, 64, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
-        if (forced == 5) return launch_fused<MDT, MODE_FAMILY, 64, 3, 6, 2, 64, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
-        if (forced == 6) return launch_fused<MDT, MODE_FAMILY, 32, 4, 6, 2, 64, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
         // measured: 128 KB operand ring 229 us / layer, 64 KB 298 us (4 B/element of state: the mainloop is the long pole)
         return launch_fused<MDT, MODE_FAMILY, 64, 4, 6, 2, 64, 128, 128, 2, 0>(probs, count, hp, dev, stream, &fs);
     }
     if (nst == 1) {
         if (big) return launch_fused<MDT, MODE_FAMILY, 64, 4, 2, 2, 64, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
-        if (forced == 1) return launch_fused<MDT, MODE_FAMILY, 32, 4, 6, 2, 64, 64, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
-        if (forced == 2) return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 64, 64, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
-        if (forced == 3) return launch_fused<MDT, MODE_FAMILY, 32, 4, 2, 2, 64, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
-        if (forced == 4) return launch_fused<MDT, MODE_FAMILY, 64, 4, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
-        if (forced == 5) return launch_fused<MDT, MODE_FAMILY, 64, 3, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
-        // measured (momentum, fp32 / bf16 state): 32 x 128 x 4 slots 465 / 376 us, 64 x 64 x 4 483 / 396, 64 x 128 x 2 514 / 417
-        if (forced == 6) return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
+        // measured (momentum, fp32 / bf16 state): 32 x 128 x 4 slots 465 / 376 us, 64 x 64 x 4 483 / 396, 64 x 128 x 2 514 / 417;
         // 128 KB operand ring + 32 x 128 x 4 slots: momentum 439 us (fp32 state), 355 us (bf16); with a 64 KB operand ring 448 / 370
         return launch_fused<MDT, MODE_FAMILY, 64, 4, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
     }
     if (big) return launch_fused<MDT, MODE_FAMILY, 64, 4, 2, 2, 64, 64, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
-    if (MDT == MDT_FP32) {      // two fp32 states: AdamW's byte count, and AdamW's two instantiations by power state
-        if (expect_power_cap(dev.device, estimate_ms(probs, count, FORGE_MOMENT_FP32)) && forced < 0)
-            return launch_fused<MDT, MODE_FAMILY, 32, 3, 2, 2, 128, 64, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
+    if (MDT == MDT_FP32)        // two fp32 states: AdamW's byte count and AdamW's instantiation
         return launch_fused<MDT, MODE_FAMILY, 32, 4, 2, 2, 64, 128, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
-    }
     return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 64, 64, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
+}
+
+// ---------------------------------------------------------------------------------------------
+// dgrad launch (dgrad_kernel.cuh): dX_i = dY_i . W_i for <= kDgMaxProblems problems
+// ---------------------------------------------------------------------------------------------
+forge_status_t launch_dgrad(const forge_problem_t *probs, void *const *dX, int count, const DeviceInfo &dev,
+                            cudaStream_t stream) {
+    constexpr int kStages = 5;
+    using Cfg = DgradCfg<kStages>;
+    auto kernel = forge_dgrad_kernel<kStages>;
+    static std::atomic<uint64_t> attr_done{0};
+    const uint64_t dev_bit = 1ull << (dev.device & 63);
+    if (!(attr_done.load(std::memory_order_acquire) & dev_bit)) {
+        const cudaError_t ae = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
+        if (ae != cudaSuccess) return cuda_fail(ae);
+        attr_done.fetch_or(dev_bit, std::memory_order_release);
+    }
+    static_assert(sizeof(DgradParams) <= 32 * 1024 - 64, "kernel parameter space");
+    DgradParams P;
+    std::memset(&P, 0, sizeof(P));
+    P.num_problems = count;
+    int tiles = 0;
+    for (int i = 0; i < count; ++i) {
+        const forge_problem_t &p = probs[i];
+        DgradProblem &d = P.prob[i];
+        bool ok = true;
+        ok &= encode_2d(&d.map_dY, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.dY, p.T, p.out, 64, DG_BM, CU_TENSOR_MAP_SWIZZLE_128B,
+                        static_cast<uint64_t>(p.lddy));
+        ok &= encode_2d(&d.map_W, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p.W, p.out, p.in, 64, DG_BK, CU_TENSOR_MAP_SWIZZLE_128B);
+        ok &= encode_2d(&d.map_dX, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, dX[i], p.T, p.in, 64, 32, CU_TENSOR_MAP_SWIZZLE_128B);
+        if (!ok) return cuda_fail(cudaErrorInvalidValue);
+        d.T = p.T; d.out = p.out; d.in = p.in;
+        d.tiles_n = (p.in + DG_BN - 1) / DG_BN;
+        d.tile_begin = tiles;
+        tiles += ((p.T + 2 * DG_BM - 1) / (2 * DG_BM)) * d.tiles_n;
+    }
+    P.total_tiles = tiles;
+    int pairs = std::min(dev.sm_count / 2, kDgMaxPairs);
+    if (pairs > tiles) pairs = tiles;
+    // longest-processing-time-first assignment of tiles (cost = depth `out`) to CTA pairs
+    P.use_list = tiles <= kDgMaxTiles ? 1 : 0;
+    if (P.use_list) {
+        std::vector<std::pair<int, int>> by_depth;            // (depth, tile)
+        by_depth.reserve(tiles);
+        for (int i = 0; i < count; ++i) {
+            const int n = (i + 1 < count ? P.prob[i + 1].tile_begin : tiles) - P.prob[i].tile_begin;
+            for (int t = 0; t < n; ++t) by_depth.push_back({probs[i].out, P.prob[i].tile_begin + t});
+        }
+        std::stable_sort(by_depth.begin(), by_depth.end(), [](const std::pair<int, int> &a, const std::pair<int, int> &b) { return a.first > b.first; });
+        std::vector<long long> load(pairs, 0);
+        std::vector<std::vector<uint16_t>> mine(pairs);
+        for (const auto &dt : by_depth) {
+            int best = 0;
+            for (int g = 1; g < pairs; ++g) if (load[g] < load[best]) best = g;
+            load[best] += dt.first + 256;                        // + per-tile overhead (epilogue hand-over) in depth units
+            mine[best].push_back(static_cast<uint16_t>(dt.second));
+        }
+        int o = 0;
+        for (int g = 0; g < pairs; ++g) {
+            P.pair_begin[g] = static_cast<uint16_t>(o);
+            for (uint16_t t : mine[g]) P.order[o++] = t;
+        }
+        P.pair_begin[pairs] = static_cast<uint16_t>(o);
+    }
+    if (dev.dry) return FORGE_OK;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(pairs * 2));
+    cfg.blockDim = dim3(kDgThreads);
+    cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kernel, P);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e);
+    g_launches.fetch_add(1);
+    g_last_kernel.store("forge_dgrad_kernel<5>");
+    return FORGE_OK;
 }
 
 }  // namespace
@@ -565,16 +599,15 @@ forge_status_t forge_wgrad_adamw_grouped(const forge_problem_t *problems, int32_
         s = validate_problem(problems[i], mdt);
         if (s != FORGE_OK) return s;
     }
+    s = validate_disjoint(problems, count, mdt, moment_bytes(mdt));
+    if (s != FORGE_OK) return s;
     DeviceInfo dev;
     s = device_info(dev);
     if (s != FORGE_OK) return s;
     const AdamWScalars hp = make_scalars(step, lr, beta1, beta2, eps, wd);
-    for (int i = 0; i < count; i += kMaxProblems) {
-        const int n = (count - i) < kMaxProblems ? (count - i) : kMaxProblems;
-        s = dispatch_fused(problems + i, n, mdt, hp, dev, reinterpret_cast<cudaStream_t>(stream));
-        if (s != FORGE_OK) return s;
-    }
-    return FORGE_OK;
+    return for_each_launch(count, dev, [&](int i, int n, const DeviceInfo &d) {
+        return dispatch_fused(problems + i, n, mdt, hp, d, reinterpret_cast<cudaStream_t>(stream));
+    });
 }
 
 forge_status_t forge_wgrad_adamw(const void *X, const void *dY, void *W, void *m, void *v, float *m_scale,
@@ -608,21 +641,21 @@ forge_status_t forge_wgrad_step_grouped(const forge_problem_t *problems, int32_t
         if (!p.X || !p.dY || !p.W) return FORGE_ERR_NULL_PTR;
         if ((nst >= 1) != (p.m != nullptr) || (nst >= 2) != (p.v != nullptr)) return FORGE_ERR_NULL_PTR;   // exactly the family's states
         if (p.m_scale || p.v_scale) return FORGE_ERR_BAD_DTYPE;
-        if (p.T < 1 || p.out < 8 || p.in < 8 || (p.out % 8) || (p.in % 8)) return FORGE_ERR_BAD_SHAPE;
-        if (!aligned16(p.X) || !aligned16(p.dY) || !aligned16(p.W) || !aligned16(p.m) || !aligned16(p.v)) return FORGE_ERR_ALIGNMENT;
+        s = validate_operands(p);
+        if (s != FORGE_OK) return s;
+        if (!aligned16(p.W) || !aligned16(p.m) || !aligned16(p.v)) return FORGE_ERR_ALIGNMENT;
     }
+    s = validate_disjoint(problems, count, mdt, moment_bytes(mdt));
+    if (s != FORGE_OK) return s;
     DeviceInfo dev;
     s = device_info(dev);
     if (s != FORGE_OK) return s;
     const FamilyScalars fs = make_family(*opt);
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-    for (int i = 0; i < count; i += kMaxProblems) {
-        const int n = (count - i) < kMaxProblems ? (count - i) : kMaxProblems;
-        s = mdt == FORGE_MOMENT_FP32 ? dispatch_family<MDT_FP32>(problems + i, n, nst, fs, dev, st)
-                                     : dispatch_family<MDT_BF16>(problems + i, n, nst, fs, dev, st);
-        if (s != FORGE_OK) return s;
-    }
-    return FORGE_OK;
+    return for_each_launch(count, dev, [&](int i, int n, const DeviceInfo &d) {
+        return mdt == FORGE_MOMENT_FP32 ? dispatch_family<MDT_FP32>(problems + i, n, nst, fs, d, st)
+                                        : dispatch_family<MDT_BF16>(problems + i, n, nst, fs, d, st);
+    });
 }
 
 forge_status_t forge_wgrad_accumulate_grouped(const forge_problem_t *problems, int32_t count, float mu,
@@ -637,12 +670,15 @@ forge_status_t forge_wgrad_accumulate_grouped(const forge_problem_t *problems, i
         const forge_problem_t &p = problems[i];
         if (!p.X || !p.dY || !p.m) return FORGE_ERR_NULL_PTR;
         if (p.W || p.v || p.m_scale || p.v_scale) return FORGE_ERR_BAD_DTYPE;      // B only: no weight is touched
-        if (p.T < 1 || p.out < 8 || p.in < 8 || (p.out % 8) || (p.in % 8)) return FORGE_ERR_BAD_SHAPE;
-        if (!aligned16(p.X) || !aligned16(p.dY) || !aligned16(p.m)) return FORGE_ERR_ALIGNMENT;
+        const forge_status_t so = validate_operands(p);
+        if (so != FORGE_OK) return so;
+        if (!aligned16(p.m)) return FORGE_ERR_ALIGNMENT;
         maxT = p.T > maxT ? p.T : maxT;
     }
+    forge_status_t s = validate_disjoint(problems, count, mdt, moment_bytes(mdt));
+    if (s != FORGE_OK) return s;
     DeviceInfo dev;
-    forge_status_t s = device_info(dev);
+    s = device_info(dev);
     if (s != FORGE_OK) return s;
     AdamWScalars hp;
     std::memset(&hp, 0, sizeof(hp));
@@ -650,18 +686,14 @@ forge_status_t forge_wgrad_accumulate_grouped(const forge_problem_t *problems, i
     std::memset(&fs, 0, sizeof(fs));
     fs.a1 = mu;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-    for (int i = 0; i < count; i += kMaxProblems) {
-        const int n = (count - i) < kMaxProblems ? (count - i) : kMaxProblems;
+    return for_each_launch(count, dev, [&](int i, int n, const DeviceInfo &d) {
         const forge_problem_t *pp = problems + i;
         if (mdt == FORGE_MOMENT_FP32)
-            s = maxT > 1024 ? launch_fused<MDT_FP32, MODE_ACCUM, 64, 4, 2, 2, 64, 128, 128, 2, 1>(pp, n, hp, dev, st, &fs)
-                            : launch_fused<MDT_FP32, MODE_ACCUM, 64, 4, 4, 2, 32, 128, 128, 2, 1>(pp, n, hp, dev, st, &fs);
-        else
-            s = maxT > 1024 ? launch_fused<MDT_BF16, MODE_ACCUM, 64, 4, 2, 2, 64, 128, 128, 2, 1>(pp, n, hp, dev, st, &fs)
-                            : launch_fused<MDT_BF16, MODE_ACCUM, 64, 4, 4, 2, 32, 128, 128, 2, 1>(pp, n, hp, dev, st, &fs);
-        if (s != FORGE_OK) return s;
-    }
-    return FORGE_OK;
+            return maxT > 1024 ? launch_fused<MDT_FP32, MODE_ACCUM, 64, 4, 2, 2, 64, 128, 128, 2, 1>(pp, n, hp, d, st, &fs)
+                               : launch_fused<MDT_FP32, MODE_ACCUM, 64, 4, 4, 2, 32, 128, 128, 2, 1>(pp, n, hp, d, st, &fs);
+        return maxT > 1024 ? launch_fused<MDT_BF16, MODE_ACCUM, 64, 4, 2, 2, 64, 128, 128, 2, 1>(pp, n, hp, d, st, &fs)
+                           : launch_fused<MDT_BF16, MODE_ACCUM, 64, 4, 4, 2, 32, 128, 128, 2, 1>(pp, n, hp, d, st, &fs);
+    });
 }
 
 forge_status_t forge_wgrad_adamw_sr_grouped(const forge_problem_t *problems, int32_t count, int64_t step, float lr,
@@ -679,25 +711,23 @@ forge_status_t forge_wgrad_adamw_sr_grouped(const forge_problem_t *problems, int
         if (s != FORGE_OK) return s;
         maxT = problems[i].T > maxT ? problems[i].T : maxT;
     }
+    s = validate_disjoint(problems, count, mdt, moment_bytes(mdt));
+    if (s != FORGE_OK) return s;
     DeviceInfo dev;
     s = device_info(dev);
     if (s != FORGE_OK) return s;
     const AdamWScalars hp = make_scalars(step, lr, beta1, beta2, eps, wd);
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     const uint32_t st32 = static_cast<uint32_t>(step);
-    for (int i = 0; i < count; i += kMaxProblems) {    // the random stream of a problem is its index in the call
-        const int n = (count - i) < kMaxProblems ? (count - i) : kMaxProblems;
+    return for_each_launch(count, dev, [&](int i, int n, const DeviceInfo &d) {    // the random stream of a problem is its index in the call
         const forge_problem_t *pp = problems + i;
         const uint32_t s0 = static_cast<uint32_t>(i);
         if (mdt == FORGE_MOMENT_FP32)
-            s = maxT > 1024 ? launch_fused<MDT_FP32, MODE_ADAMW_SR, 64, 4, 2, 2, 64, 64>(pp, n, hp, dev, st, nullptr, seed, st32, s0)
-                            : launch_fused<MDT_FP32, MODE_ADAMW_SR, 32, 4, 2, 2, 64, 128>(pp, n, hp, dev, st, nullptr, seed, st32, s0);
-        else
-            s = maxT > 1024 ? launch_fused<MDT_BF16, MODE_ADAMW_SR, 64, 4, 2, 2, 64, 64>(pp, n, hp, dev, st, nullptr, seed, st32, s0)
-                            : launch_fused<MDT_BF16, MODE_ADAMW_SR, 32, 4, 4, 2, 64, 64>(pp, n, hp, dev, st, nullptr, seed, st32, s0);
-        if (s != FORGE_OK) return s;
-    }
-    return FORGE_OK;
+            return maxT > 1024 ? launch_fused<MDT_FP32, MODE_ADAMW_SR, 64, 4, 2, 2, 64, 64>(pp, n, hp, d, st, nullptr, seed, st32, s0)
+                               : launch_fused<MDT_FP32, MODE_ADAMW_SR, 32, 4, 2, 2, 64, 128>(pp, n, hp, d, st, nullptr, seed, st32, s0);
+        return maxT > 1024 ? launch_fused<MDT_BF16, MODE_ADAMW_SR, 64, 4, 2, 2, 64, 64>(pp, n, hp, d, st, nullptr, seed, st32, s0)
+                           : launch_fused<MDT_BF16, MODE_ADAMW_SR, 32, 4, 4, 2, 64, 64>(pp, n, hp, d, st, nullptr, seed, st32, s0);
+    });
 }
 
 forge_status_t forge_layer_backward_grouped(const forge_problem_t *problems, void *const *dX, int32_t count,
@@ -715,25 +745,39 @@ forge_status_t forge_layer_backward_grouped(const forge_problem_t *problems, voi
         if (!dX[i]) return FORGE_ERR_NULL_PTR;
         if (!aligned16(dX[i])) return FORGE_ERR_ALIGNMENT;
     }
+    // dX may not overlap anything the call reads or writes
+    std::vector<size_t> dx_bytes(count);
+    for (int i = 0; i < count; ++i) dx_bytes[i] = static_cast<size_t>(problems[i].T) * problems[i].in * 2;
+    s = validate_disjoint(problems, count, mdt, moment_bytes(mdt), dX, dx_bytes.data());
+    if (s != FORGE_OK) return s;
     DeviceInfo dev;
     s = device_info(dev);
     if (s != FORGE_OK) return s;
-    static thread_local cublasHandle_t handle = nullptr;
-    if (!handle && cublasCreate(&handle) != CUBLAS_STATUS_SUCCESS) return cuda_fail(cudaErrorInitializationError);
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-    if (cublasSetStream(handle, st) != CUBLAS_STATUS_SUCCESS) return cuda_fail(cudaErrorUnknown);
-    // 1. dX = dY . W from the PRE-update W (Alg. 1 line 1; 296 Remark 2).  Row-major
-    //    dX[T,in] = dY[T,out] W[out,in] is the column-major product dX^T[in,T] = W^T[in,out] dY^T[out,T].
-    const float one = 1.0f, zero = 0.0f;
-    for (int i = 0; i < count; ++i) {
-        const forge_problem_t &p = problems[i];
-        cublasStatus_t cs = cublasGemmEx(handle, CUBLAS_OP_N, CUBLAS_OP_N, p.in, p.T, p.out, &one, p.W, CUDA_R_16BF, p.in,
-                                         p.dY, CUDA_R_16BF, p.lddy ? p.lddy : p.out, &zero, dX[i], CUDA_R_16BF, p.in, CUBLAS_COMPUTE_32F,
-                                         CUBLAS_GEMM_DEFAULT);
-        if (cs != CUBLAS_STATUS_SUCCESS) return cuda_fail(cudaErrorUnknown);
+    const AdamWScalars hp = make_scalars(step, lr, beta1, beta2, eps, wd);
+    // Everything is prepared before anything is enqueued: a dry pass over the dgrad launches and the fused launches
+    // encodes every tensor map and sets every function attribute.
+    DeviceInfo dry = dev;
+    dry.dry = true;
+    for (int i = 0; i < count; i += kDgMaxProblems) {
+        s = launch_dgrad(problems + i, dX + i, std::min(count - i, kDgMaxProblems), dry, st);
+        if (s != FORGE_OK) return s;
     }
-    // 2. the fused weight-gradient + AdamW step, stream-ordered after every dgrad GEMM that reads W
-    return forge_wgrad_adamw_grouped(problems, count, step, lr, beta1, beta2, eps, wd, moment_dtype, stream);
+    for (int i = 0; i < count; i += kMaxProblems) {
+        s = dispatch_fused(problems + i, std::min(count - i, kMaxProblems), mdt, hp, dry, st);
+        if (s != FORGE_OK) return s;
+    }
+    // 1. dX = dY . W from the PRE-update W (Alg. 1 line 1; 296 Remark 2): the hand-written tcgen05 dgrad
+    for (int i = 0; i < count; i += kDgMaxProblems) {
+        s = launch_dgrad(problems + i, dX + i, std::min(count - i, kDgMaxProblems), dev, st);
+        if (s != FORGE_OK) return s;
+    }
+    // 2. the fused weight-gradient + AdamW step, stream-ordered after every dgrad launch that reads W
+    for (int i = 0; i < count; i += kMaxProblems) {
+        s = dispatch_fused(problems + i, std::min(count - i, kMaxProblems), mdt, hp, dev, st);
+        if (s != FORGE_OK) return s;
+    }
+    return FORGE_OK;
 }
 
 forge_status_t forge_wgrad_store_g_grouped(const forge_problem_t *problems, int32_t count, forge_stream_t stream) {
@@ -744,14 +788,15 @@ forge_status_t forge_wgrad_store_g_grouped(const forge_problem_t *problems, int3
         const forge_problem_t &p = problems[i];
         if (!p.X || !p.dY || !p.m) return FORGE_ERR_NULL_PTR;
         if (p.W || p.v || p.m_scale || p.v_scale) return FORGE_ERR_BAD_DTYPE;   // a gradient has no state besides G
-        if (p.T < 1 || p.out < 8 || p.in < 8 || (p.out % 8) || (p.in % 8)) return FORGE_ERR_BAD_SHAPE;
-        if (p.ldx != 0 && (p.ldx < p.in || p.ldx % 8 != 0)) return FORGE_ERR_BAD_SHAPE;
-        if (p.lddy != 0 && (p.lddy < p.out || p.lddy % 8 != 0)) return FORGE_ERR_BAD_SHAPE;
-        if (!aligned16(p.X) || !aligned16(p.dY) || !aligned16(p.m)) return FORGE_ERR_ALIGNMENT;
+        const forge_status_t so = validate_operands(p);
+        if (so != FORGE_OK) return so;
+        if (!aligned16(p.m)) return FORGE_ERR_ALIGNMENT;
         maxT = p.T > maxT ? p.T : maxT;
     }
+    forge_status_t s = validate_disjoint(problems, count, FORGE_MOMENT_FP32, 4);
+    if (s != FORGE_OK) return s;
     DeviceInfo dev;
-    forge_status_t s = device_info(dev);
+    s = device_info(dev);
     if (s != FORGE_OK) return s;
     AdamWScalars hp;
     std::memset(&hp, 0, sizeof(hp));
@@ -759,14 +804,10 @@ forge_status_t forge_wgrad_store_g_grouped(const forge_problem_t *problems, int3
     // grouping, so store-G + forge_adamw_from_g is bit-identical to the fused call of any instantiation
     const int variant = pick_variant(maxT);
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-    for (int i = 0; i < count; i += kMaxProblems) {
-        const int n = (count - i) < kMaxProblems ? (count - i) : kMaxProblems;
-        if (variant == 1) s = launch_fused<MDT_FP32, MODE_STORE_G, 64, 3, 2, 1, 64, 64>(problems + i, n, hp, dev, st);
-        else if (variant == 4 || variant == 5) s = launch_fused<MDT_FP32, MODE_STORE_G, 64, 4, 2, 2, 64, 64>(problems + i, n, hp, dev, st);
-        else s = launch_fused<MDT_FP32, MODE_STORE_G, 32, 4, 2, 2, 64, 128>(problems + i, n, hp, dev, st);
-        if (s != FORGE_OK) return s;
-    }
-    return FORGE_OK;
+    return for_each_launch(count, dev, [&](int i, int n, const DeviceInfo &d) {
+        if (variant != V_SMALL_T) return launch_fused<MDT_FP32, MODE_STORE_G, 64, 4, 2, 2, 64, 64>(problems + i, n, hp, d, st);
+        return launch_fused<MDT_FP32, MODE_STORE_G, 32, 4, 2, 2, 64, 128>(problems + i, n, hp, d, st);
+    });
 }
 
 forge_status_t forge_wgrad_store_g(const void *X, const void *dY, float *G, int32_t T, int32_t out, int32_t in,
@@ -895,7 +936,7 @@ forge_status_t forge_wgrad_adamw_grouped_host(const forge_problem_t *problems, i
     // (PCIe is full duplex); without the slicing the first upload and the last download (0.6 GB each for gate_proj)
     // overlap nothing.
     const bool i8 = mdt == FORGE_MOMENT_INT8, f8 = mdt == FORGE_MOMENT_FP8;
-    const int slice_mb = env_int("FORGE_HOST_SLICE_MB", 64);   // tuning only; 0 = one slice per problem
+    const int slice_mb = env_int("FORGE_HOST_SLICE_MB", 64);   // FORGE_PROFILING build only; 0 = one slice per problem
     auto chunk_rows = [&](const forge_problem_t &p) {
         if (slice_mb <= 0) return static_cast<int>(p.out);
         const size_t row_bytes = static_cast<size_t>(p.in) * (2 + 2 * mom);
@@ -1006,6 +1047,7 @@ forge_status_t forge_wgrad_adamw_grouped_host(const forge_problem_t *problems, i
 size_t forge_workspace_bytes(void) { return 0; }
 uint64_t forge_launch_count(void) { return g_launches.load(); }
 int forge_last_cuda_error(void) { return g_last_cuda_error.load(); }
+const char *forge_last_kernel(void) { return g_last_kernel.load(); }
 int forge_version(void) { return FORGE_VERSION; }
 
 const char *forge_status_string(forge_status_t status) {

@@ -81,12 +81,17 @@ struct alignas(64) KernelParams {
     int32_t num_problems;
     int32_t total_tiles;
     uint32_t sr_seed_lo; // MODE_ADAMW_SR
-    int32_t debug;       // ablation switches for profiling ONLY (results are wrong when set):
-                         // 1 = no operand loads / MMA, 2 = no state loads / stores, 4 = no epilogue math,
-                         // 8 = no state stores (direct path only)
+    int32_t debug;       // -DFORGE_PROFILING builds only (libforge_b200_prof.so, used by the profiles/ commands): ablation
+                         // switches, results are WRONG when set.  1 = no operand loads / MMA, 2 = no state loads / stores,
+                         // 4 = no epilogue math, 8 = no state stores (direct path only).  The product build never reads it.
 };
 enum : int { DBG_NO_MAINLOOP = 1, DBG_NO_STATE = 2, DBG_NO_EPILOGUE = 4, DBG_NO_STORE = 8 /* direct path only */,
               DBG_NO_A = 16 /* CTA pairs: dY chunks loaded for the first ring pass only (operand traffic halved) */ };
+#ifdef FORGE_PROFILING
+#define FORGE_DBG(P, bit) (((P).debug & (bit)) != 0)
+#else
+#define FORGE_DBG(P, bit) false
+#endif
 
 // CG = 1: one CTA per 128x256 tile.  CG = 2: a CTA pair (cluster of 2, tcgen05 cta_group::2) shares
 // a 256x256 tile: each CTA stages its own 128 rows of A = dY^T and only HALF of B = X (128 of the
@@ -704,7 +709,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
 
     if (warp == 0) {
         // ================= operand producer (Alg. 1 lines 3-5: stream dY_k,i and X_k,j) ==========
-        if (lane == 0 && !(P.debug & DBG_NO_MAINLOOP)) {
+        if (lane == 0 && !FORGE_DBG(P, DBG_NO_MAINLOOP)) {
             uint32_t it = 0;  // running k-block counter over all tiles of this CTA
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step) {
                 const TileCoord tc = decode_tile<CG>(P, tile, rank);
@@ -727,7 +732,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                                         kb * kBlockK, kEvictLast);
                     } else {
                         // both CTAs' bytes are counted on the LEADER's full barrier
-                        const bool no_a = (P.debug & DBG_NO_A) && it >= kStages;
+                        const bool no_a = FORGE_DBG(P, DBG_NO_A) && it >= kStages;
                         if (rank == 0) mbar_expect_tx(bar_ml_full + 8 * s, 2 * (Cfg::ML_STAGE - (no_a ? Cfg::A_STAGE : 0)));
                         const uint32_t full = mapa_shared(bar_ml_full + 8 * s, 0);
 #pragma unroll
@@ -745,7 +750,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         }
     } else if (warp == 1) {
         // ================= MMA issuer (Alg. 1 line 4: G_ij += dY_k,i^T X_k,j) =====================
-        if (lane == 0 && rank == 0 && !(P.debug & DBG_NO_MAINLOOP)) {
+        if (lane == 0 && rank == 0 && !FORGE_DBG(P, DBG_NO_MAINLOOP)) {
             constexpr uint32_t idesc = make_idesc_bf16_f32_mnmn(BLOCK_M * CG, BLOCK_N);
             uint32_t it = 0, titer = 0;
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step, ++titer) {
@@ -780,9 +785,9 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
     } else if (warp == 2) {
         // ================= state loader (Alg. 1 line 6: load W_ij, m_ij, v_ij) ===================
         if constexpr (MDT == MDT_INT8) {
-            if (lane == 0 && !(P.debug & DBG_NO_STATE))
+            if (lane == 0 && !FORGE_DBG(P, DBG_NO_STATE))
                 int8_loader<Cfg, kStateStages, CG>(P, rank, first_tile, tile_step, sST, bar_st_full, bar_st_empty, i8);
-        } else if (!DIRECT && MODE != MODE_STORE_G && lane == 0 && !(P.debug & DBG_NO_STATE)) {
+        } else if (!DIRECT && MODE != MODE_STORE_G && lane == 0 && !FORGE_DBG(P, DBG_NO_STATE)) {
             uint32_t ci = 0;  // running chunk counter
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step) {
                 const TileCoord tc = decode_tile<CG>(P, tile, rank);
@@ -835,7 +840,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                     mbar_wait(bar_st_done + 8 * s, ph);
                     const uint32_t base = sST + s * Cfg::ST_STAGE;
                     const int x = tc.tn * BLOCK_N + (c / Cfg::RB) * CN, y = tc.tm * BLOCK_M + (c % Cfg::RB) * CM;
-                    if (P.debug & DBG_NO_STATE) {
+                    if (FORGE_DBG(P, DBG_NO_STATE)) {
                     } else {
                         if constexpr (MODE != MODE_STORE_G && HASW) {
 #pragma unroll
@@ -877,7 +882,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         uint32_t titer = 0;
         for (int tile = first_tile; tile < P.total_tiles; tile += tile_step, ++titer) {
             const uint32_t as = titer & 1u, aph = (titer >> 1) & 1u;
-            if (!(P.debug & DBG_NO_MAINLOOP)) mbar_wait(bar_tm_full + 8 * as, aph);
+            if (!FORGE_DBG(P, DBG_NO_MAINLOOP)) mbar_wait(bar_tm_full + 8 * as, aph);
             tc_fence_after();
             const uint32_t taddr = tmem_base + ((quad * 32u) << 16) + as * BLOCK_N;
             uint32_t sr_rowkey = 0, sr_col0 = 0;
@@ -903,7 +908,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                 constexpr int MB = Cfg::kMomBytes;
                 const int grow = tc.tm * BLOCK_M + static_cast<int>(row_t);
                 const int col0 = tc.tn * BLOCK_N + wg * (BLOCK_N / 2);
-                const bool row_ok = grow < pd.out && !(P.debug & DBG_NO_STATE);
+                const bool row_ok = grow < pd.out && !FORGE_DBG(P, DBG_NO_STATE);
                 const size_t e0 = static_cast<size_t>(row_ok ? grow : 0) * pd.in + col0;
                 char *Wp = pd.pW + e0 * 2, *Mp = pd.pM + e0 * MB, *Vp = pd.pV + e0 * MB;
                 constexpr int STEPS = BLOCK_N / 2 / 16;
@@ -917,9 +922,9 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                     if (st + 1 < STEPS && row_ok && col0 + (st + 1) * 16 < pd.in)
                         direct_load<MDT>(R[(st + 1) & 1], Wp + (st + 1) * 32, Mp + (st + 1) * 16 * MB, Vp + (st + 1) * 16 * MB);
                     tmem_ld_wait();
-                    if (ok && !(P.debug & DBG_NO_EPILOGUE))
+                    if (ok && !FORGE_DBG(P, DBG_NO_EPILOGUE))
                         direct_step<MDT>(hp, g, R[st & 1], Wp + st * 32, Mp + st * 16 * MB, Vp + st * 16 * MB,
-                                         (P.debug & DBG_NO_STORE) != 0);
+                                         FORGE_DBG(P, DBG_NO_STORE));
                 }
             } else if constexpr (MDT != MDT_INT8) {
                 for (int cb = 0; cb < Cfg::CB; ++cb) {
@@ -927,7 +932,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                     const uint32_t ci = titer * CHUNKS + cb * Cfg::RB + rb;
                     const uint32_t s = ci % SSN, ph = (ci / SSN) & 1u;
                     const uint32_t base = sST + s * Cfg::ST_STAGE;
-                    if (MODE != MODE_STORE_G && !(P.debug & DBG_NO_STATE)) mbar_wait(bar_st_full + 8 * s, ph);
+                    if (MODE != MODE_STORE_G && !FORGE_DBG(P, DBG_NO_STATE)) mbar_wait(bar_st_full + 8 * s, ph);
                     else mbar_wait(bar_st_empty + 8 * s, ph ^ 1u);
                     for (int j32 = (Cfg::SUBS >= 2 ? wg : 0); j32 < Cfg::SUBS; j32 += Cfg::WGS) {
                         uint32_t g[32];
@@ -935,9 +940,9 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                         const SubAddr<Cfg> a(base, j32 * SUB);
                         tmem_ld_wait();
                         if constexpr (MODE == MODE_ADAMW && MDT == MDT_FP8) {
-                            if (!(P.debug & DBG_NO_EPILOGUE)) epi_sub_fp8<Cfg>(hp, f8, g, a, row, f8_pm, f8_pv);
+                            if (!FORGE_DBG(P, DBG_NO_EPILOGUE)) epi_sub_fp8<Cfg>(hp, f8, g, a, row, f8_pm, f8_pv);
                         } else if constexpr (MODE == MODE_ADAMW) {
-                            if (!(P.debug & DBG_NO_EPILOGUE)) epi_sub_fp<MDT, Cfg>(hp, g, a, row);
+                            if (!FORGE_DBG(P, DBG_NO_EPILOGUE)) epi_sub_fp<MDT, Cfg>(hp, g, a, row);
                         } else if constexpr (MODE == MODE_ADAMW_SR) {
                             epi_sub_fp<MDT, Cfg, true>(hp, g, a, row, sr_rowkey, sr_col0 + cb * CN + j32 * SUB);
                         } else if constexpr (MODE == MODE_FAMILY) {
@@ -970,8 +975,8 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                 if (tile + tile_step < P.total_tiles) i8row = int8_row<CG>(P, hp, tile + tile_step, rank, row_t);
                 R.finish(hp);
                 float pm, pv;
-                int8_pass1<Cfg>(hp, R, titer, taddr, i8, row_t, wg, pm, pv, (P.debug & DBG_NO_EPILOGUE) != 0,
-                                (P.debug & DBG_NO_STATE) != 0);
+                int8_pass1<Cfg>(hp, R, titer, taddr, i8, row_t, wg, pm, pv, FORGE_DBG(P, DBG_NO_EPILOGUE),
+                                FORGE_DBG(P, DBG_NO_STATE));
                 // combine the two warpgroups' halves of the row (same TMEM quadrant: warps quad and 4 + quad)
                 const uint32_t xb = i8.xchg + (titer & 1u) * (kI8W * 1024u);
                 asm volatile("st.shared.v2.f32 [%0], {%1, %2};\n" ::"r"(xb + (wg * 128u + row_t) * 8u), "f"(pm), "f"(pv) : "memory");
@@ -985,7 +990,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                     a_v = fmaxf(a_v, ov);
                 }
                 int8_pass2<Cfg, kStateStages>(hp, R, a_m, a_v, titer, taddr, sST, bar_st_full, bar_st_done, bar_st_empty,
-                                              row_t, wg, (P.debug & DBG_NO_EPILOGUE) != 0, (P.debug & DBG_NO_STATE) != 0);
+                                              row_t, wg, FORGE_DBG(P, DBG_NO_EPILOGUE), FORGE_DBG(P, DBG_NO_STATE));
                 if (wg == 0 && R.valid) {
                     const ProblemDesc &pd = P.prob[decode_tile<CG>(P, tile, rank).p];
                     pd.m_scale[R.sidx] = a_m;

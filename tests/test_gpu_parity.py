@@ -246,16 +246,24 @@ def test_result_independent_of_grid_size_and_repeatable():
     result is bitwise independent of how many CTAs share the tile list."""
     p = synth.make_problem("x", 512, 1024, 1536, seed=11)
     outs = []
-    for grid in (None, "1", "37", None):
-        if grid:
-            os.environ["FORGE_GRID"] = grid
-        else:
-            os.environ.pop("FORGE_GRID", None)
-        d, _ = gpu_state(p, "fp32")
-        fb.forge_wgrad_adamw(d["X"], d["dY"], d["W"], d["m"], d["v"], 3, **HP)
-        torch.cuda.synchronize()
-        outs.append(d)
-    os.environ.pop("FORGE_GRID", None)
+    d, _ = gpu_state(p, "fp32")
+    fb.forge_wgrad_adamw(d["X"], d["dY"], d["W"], d["m"], d["v"], 3, **HP)      # the product library
+    torch.cuda.synchronize()
+    outs.append(d)
+    fb.use_profiling_library(True)          # FORGE_GRID exists only in the -DFORGE_PROFILING build
+    try:
+        for grid in (None, "1", "37", None):
+            if grid:
+                os.environ["FORGE_GRID"] = grid
+            else:
+                os.environ.pop("FORGE_GRID", None)
+            d, _ = gpu_state(p, "fp32")
+            fb.forge_wgrad_adamw(d["X"], d["dY"], d["W"], d["m"], d["v"], 3, **HP)
+            torch.cuda.synchronize()
+            outs.append(d)
+    finally:
+        os.environ.pop("FORGE_GRID", None)
+        fb.use_profiling_library(False)
     for d in outs[1:]:
         for k in ("W", "m", "v"):
             assert torch.equal(outs[0][k], d[k])
@@ -263,7 +271,7 @@ def test_result_independent_of_grid_size_and_repeatable():
 
 def test_randomised_shapes_strides_and_dispatch_paths_equal_the_twin_bitwise():
     """40 seeded random cases over T (1 ... 9000: ring, large-T ring, direct path), ragged out / in, the three moment dtypes,
-    strided operand views and both power-state instantiations: the fused call must equal store-G + the same update bit
+    strided operand views: the fused call must equal store-G + the same update bit
     for bit.  (The gradient itself is checked against the oracle by the tests above.)"""
     import random
     rnd = random.Random(20260622)
@@ -283,12 +291,7 @@ def test_randomised_shapes_strides_and_dispatch_paths_equal_the_twin_bitwise():
             wx[:, 8:8 + inn], wy[:, 16:16 + out] = X, dY
             d1["X"], d1["dY"] = wx[:, 8:8 + inn], wy[:, 16:16 + out]
         d2 = {k: (v if k in ("X", "dY") else v.clone()) for k, v in d1.items()}
-        if rnd.random() < 0.3:
-            os.environ["FORGE_POWER_STATE"] = "capped"
-        try:
-            fb.forge_wgrad_adamw_grouped([d1], *hp_args(5), {"fp32": fb.FP32, "bf16": fb.BF16, "int8": fb.INT8}[moment])
-        finally:
-            os.environ.pop("FORGE_POWER_STATE", None)
+        fb.forge_wgrad_adamw_grouped([d1], *hp_args(5), {"fp32": fb.FP32, "bf16": fb.BF16, "int8": fb.INT8}[moment])
         G = torch.full((out, inn), float("nan"), device=DEV)
         fb.forge_wgrad_store_g(X, dY, G)
         fb.forge_adamw_from_g(G, d2["W"], d2["m"], d2["v"], 5, m_scale=d2.get("m_scale"), v_scale=d2.get("v_scale"), **HP)
@@ -299,21 +302,47 @@ def test_randomised_shapes_strides_and_dispatch_paths_equal_the_twin_bitwise():
                 assert torch.equal(d1[k].view(torch.uint8), d2[k].view(torch.uint8)), (it, moment, T, out, inn, k)
 
 
-def test_power_state_variants_are_bit_identical():
-    """The fp32 path switches chunk shape when the library expects the launch to run under the board's power cap
-    (forge_api.cu expect_power_cap); FORGE_POWER_STATE forces either side.  Same bits, grouped launch, ragged shapes."""
+def test_stray_profiling_environment_cannot_change_a_product_result():
+    """The ablation / grid / variant switches are compiled only into libforge_b200_prof.so: with the product library a
+    FORGE_ABLATE=2 (\"no state loads / stores\") left over in the environment must change nothing."""
+    ps = [synth.make_problem("a", 512, 640, 768, 21), synth.make_problem("b", 200, 136, 264, 22)]
+    outs = []
+    stray = {"FORGE_ABLATE": "2", "FORGE_GRID": "3", "FORGE_CFG": "7", "FORGE_POWER_STATE": "capped"}
+    for env in ({}, stray):
+        os.environ.update(env)
+        try:
+            devs = [dict(X=p.X.to(DEV), dY=p.dY.to(DEV), W=p.W.to(DEV).clone(), m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone()) for p in ps]
+            fb.forge_wgrad_adamw_grouped(devs, *hp_args(4), fb.FP32)
+            torch.cuda.synchronize()
+        finally:
+            for k in env:
+                os.environ.pop(k, None)
+        outs.append(devs)
+    for a, b in zip(outs[0], outs[1]):
+        for k in ("W", "m", "v"):
+            assert torch.equal(a[k], b[k]), k
+    assert not torch.equal(outs[0][0]["W"], ps[0].W.to(DEV))
+
+
+def test_chunk_geometries_are_bit_identical():
+    """Every instantiation sums the tokens in the same order and applies the same per-element update, so the chunk shape
+    and ring depths are invisible in the results (FORGE_CFG, profiling build): grouped launch, ragged shapes."""
     ps = [synth.make_problem("a", 512, 640, 768, 21), synth.make_problem("b", 200, 136, 264, 22), synth.make_problem("c", 512, 1024, 1536, 23)]
     outs = []
-    for state in ("boost", "capped", None):
-        if state:
-            os.environ["FORGE_POWER_STATE"] = state
-        else:
-            os.environ.pop("FORGE_POWER_STATE", None)
-        devs = [dict(X=p.X.to(DEV), dY=p.dY.to(DEV), W=p.W.to(DEV).clone(), m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone()) for p in ps]
-        fb.forge_wgrad_adamw_grouped(devs, *hp_args(4), fb.FP32)
-        torch.cuda.synchronize()
-        outs.append(devs)
-    os.environ.pop("FORGE_POWER_STATE", None)
+    fb.use_profiling_library(True)
+    try:
+        for cfg in (None, "17", "5", "7"):
+            if cfg:
+                os.environ["FORGE_CFG"] = cfg
+            else:
+                os.environ.pop("FORGE_CFG", None)
+            devs = [dict(X=p.X.to(DEV), dY=p.dY.to(DEV), W=p.W.to(DEV).clone(), m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone()) for p in ps]
+            fb.forge_wgrad_adamw_grouped(devs, *hp_args(4), fb.FP32)
+            torch.cuda.synchronize()
+            outs.append(devs)
+    finally:
+        os.environ.pop("FORGE_CFG", None)
+        fb.use_profiling_library(False)
     for devs in outs[1:]:
         for a, b in zip(outs[0], devs):
             for k in ("W", "m", "v"):
@@ -443,6 +472,36 @@ def test_layer_backward_dgrad_reads_pre_update_weights_then_fused_step():
     assert fb.forge_layer_backward_grouped(bad, dXs, *hp_args(11), fb.FP32, check=False) == 1
     torch.cuda.synchronize()
     assert torch.equal(probs[0]["W"], W0)
+
+
+def test_dgrad_kernel_multi_tile_grouped_depths_and_strided_dy():
+    """The hand-written tcgen05 dgrad (csrc/dgrad_kernel.cuh) against the oracle's plain definition
+    dX[t,q] = sum_p dY[t,p] W[p,q] (Alg. 1 line 1) on a group whose tiles differ in depth (the
+    longest-first assignment), span several 256 x 256 tiles with ragged T / in / out tails, and read dY as a column
+    slice of a wider tensor (lddy)."""
+    shapes = [("a", 512, 1024, 768), ("b", 300, 2056, 520), ("c", 700, 136, 264), ("d", 128, 4096, 256), ("e", 1, 64, 8)]
+    ps = [synth.make_problem(n, T, o, i, 70 + k) for k, (n, T, o, i) in enumerate(shapes)]
+    probs, dXs = [], []
+    for k, p in enumerate(ps):
+        dY = p.dY.to(DEV)
+        if k % 2 == 1:                                   # strided view
+            wide = torch.zeros(p.T, p.out + 48, dtype=torch.bfloat16, device=DEV)
+            wide[:, 24:24 + p.out] = dY
+            dY = wide[:, 24:24 + p.out]
+        probs.append(dict(X=p.X.to(DEV), dY=dY, W=p.W.to(DEV).clone(), m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone()))
+        dXs.append(torch.full((p.T, p.inn), float("nan"), dtype=torch.bfloat16, device=DEV))
+    launches0 = fb.forge_launch_count()
+    fb.forge_layer_backward_grouped(probs, dXs, *hp_args(10), fb.FP32)
+    torch.cuda.synchronize()
+    assert fb.forge_launch_count() - launches0 == 2          # one dgrad launch + one fused launch
+    for p, dX in zip(ps, dXs):
+        dYf, Wf = fo.bf16_to_f64(synth.bf16_bits(p.dY)), fo.bf16_to_f64(synth.bf16_bits(p.W))
+        ref = fo.dgrad(synth.bf16_bits(p.dY), synth.bf16_bits(p.W))
+        got = fo.bf16_to_f64(synth.bf16_bits(dX))
+        assert not np.isnan(got).any()
+        bound = p.out * 2.0 ** -23 * (np.abs(dYf) @ np.abs(Wf))
+        assert np.all(np.abs(got - ref) <= pu.bf16_ulp(ref) + bound), (p.name, np.abs(got - ref).max())
+        assert float((synth.bf16_bits(dX) == fo.f64_to_bf16(ref)).mean()) > 0.98, p.name
 
 
 def test_grouped_host_entry_matches_device_path_bitwise():
