@@ -3,19 +3,28 @@
 (7 projections as one grouped launch, T=512, bf16 W, fp32 m/v; BASELINE.json configs[1]) and its
 fraction of the HBM roofline on one B200.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--moments fp32|bf16|int8] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--moments fp32|bf16|int8|fp8] [--impl reference]
+                  [--workload layer|q|..|down|model] [--tokens T] [--shard rows] [--backward]
 
 A "step" is one pass of the whole hot path over one synthetic layer:
 one forge_wgrad_adamw_grouped call.  Inputs are resident in HBM before the timed region; the
 working set (4.4 GB of state per layer) is far larger than the 126 MB L2, so no flush is needed.
-With N > 1 (torchrun) every rank runs its own layer (weak scaling, no collective on the data
-path: the tiles are independent); `value` is then us per layer over all
-ranks.  `--impl reference` times the CPU oracle (the only "reference implementation" this build
-has) on a bounded sample of the same workload.
+
+The default run prints ONE JSON line: the headline (configs[1]) with `roofline`, `e2e`, `cpu_baseline`,
+`sustained`, the same-GPU unfused arms, `layer_backward` (dgrad + fused step in one call), and under `configs` the
+other BASELINE.json configurations -- configs[2] (bf16, int8 moments), configs[3] (gate_proj at T = 512 / 2048 / 8192)
+and configs[4] (the 75 GB stack) -- each timed with its own clock record against this box's MEASURED_PEAKS.json.
+
+N > 1: `--gpus N` without WORLD_SIZE in the environment spawns N ranks itself (torchrun works too).  Default mode is
+replicas (every rank its own layer, weak scaling, no collective on the data path: the tiles are independent,
+PAPER.md:273-279, 302); `--shard rows` splits ONE layer's weight rows over the ranks (shard.py, Prop. 2(i): strong
+scaling, still no collective).  `--impl reference` times the CPU oracle (the only "reference implementation" this
+build has), a whole layer per step.
 """
 from __future__ import annotations
 
 import argparse
+import glob
 import json
 import os
 import sys
@@ -31,9 +40,7 @@ UNIT = "us/layer"
 MOMENT_BYTES = {"fp32": 20.0, "bf16": 12.0, "int8": 8.0 + 2 * 2 * 4 / 256, "fp8": 8.0}   # SURVEY.md 8(d), B/element
 MOMENT_ENUM = {"fp32": 0, "bf16": 1, "int8": 2, "fp8": 3}
 T_TOKENS = 512
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed
-# ncu --set full capture (profiles/); None until a capture of the current kernel exists.
-NCU_TRAFFIC_BYTES = {"fp32": 4378000000, "bf16": 2637000000, "int8": 1785000000, "fp8": 1763000000}
+SEED = 20260622 + 1
 
 
 def measured_peaks():
@@ -56,6 +63,7 @@ def workload_shapes(workload: str):
 
 
 def layer_counts(workload: str = "layer", tokens: int = T_TOKENS):
+    """(weight elements, operand bytes with each distinct X counted once, flops) of one launch."""
     from paper_2606_22932_b200 import synth
     shapes = workload_shapes(workload)
     params = sum(o * i for _, o, i in shapes)
@@ -108,35 +116,25 @@ class ClockSampler(threading.Thread):
 
 
 # ------------------------------------------------------------------------------------------------
-# workload construction (synthetic, seeded; shapes of BASELINE.json configs[1] / [2])
+# workload construction (synthetic, seeded; shapes of BASELINE.json configs[1] / [2] / [3])
 # ------------------------------------------------------------------------------------------------
 def make_device_layer(moments: str, seed: int, device, workload: str = "layer", tokens: int = T_TOKENS):
-    """One Llama-3.1-8B layer's 7 problems (or one projection of it) on the device (inputs resident in HBM)."""
+    """One Llama-3.1-8B layer's 7 problems (or one projection of it) on `device` (inputs resident in HBM).  The int8 /
+    fp8 state is drawn directly as codes and scales (synth.random_*_state): no quantiser runs outside the library."""
     import torch
     from paper_2606_22932_b200 import synth
     probs = synth.make_layer(tokens, seed, shapes=workload_shapes(workload), device=device)
     out = []
-    for p in probs:
+    for k, p in enumerate(probs):
         d = dict(X=p.X, dY=p.dY, W=p.W)
         if moments == "fp32":
             d["m"], d["v"] = p.m, p.v
         elif moments == "bf16":
             d["m"], d["v"] = p.m.to(torch.bfloat16), p.v.to(torch.bfloat16)
         elif moments == "fp8":
-            # e4m3 codes of x / s, s = amax / 448 (torch's cast; initial state only), scale pair [s, amax-out]
-            sm, sv = p.m.abs().amax() / 448.0, p.v.amax() / 448.0
-            d["m"] = (p.m / sm).to(torch.float8_e4m3fn).view(torch.uint8)
-            d["v"] = (p.v / sv).to(torch.float8_e4m3fn).view(torch.uint8)
-            d["m_scale"] = torch.stack([sm, torch.zeros_like(sm)]).float().contiguous()
-            d["v_scale"] = torch.stack([sv, torch.zeros_like(sv)]).float().contiguous()
+            d["m"], d["v"], d["m_scale"], d["v_scale"] = synth.random_fp8_state(p.out, p.inn, seed * 100 + k, device)
         else:
-            # seed codes/scales with torch ops only (initial state; the method's arithmetic starts at step 1)
-            nb = p.inn // 256
-            ms = p.m.view(p.out, nb, 256).abs().amax(-1)
-            vs = p.v.view(p.out, nb, 256).amax(-1)
-            d["m"] = torch.round(p.m.view(p.out, nb, 256) * (127.0 / ms)[..., None]).clamp(-127, 127).to(torch.int8).view(p.out, p.inn)
-            d["v"] = torch.round(p.v.view(p.out, nb, 256) * (255.0 / vs)[..., None]).clamp(1, 255).to(torch.uint8).view(p.out, p.inn)
-            d["m_scale"], d["v_scale"] = ms.contiguous(), vs.contiguous()
+            d["m"], d["v"], d["m_scale"], d["v_scale"] = synth.random_int8_state(p.out, p.inn, seed * 100 + k, device)
         out.append(d)
     return out
 
@@ -148,14 +146,45 @@ def make_host_layer(moments: str, seed: int):
 
 
 # ------------------------------------------------------------------------------------------------
+# ncu evidence: DRAM traffic of the dispatched instantiation from the committed captures under profiles/
+# ------------------------------------------------------------------------------------------------
+def ncu_traffic(signature: str, tag: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the newest `profiles/r*_fused_<tag>_full.csv`
+    (tag = the workload: fp32 | bf16 | int8 | fp8 for the layer, gate_<T> for configs[3]) whose `Kernel Name` is the
+    instantiation this run dispatched (forge_last_kernel); (None, reason) if no capture matches."""
+    best = None
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", f"r*_fused_{tag}_full.csv")), reverse=True):
+        name, rd, wr = None, None, None
+        scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+        try:
+            with open(path) as f:
+                for line in f:
+                    parts = line.rstrip("\n").split(",")
+                    if parts[0] == "Kernel Name":
+                        name = line.split(",", 2)[2].strip().strip('"')
+                    elif parts[0] == "dram__bytes_read.sum":
+                        rd = float(parts[2]) * scale.get(parts[1], 1.0)
+                    elif parts[0] == "dram__bytes_write.sum":
+                        wr = float(parts[2]) * scale.get(parts[1], 1.0)
+        except Exception:
+            continue
+        if name and rd is not None and wr is not None and signature and signature in name.replace("forge::", ""):
+            best = {"bytes": rd + wr, "file": os.path.relpath(path, ROOT), "kernel": name}
+            break
+    if best:
+        return best["bytes"], best
+    return None, {"bytes": None, "reason": f"no ncu --set full capture of {signature!r} for workload {tag!r} under profiles/"}
+
+
+# ------------------------------------------------------------------------------------------------
 # CPU oracle timing (cpu_baseline leg and --impl reference)
 # ------------------------------------------------------------------------------------------------
 _CPU_LAYER = {}
 
 
 def oracle_time_sample(frac_den: int, seed: int):
-    """Times the oracle, as it stands, on rows [0, out/frac_den) of every projection of one layer.
-    Returns (seconds, description, threads)."""
+    """Times the oracle, as it stands, on rows [0, out/frac_den) of every projection of one layer (frac_den = 1: the
+    whole layer).  Returns (seconds, description, threads)."""
     from oracle import forge_oracle as fo
     from paper_2606_22932_b200 import synth
     hp = synth.HP_DEFAULT
@@ -173,46 +202,100 @@ def oracle_time_sample(frac_den: int, seed: int):
         G = fo.wgrad(dY, X, rows=(0, r))
         fo.adamw_fp32(W, m, v, G, 10, hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
     dt = time.perf_counter() - t0
-    return dt, f"first 1/{frac_den} of the rows of each of the 7 projections, T=512, fp32 moments, scaled x{frac_den}", fo.num_threads()
+    what = "the whole layer" if frac_den == 1 else f"first 1/{frac_den} of the rows of each projection"
+    return dt, f"{what}: 7 projections, T=512, fp32 moments", fo.num_threads()
 
 
 def cpu_baseline(seed: int):
-    den = 16
-    dt, desc, threads = oracle_time_sample(den, seed)
-    while den > 1 and dt * 4 < 30.0:       # aim at ~10-30 s of CPU work: 1/16, 1/4, then the whole layer
-        den //= 4
+    """The oracle on the host cores over a WHOLE layer when that takes under ~40 s (it does: ~12 s on the GPU box's 16
+    threads); otherwise over the largest 1/4 or 1/16 row sample that does, scaled to the metric's unit, and `sample`
+    says which."""
+    dt, desc, threads = oracle_time_sample(16, seed)
+    den = 1 if dt * 16 < 40.0 else (4 if dt * 4 < 40.0 else 16)
+    if den != 16:
         dt, desc, threads = oracle_time_sample(den, seed)
-    return {"value": dt * den * 1e6, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
-            "sample_seconds": round(dt, 3)}
+    return {"value": dt * den * 1e6, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": desc + ("" if den == 1 else f", scaled x{den}"), "sample_seconds": round(dt, 3)}
 
 
 def run_reference(args):
-    """--impl reference: the oracle on the host cores, rank 0 only."""
+    """--impl reference: the oracle, as it stands, on the host cores; rank 0 only.  Every timed step is ONE WHOLE
+    LAYER (about 12 s on the GPU box's 16 threads): `steps` is the number that actually ran inside a ~100 s budget,
+    never an extrapolation.  The warm-up is one 1/16-layer pass (loads the library, touches the inputs)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    den = 16
-    times = []
-    for i in range(args.warmup + args.steps):
-        dt, desc, threads = oracle_time_sample(den, 20260622 + 1)
-        if i >= args.warmup:
-            times.append(dt)
-        if sum(times) > 150:
+    budget_s = 100.0
+    oracle_time_sample(16, SEED)
+    times, desc, threads = [], "", 0
+    t_begin = time.perf_counter()
+    for _ in range(max(1, args.steps)):
+        dt, desc, threads = oracle_time_sample(1, SEED)
+        times.append(dt)
+        if time.perf_counter() - t_begin + dt > budget_s:
             break
-    us = sum(times) / len(times) * den * 1e6
+    us = sum(times) / len(times) * 1e6
     line = {"impl": "reference", "metric": METRIC, "value": us, "unit": UNIT, "n_gpus": args.gpus,
-            "steps": len(times), "warmup": args.warmup, "ms_per_step": us / 1e3, "higher_is_better": False,
+            "steps": len(times), "warmup": 1, "ms_per_step": us / 1e3, "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "configs[1]: Llama-3.1-8B layer, 7 projections in one grouped launch, T=512",
                        "moments": "fp32", "params_per_layer": layer_counts()[0], "tokens": T_TOKENS},
             "cpu_baseline": {"value": us, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
             "e2e": {"value": us, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "gpu_launches": 0}
+            "gpu_launches": 0,
+            "note": f"requested steps={args.steps} warmup={args.warmup}; ran {len(times)} whole-layer steps (budget {budget_s:.0f} s) after one 1/16-layer warm-up"}
     print(json.dumps(line), flush=True)
 
 
 # ------------------------------------------------------------------------------------------------
-# the CUDA arm
+# timing and roofline helpers of the CUDA arm
 # ------------------------------------------------------------------------------------------------
+def time_steps(step, steps: int, warmup: int, stream, local: int, barrier=None):
+    """W untimed warm-up calls, then exactly K calls bracketed by CUDA events on the launching stream (barrier +
+    synchronize on both sides), NVML clock samples taken while they execute.  step(t) enqueues one step."""
+    import torch
+    for i in range(warmup):
+        step(1 + i)
+    if barrier:
+        barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    evs[0].record(stream)
+    for i in range(steps):
+        step(1 + warmup + i)
+        evs[i + 1].record(stream)
+    time.sleep(0.004)                              # the launches are asynchronous: let the sampler see the GPU under load
+    if barrier:
+        barrier()
+    torch.cuda.synchronize()
+    sampler.stop_flag = True
+    per = sorted(evs[i].elapsed_time(evs[i + 1]) for i in range(steps))
+    return {"total_ms": evs[0].elapsed_time(evs[-1]), "median_ms": per[len(per) // 2], "clocks": sampler.result()}
+
+
+def roofline_obj(params, in_bytes, flops, bytes_per_elem, launch_us, clocks):
+    """Per-shape roofline max(flops / P_bf16, bytes / B_HBM) (north_star) against the MEASURED peaks.  The tensor term
+    takes the cuBLAS figure of the power state the timed region ran in (B200_PROFILING.md): K launches that stay at
+    the boost clock are a burst measurement, a region that reached the power cap is compared with the sustained one."""
+    hbm_peak, tf_burst, tf_sus, peak_src = measured_peaks()
+    alg_bytes = params * bytes_per_elem + in_bytes
+    gbs, tfs = alg_bytes / launch_us / 1e3, flops / launch_us / 1e6
+    capped = "sw_power_cap" in clocks["reasons"] or bool(clocks["sm_mhz"] and clocks["sm_max_mhz"] and clocks["sm_mhz"] < 0.95 * clocks["sm_max_mhz"])
+    tf_peak, tf_kind = (tf_sus, "sustained") if capped else (tf_burst, "burst")
+    t_hbm, t_tc = alg_bytes / hbm_peak / 1e3, flops / tf_peak / 1e6
+    if t_hbm >= t_tc:
+        r = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak}
+    else:
+        r = {"bound": "tensor", "achieved": tfs, "peak": tf_peak, "unit": "TFLOP/s", "frac": tfs / tf_peak,
+             "peak_kind": tf_kind, "burst_peak": tf_burst, "sustained_peak": tf_sus}
+    r.update({"traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes, "flops_per_launch": flops,
+              "roofline_us": max(t_hbm, t_tc), "hbm_term_us": t_hbm, "tensor_term_us": t_tc,
+              "frac_of_max_term": max(t_hbm, t_tc) / launch_us, "launch_us_avg": launch_us, "gbs": gbs, "tflops": tfs,
+              "frac_of_datasheet_8TBs": gbs / 8000.0, "frac_of_datasheet_2250TF": tfs / 2250.0})
+    return r, flops / tf_sus / 1e6
+
+
 def time_unfused_baselines(layer, hp, steps):
     """Context arms on the same GPU: cuBLAS dW then a separate optimizer pass.
     B3: fp32 dW (cuBLAS via torch.mm) + this library's elementwise kernel over the materialised G
@@ -222,20 +305,19 @@ def time_unfused_baselines(layer, hp, steps):
     from paper_2606_22932_b200 import binding as fb
     res = {}
     Gs = [torch.empty(d["W"].shape, dtype=torch.float32, device=d["W"].device) for d in layer]
+    has_out_dtype = True
+    try:
+        torch.mm(layer[1]["dY"].t(), layer[1]["X"], out_dtype=torch.float32)
+    except Exception:
+        has_out_dtype = False
 
     def run_b3():
         for d, G in zip(layer, Gs):
-            if HAS_OUT_DTYPE[0]:
+            if has_out_dtype:
                 torch.mm(d["dY"].t(), d["X"], out_dtype=torch.float32, out=G)
             else:   # bf16 cuBLAS output widened afterwards (torch build without out_dtype)
                 G.copy_(torch.mm(d["dY"].t(), d["X"]))
             fb.forge_adamw_from_g(G, d["W"], d["m"], d["v"], 10, hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"])
-
-    HAS_OUT_DTYPE = [True]
-    try:
-        torch.mm(layer[1]["dY"].t(), layer[1]["X"], out_dtype=torch.float32)
-    except Exception:
-        HAS_OUT_DTYPE[0] = False
 
     def timeit(fn, n):
         for _ in range(2):
@@ -251,7 +333,7 @@ def time_unfused_baselines(layer, hp, steps):
 
     if layer[0]["m"].dtype == torch.float32:
         res["cublas_dw_fp32_plus_elementwise_adamw_us"] = timeit(run_b3, steps)
-        res["cublas_dw_out_dtype_fp32"] = HAS_OUT_DTYPE[0]
+        res["cublas_dw_out_dtype_fp32"] = has_out_dtype
     try:
         Wb = [d["W"].clone() for d in layer]
         mb = [torch.zeros_like(w) for w in Wb]
@@ -269,59 +351,126 @@ def time_unfused_baselines(layer, hp, steps):
     return res
 
 
-def run_model(args):
+def backward_leg(layer, hpt, mdt, steps, stream, local):
+    """forge_layer_backward_grouped (the hand-written tcgen05 dgrad of all 7 projections in one
+    launch, then the fused launch) next to cuBLAS dgrad (torch.mm, 7 GEMMs) + the same fused call, on this box."""
+    import torch
+    from paper_2606_22932_b200 import binding as fb
+    dXs = [torch.empty((d["X"].shape[0], d["W"].shape[1]), dtype=torch.bfloat16, device=d["W"].device) for d in layer]
+    arr = fb.make_problem_array(layer)
+    flops = sum(2.0 * d["X"].shape[0] * d["W"].shape[0] * d["W"].shape[1] for d in layer)
+
+    def ours(t):
+        fb.forge_layer_backward_grouped(layer, dXs, t, *hpt, mdt, stream=stream)
+
+    def cublas(t):
+        for d, dX in zip(layer, dXs):
+            torch.mm(d["dY"], d["W"], out=dX)
+        fb.forge_wgrad_adamw_grouped(layer, t, *hpt, mdt, stream=stream, _arr=arr)
+
+    def cublas_dgrad_only(t):
+        for d, dX in zip(layer, dXs):
+            torch.mm(d["dY"], d["W"], out=dX)
+
+    a = time_steps(ours, steps, 3, stream, local)
+    sig = fb.lib().forge_last_kernel().decode()
+    b = time_steps(cublas, steps, 3, stream, local)
+    c = time_steps(cublas_dgrad_only, steps, 3, stream, local)
+    f = time_steps(lambda t: fb.forge_wgrad_adamw_grouped(layer, t, *hpt, mdt, stream=stream, _arr=arr), steps, 3, stream, local)
+    ours_us, fused_us = a["total_ms"] / steps * 1e3, f["total_ms"] / steps * 1e3
+    dgrad_us = max(ours_us - fused_us, 1e-3)
+    _, tf_burst, tf_sus, _ = measured_peaks()
+    return {"value": ours_us, "unit": UNIT, "api": "forge_layer_backward_grouped: 1 dgrad launch (tcgen05, all 7 projections) + 1 fused launch",
+            "fused_step_alone_us": fused_us, "dgrad_us_by_difference": dgrad_us, "dgrad_tflops": flops / dgrad_us / 1e6,
+            "dgrad_frac_of_bf16_burst_peak": flops / dgrad_us / 1e6 / tf_burst, "dgrad_flops": flops,
+            "cublas_dgrad_plus_fused_us": b["total_ms"] / steps * 1e3, "cublas_dgrad_alone_us": c["total_ms"] / steps * 1e3,
+            "cublas_dgrad_tflops": flops / (c["total_ms"] / steps * 1e3) / 1e6, "last_kernel": sig, "clocks": a["clocks"]}
+
+
+def model_leg(dev, tokens: int, steps: int, with_pool: bool):
     """BASELINE.json configs[4]: 32 layers + lm_head resident (75 GB of state), one optimizer step layer by
     layer in reverse order; total step time and peak device memory with and without a materialised dW pool."""
     import torch
     from paper_2606_22932_b200 import binding as fb
     from paper_2606_22932_b200 import stack, synth
-    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
-    torch.cuda.set_device(dev)
-    fb.lib()
     hp = synth.HP_DEFAULT
     free0, total = torch.cuda.mem_get_info()
-    st = stack.build_stack(dev, tokens=args.tokens)
+    need = 7_504_658_432 * 10 + (3 << 30)
+    if free0 < need:
+        return {"skipped": f"configs[4] needs {need / 1e9:.1f} GB of free device memory, {free0 / 1e9:.1f} GB available"}
+    st = stack.build_stack(dev, tokens=tokens)
     torch.cuda.synchronize()
     stream = torch.cuda.current_stream()
+    local = dev.index or 0
 
     def timed(fn, n, warm):
-        for i in range(warm):
-            fn(1 + i)
-        torch.cuda.synchronize()
         torch.cuda.reset_peak_memory_stats()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        for i in range(n):
-            fn(1 + warm + i)
-        e1.record(stream)
-        torch.cuda.synchronize()
-        return e0.elapsed_time(e1) / n, torch.cuda.max_memory_allocated()
+        r = time_steps(fn, n, warm, stream, local)
+        return r["total_ms"] / n, torch.cuda.max_memory_allocated(), r["clocks"]
 
-    n = max(1, min(args.steps, 5))
+    n = max(1, min(steps, 5))
     launches0 = fb.forge_launch_count()
-    fused_ms, fused_peak = timed(lambda t: stack.step_fused(st, t, hp, stream), n, 1)
+    fused_ms, fused_peak, clocks = timed(lambda t: stack.step_fused(st, t, hp, stream), n, 1)
     launches = (fb.forge_launch_count() - launches0) // (n + 1)
     alg_bytes = st.params * 20.0 + st.input_bytes
-    hbm_peak, tf_burst, tf_sus, peak_src = measured_peaks()
-    pool = stack.alloc_dw_pool(st, dev)
-    pool_bytes = sum(g.numel() * 4 for layer in pool for g in layer)
-    pool_ms, pool_peak = timed(lambda t: stack.step_dw_pool(st, pool, t, hp), max(1, n // 2), 1)
+    hbm_peak, _, _, peak_src = measured_peaks()
     gbs = alg_bytes / (fused_ms * 1e-3) / 1e9
+    out = {"value": fused_ms, "unit": "ms/step", "steps": n, "warmup": 1,
+           "workload": "configs[4]: 32 x 7 projections + lm_head[128256,4096], bf16 W + fp32 m/v resident, reverse layer order",
+           "params": st.params, "state_bytes": st.state_bytes, "input_bytes": st.input_bytes, "tokens": tokens,
+           "roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak, "traffic": None,
+                        "peak_source": peak_src, "algorithmic_bytes_per_step": alg_bytes, "roofline_ms": alg_bytes / hbm_peak / 1e6},
+           "gpu_launches_per_step": int(launches), "clocks": clocks,
+           "peak_device_memory": {"fused_bytes": int(fused_peak), "dw_bytes_allocated_by_fused_path": 0,
+                                  "device_total_bytes": int(total)}}
+    if with_pool:
+        pool = stack.alloc_dw_pool(st, dev)
+        pool_bytes = sum(g.numel() * 4 for layer in pool for g in layer)
+        pool_ms, pool_peak, _ = timed(lambda t: stack.step_dw_pool(st, pool, t, hp), max(1, n // 2), 1)
+        out["peak_device_memory"].update({"dw_pool_arm_bytes": int(pool_peak), "dw_pool_bytes": int(pool_bytes)})
+        out["dw_pool_arm"] = {"ms_per_step": pool_ms, "what": "cuBLAS fp32 dW for all layers into a 30 GB pool, then elementwise AdamW over the pool"}
+        out["speedup_vs_dw_pool_arm"] = pool_ms / fused_ms
+        del pool
+    del st
+    torch.cuda.empty_cache()
+    return out
+
+
+def run_model(args):
+    import torch
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    r = model_leg(dev, args.tokens, args.steps, with_pool=True)
+    if "skipped" in r:
+        raise SystemExit(r["skipped"])
     line = {"metric": "full Llama-3.1-8B linear stack optimizer step, ms (32 layers + lm_head, BT=%d, 1xB200)" % args.tokens,
-            "value": fused_ms, "unit": "ms/step", "n_gpus": 1, "steps": n, "warmup": 1, "ms_per_step": fused_ms,
+            "value": r["value"], "unit": "ms/step", "n_gpus": 1, "steps": r["steps"], "warmup": 1, "ms_per_step": r["value"],
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": "configs[4]: 32 x 7 projections + lm_head[128256,4096], bf16 W + fp32 m/v resident, reverse layer order",
-                       "params": st.params, "state_bytes": st.state_bytes, "input_bytes": st.input_bytes, "tokens": args.tokens,
-                       "l2": "75 GB working set >> 126 MB L2"},
-            "roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak, "traffic": None,
-                         "peak_source": peak_src, "algorithmic_bytes_per_step": alg_bytes, "roofline_ms": alg_bytes / hbm_peak / 1e6},
-            "gpu_launches": int(launches),
-            "peak_device_memory": {"fused_bytes": int(fused_peak), "dw_pool_arm_bytes": int(pool_peak),
-                                   "dw_pool_bytes": int(pool_bytes), "dw_bytes_allocated_by_fused_path": 0,
-                                   "device_total_bytes": int(total)},
-            "dw_pool_arm": {"ms_per_step": pool_ms, "what": "cuBLAS fp32 dW for all layers into a 30 GB pool, then elementwise AdamW over the pool"},
-            "speedup_vs_dw_pool_arm": pool_ms / fused_ms}
+            "config": {"workload": r["workload"], "params": r["params"], "state_bytes": r["state_bytes"],
+                       "input_bytes": r["input_bytes"], "tokens": args.tokens, "l2": "75 GB working set >> 126 MB L2"},
+            "roofline": r["roofline"], "gpu_launches": r["gpu_launches_per_step"] * r["steps"], "clocks": r["clocks"],
+            "peak_device_memory": r["peak_device_memory"], "dw_pool_arm": r.get("dw_pool_arm"),
+            "speedup_vs_dw_pool_arm": r.get("speedup_vs_dw_pool_arm")}
     print(json.dumps(line), flush=True)
+
+
+def config_leg(name, moments, workload, tokens, dev, steps, hpt, stream, local, tag):
+    """One extra BASELINE.json configuration inside the default run: build, time K launches, free."""
+    import torch
+    from paper_2606_22932_b200 import binding as fb
+    layer = make_device_layer(moments, SEED, dev, workload, tokens)
+    arr = fb.make_problem_array(layer)
+    mdt = MOMENT_ENUM[moments]
+    r = time_steps(lambda t: fb.forge_wgrad_adamw_grouped(layer, t, *hpt, mdt, stream=stream, _arr=arr), steps, 3, stream, local)
+    sig = fb.lib().forge_last_kernel().decode()
+    us = r["total_ms"] / steps * 1e3
+    params, in_bytes, flops = layer_counts(workload, tokens)
+    roof, _ = roofline_obj(params, in_bytes, flops, MOMENT_BYTES[moments], us, r["clocks"])
+    roof["traffic"], roof["traffic_source"] = ncu_traffic(sig, tag)
+    del layer, arr
+    torch.cuda.empty_cache()
+    return {"config": name, "us": us, "launch_us_median": r["median_ms"] * 1e3, "steps": steps, "moments": moments,
+            "workload": workload, "tokens": tokens, "kernel": sig, "roofline": roof, "clocks": r["clocks"]}
 
 
 def run_cuda(args):
@@ -344,7 +493,16 @@ def run_cuda(args):
     fb.lib()                                       # fails loudly if the CUDA library is missing
     hp = synth.HP_DEFAULT
     mdt = MOMENT_ENUM[args.moments]
-    layer = make_device_layer(args.moments, 20260622 + 1 + rank, dev, args.workload, args.tokens)
+    sharded = args.shard == "rows" and world > 1
+    # replicas: every rank its own layer (own seed); --shard rows: ONE layer (same seed everywhere), each rank keeps
+    # its 128-aligned row range of every W / m / v and the matching column slice of dY (shard.py; Prop. 2(i))
+    layer = make_device_layer(args.moments, SEED + (0 if sharded else rank), dev, args.workload, args.tokens)
+    if sharded:
+        if args.moments == "fp8":
+            raise SystemExit("--shard rows: fp8 moments keep one scale per TENSOR; shard fp32 / bf16 / int8 state")
+        full = layer
+        layer = [s for s in (shard.shard_problem(d, world, rank) for d in full) if s is not None]
+        layer = [{k: v for k, v in d.items() if k != "rows"} for d in layer]
     nst = fb.FAMILY_STATES.get(args.optimizer, 0)
     if args.optimizer == "storeg":
         if args.workload in ("layer", "model"):
@@ -363,17 +521,17 @@ def run_cuda(args):
     # re-stepping one, the footprint a real model presents (profiles/r01_summary.md, "Footprint")
     rot = [(layer, arr)]
     if args.distinct_layers > 1:
-        if args.optimizer != "adamw":
-            raise SystemExit("--distinct-layers is implemented for --optimizer adamw")
+        if args.optimizer != "adamw" or sharded:
+            raise SystemExit("--distinct-layers is implemented for --optimizer adamw, unsharded")
         for k in range(1, args.distinct_layers):
-            lk = make_device_layer(args.moments, 20260622 + 1000 * k + rank, dev, args.workload, args.tokens)
+            lk = make_device_layer(args.moments, SEED + 1000 * k + rank, dev, args.workload, args.tokens)
             rot.append((lk, fb.make_problem_array(lk)))
 
     G_ctl = torch.empty(layer[0]["W"].shape, dtype=torch.float32, device=dev) if args.optimizer == "storeg" else None
     dp_plan = dp_pool = None
     if args.schedule == "bucket":                    # the data-parallel bucket-transient schedule
-        if args.optimizer != "adamw" or args.moments == "fp8" or args.distinct_layers > 1:
-            raise SystemExit("--schedule bucket: AdamW with fp32 / bf16 / int8 moments")
+        if args.optimizer != "adamw" or args.moments == "fp8" or args.distinct_layers > 1 or sharded:
+            raise SystemExit("--schedule bucket: AdamW with fp32 / bf16 / int8 moments, unsharded")
         from paper_2606_22932_b200 import dp
         dp_plan = dp.BucketPlan([tuple(d["W"].shape) for d in layer], args.bucket_mb << 20, slots=2)
         dp_pool = [torch.empty(dp_plan.slot_elems, dtype=torch.float32, device=dev) for _ in range(dp_plan.slots)]
@@ -382,7 +540,7 @@ def run_cuda(args):
         if args.optimizer == "storeg":             # the paper's store-G control: same mainloop, G stored
             fb.forge_wgrad_store_g(layer[0]["X"], layer[0]["dY"], G_ctl, stream=stream)
         elif dp_plan is not None:                      # store-G into the rotating bucket, (all-reduce,) update from it
-            dp.bucket_step_adamw(layer, t, hpt, dp_plan, dp_pool, group=None)
+            dp.bucket_step_adamw(layer, t, hpt, dp_plan, dp_pool, group=dist.group.WORLD if world > 1 else None)
         elif args.optimizer == "adamw":
             lk, ak = rot[t % len(rot)]
             fb.forge_wgrad_adamw_grouped(lk, t, *hpt, mdt, stream=stream, _arr=ak)
@@ -395,72 +553,53 @@ def run_cuda(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for i in range(args.warmup):
-        step(1 + i)
-    barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
     launches0 = fb.forge_launch_count()
-    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    evs[0].record(stream)
-    for i in range(args.steps):
-        step(1 + args.warmup + i)
-        evs[i + 1].record(stream)
-    time.sleep(0.004)                              # the launches are asynchronous: let the sampler see the GPU under load
-    barrier()
-    sampler.stop_flag = True
-    launches = fb.forge_launch_count() - launches0
-    total_ms = evs[0].elapsed_time(evs[-1])
-    per_launch_ms = sorted(evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps))
-    total_ms = shard.max_over_ranks(total_ms, device=dev)
+    r = time_steps(step, args.steps, args.warmup, stream, local, barrier)
+    launches = fb.forge_launch_count() - launches0 - 0
+    launches = launches * args.steps // (args.steps + args.warmup)
+    signature = fb.lib().forge_last_kernel().decode()
+    total_ms = shard.max_over_ranks(r["total_ms"], device=dev)
     ms_per_step = total_ms / args.steps
-    us_per_layer = ms_per_step * 1e3 / world       # layers processed by all ranks per step = world
+    layers_per_step = 1 if sharded else world          # shards: all ranks together step ONE layer
+    us_per_layer = ms_per_step * 1e3 / layers_per_step
 
     params, in_bytes, flops = layer_counts(args.workload, args.tokens)
+    if sharded:                                        # this rank's share of the launch (its rows; X whole, dY its columns)
+        params = sum(d["W"].numel() for d in layer)
+        flops = 2 * params * args.tokens
+        xs = {d["X"].data_ptr(): d["X"].numel() for d in layer}
+        in_bytes = 2 * (sum(xs.values()) + sum(d["dY"].shape[0] * d["dY"].shape[1] for d in layer))
     state_b = {"fp32": 8.0, "bf16": 4.0}.get(args.moments, 0.0)
-    alg_bytes = params * (MOMENT_BYTES[args.moments] if args.optimizer == "adamw" else
-                          (4.0 if args.optimizer == "storeg" else 4.0 + nst * state_b)) + in_bytes   # store-G: 4 B/element of G out
-    hbm_peak, tf_burst, tf_sustained, peak_src = measured_peaks()
-    kernel_ms = (evs[0].elapsed_time(evs[-1])) / args.steps       # this rank's average launch duration
-    gbs = alg_bytes / (kernel_ms * 1e-3) / 1e9
-    tfs = flops / (kernel_ms * 1e-3) / 1e12
-    # per-shape roofline max(flops / P_bf16, bytes / B_HBM) (north_star).  The tensor term takes the cuBLAS figure of
-    # the power state the timed region actually ran in (B200_PROFILING.md): K launches that stay at the boost clock
-    # are a burst measurement; a region that reached the power cap is compared with the sustained figure
-    clk = sampler.result()
-    capped = "sw_power_cap" in clk["reasons"] or (clk["sm_mhz"] and clk["sm_max_mhz"] and clk["sm_mhz"] < 0.95 * clk["sm_max_mhz"])
-    tf_peak, tf_kind = (tf_sustained, "sustained") if capped else (tf_burst, "burst")
-    t_hbm_us, t_tensor_us = alg_bytes / hbm_peak / 1e3, flops / tf_peak / 1e6
-    t_tensor_sus_us = flops / tf_sustained / 1e6
-    if t_hbm_us >= t_tensor_us:
-        roofline = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak}
-    else:
-        roofline = {"bound": "tensor", "achieved": tfs, "peak": tf_peak, "unit": "TFLOP/s", "frac": tfs / tf_peak,
-                    "peak_kind": tf_kind, "burst_peak": tf_burst, "sustained_peak": tf_sustained}
-    is_headline = args.workload == "layer" and args.tokens == T_TOKENS and args.optimizer == "adamw" and dp_plan is None
-    roofline.update({"traffic": NCU_TRAFFIC_BYTES[args.moments] if is_headline else None, "peak_source": peak_src,
-                     "algorithmic_bytes_per_launch": alg_bytes, "flops_per_launch": flops,
-                     "roofline_us": max(t_hbm_us, t_tensor_us), "hbm_term_us": t_hbm_us, "tensor_term_us": t_tensor_us,
-                     "launch_us_avg": kernel_ms * 1e3,
-                     "launch_us_median": per_launch_ms[len(per_launch_ms) // 2] * 1e3,
-                     "gbs": gbs, "tflops": tfs, "frac_of_datasheet_8TBs": gbs / 8000.0,
-                     "frac_of_datasheet_2250TF": tfs / 2250.0})
+    bpe = (MOMENT_BYTES[args.moments] if args.optimizer == "adamw" else
+           (4.0 if args.optimizer == "storeg" else 4.0 + nst * state_b))          # store-G: 4 B/element of G out
+    kernel_us = r["total_ms"] / args.steps * 1e3          # this rank's average launch duration
+    clk = r["clocks"]
+    roofline, t_tensor_sus_us = roofline_obj(params, in_bytes, flops, bpe, kernel_us, clk)
+    roofline["launch_us_median"] = r["median_ms"] * 1e3
+    is_headline = (args.workload == "layer" and args.tokens == T_TOKENS and args.optimizer == "adamw" and dp_plan is None
+                   and not sharded)
+    tag = args.moments if args.workload == "layer" else f"{args.workload}_{args.tokens}"
+    if args.optimizer == "adamw" and dp_plan is None and not sharded and (args.workload == "layer" or args.moments == "fp32"):
+        roofline["traffic"], roofline["traffic_source"] = ncu_traffic(signature, tag)
+    roofline["kernel"] = signature
 
     line = {"metric": METRIC, "value": us_per_layer, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False,
+            "scaling": "strong" if sharded else "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": (("configs[1]: Llama-3.1-8B layer, 7 projections in one grouped launch, T=512"
                                      if args.moments == "fp32" else f"configs[2]: same layer, {args.moments} moments")
-                                    if is_headline else f"configs[3]-style: {args.workload} of a Llama-3.1-8B layer, T={args.tokens}, "
+                                    if (is_headline or sharded) else f"configs[3]-style: {args.workload} of a Llama-3.1-8B layer, T={args.tokens}, "
                                     f"{args.optimizer} with {nst} {args.moments} state tensor(s)"),
-                       "moments": args.moments, "params_per_layer": params, "tokens": args.tokens,
+                       "moments": args.moments, "params_per_layer": layer_counts(args.workload, args.tokens)[0], "tokens": args.tokens,
                        "distinct_layers": len(rot),
                        "schedule": ("fused" if dp_plan is None else
                                     f"dp bucket-transient: {len(dp_plan.buckets)} buckets, {dp_plan.transient_bytes >> 20} MiB of fp32 "
                                     f"gradient in flight, all-reduce over {world} rank(s)"),
                        "l2": "working set 4.4 GB/layer >> 126 MB L2, no flush needed",
-                       "parallelism": f"replicated layers x{world}, no collective"},
-            "roofline": roofline, "gpu_launches": int(launches), "clocks": sampler.result(),
+                       "parallelism": (f"one layer row-sharded over {world} ranks (shard.py), no collective" if sharded
+                                       else f"replicated layers x{world}, no collective")},
+            "roofline": roofline, "gpu_launches": int(launches), "clocks": clk,
             "dw_bytes_allocated": 0 if dp_plan is None else dp_plan.transient_bytes,
             "library_workspace_bytes": fb.forge_workspace_bytes()}
 
@@ -486,12 +625,14 @@ def run_cuda(args):
         sus_sampler.stop_flag = True
         sus_us = s_evs[0].elapsed_time(s_evs[1]) / n_tail * 1e3
         line["sustained"] = {"value": sus_us, "unit": UNIT, "launches": n_sus, "timed": f"last {n_tail} launches",
-                             "frac": max(t_hbm_us, t_tensor_sus_us) / sus_us, "tensor_peak_kind": "sustained",
-                             "clocks": sus_sampler.result()}
+                             "frac": max(roofline["hbm_term_us"], t_tensor_sus_us) / sus_us, "tensor_peak_kind": "sustained",
+                             "ratio_to_boost": sus_us / kernel_us, "clocks": sus_sampler.result()}
         time.sleep(1.0)                            # let the power state recover before the other legs
+    if rank == 0 and world == 1 and args.backward:
+        line["layer_backward"] = backward_leg(layer, hpt, mdt, max(5, min(args.steps, 20)), stream, local)
     if rank == 0 and not args.no_extras and is_headline:
         # ---- end to end through the C ABI with HOST buffers (H2D + kernel + D2H inside the call)
-        host = make_host_layer(args.moments, 20260622 + 1)
+        host = make_host_layer(args.moments, SEED)
         h2d = sum(sum(v.numel() * v.element_size() for v in d.values()) for d in host)
         d2h = sum(sum(d[k].numel() * d[k].element_size() for k in d if k not in ("X", "dY")) for d in host)
         host_arr = fb.make_problem_array(host)
@@ -508,13 +649,39 @@ def run_cuda(args):
         line["e2e"] = {"value": e2e_us, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                        "steps": n_e2e, "api": "forge_wgrad_adamw_grouped_host, 7 problems pipelined over 3 streams (pinned host buffers)"}
         del host
-        line["baselines_same_gpu"] = time_unfused_baselines(layer, hp, max(3, min(10, args.steps)))
         if world == 1:
-            line["cpu_baseline"] = cpu_baseline(20260622 + 1)
+            if not args.backward:
+                line["layer_backward"] = backward_leg(layer, hpt, mdt, 10, stream, local)
+            line["baselines_same_gpu"] = time_unfused_baselines(layer, hp, max(3, min(10, args.steps)))
+            # ---- the other BASELINE.json configurations, timed on this box in this run
+            del layer, arr, rot
+            torch.cuda.empty_cache()
+            k = max(10, min(args.steps, 20))
+            cfgs = []
+            for name, mom, wl, tok, tag2 in (("configs[2] bf16 moments", "bf16", "layer", 512, "bf16"),
+                                             ("configs[2] int8 moments", "int8", "layer", 512, "int8"),
+                                             ("fp8 moments (8(f) rank 1)", "fp8", "layer", 512, "fp8"),
+                                             ("configs[3] gate T=512", "fp32", "gate", 512, "gate_512"),
+                                             ("configs[3] gate T=2048", "fp32", "gate", 2048, "gate_2048"),
+                                             ("configs[3] gate T=8192", "fp32", "gate", 8192, "gate_8192")):
+                cfgs.append(config_leg(name, mom, wl, tok, dev, k, hpt, stream, local, tag2))
+                time.sleep(0.3)
+            m4 = model_leg(dev, T_TOKENS, 3, with_pool=False)
+            m4["config"] = "configs[4] full stack"
+            cfgs.append(m4)
+            line["configs"] = cfgs
+            line["cpu_baseline"] = cpu_baseline(SEED)
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def _spawn_entry(rank: int, world: int, port: int, argv):
+    os.environ.update({"RANK": str(rank), "LOCAL_RANK": str(rank), "WORLD_SIZE": str(world),
+                       "MASTER_ADDR": "127.0.0.1", "MASTER_PORT": str(port)})
+    sys.argv = argv
+    main()
 
 
 def main():
@@ -534,14 +701,36 @@ def main():
     ap.add_argument("--schedule", choices=["fused", "bucket"], default="fused",
                     help="bucket = the data-parallel schedule of dp.py (gradient through a rotating fp32 bucket)")
     ap.add_argument("--bucket-mb", type=int, default=256)
+    ap.add_argument("--shard", choices=["none", "rows"], default="none",
+                    help="rows = N > 1 ranks split ONE layer's weight rows (strong scaling); none = one layer per rank (weak)")
+    ap.add_argument("--backward", action="store_true", help="add the layer-backward leg (dgrad + fused step) with --no-extras / other modes")
     ap.add_argument("--sustained", action="store_true", help="add the sustained-load leg even with --no-extras / other workloads")
-    ap.add_argument("--no-extras", action="store_true", help="skip e2e, same-GPU baselines and the CPU oracle leg")
+    ap.add_argument("--no-extras", action="store_true", help="skip e2e, same-GPU baselines, the extra configs and the CPU oracle leg")
+    ap.add_argument("--profiling-lib", action="store_true",
+                    help="load libforge_b200_prof.so (the -DFORGE_PROFILING build: FORGE_CFG / FORGE_GRID / FORGE_ABLATE); profiles/ commands only")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     if args.impl == "reference":
-        run_reference(args)
-    else:
-        run_cuda(args)
+        return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # no launcher: spawn the ranks here, one per GPU, NCCL's communicator lines (NCCL_DEBUG=INFO) to stderr
+        import socket
+        import torch
+        if torch.cuda.device_count() < args.gpus:
+            raise SystemExit(f"bench.py --gpus {args.gpus}: only {torch.cuda.device_count()} CUDA device(s) visible")
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+        os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
+        with socket.socket() as s:
+            s.bind(("127.0.0.1", 0))
+            port = s.getsockname()[1]
+        import torch.multiprocessing as mp
+        mp.spawn(_spawn_entry, args=(args.gpus, port, list(sys.argv)), nprocs=args.gpus, join=True)
+        return
+    if args.profiling_lib:
+        from paper_2606_22932_b200 import binding as fb
+        fb.use_profiling_library(True)
+    run_cuda(args)
 
 
 if __name__ == "__main__":

@@ -22,6 +22,11 @@ struct AdamWScalars {
     float inv_sqrt_bc2;             // 1 / sqrt(1 - beta2^t)
     float eps;
     float decay;                    // 1 - lr*wd   (decoupled decay on the pre-update W)
+    // int8 moments work on the SCALED moments m'' = m'/(1-beta1), v'' = v'/(1-beta2) (adamw_moments2_qs): one FMA
+    // each instead of a multiply and an FMA; the codes are scale-invariant and the factors fold into constants
+    float q_b1, q_b2;               // beta/(1-beta)
+    float q_c;                      // sqrt(1-beta2) / (sqrt(1-beta2^t) (1-beta1)):  m'/(sqrt(v'/bc2)+eps) = m''/(sqrt(v'') q_c + q_eps)
+    float q_eps;                    // eps/(1-beta1)
 };
 
 // ------------------------------------------------------------------ packed fp32 pairs ------
@@ -90,6 +95,18 @@ __device__ __forceinline__ void adamw_moments2_q(const AdamWScalars &h, f32x2 g,
                                                  float bm, float bv, f32x2 &m, f32x2 &v) {
     m = fma2(bc2(bm), code_m, mul2(bc2(h.one_minus_beta1), g));
     v = fma2(bc2(bv), code_v, mul2(mul2(bc2(h.one_minus_beta2), g), g));
+}
+// int8 state on the scaled moments: m'' = m'/(1-b1) = (b1/(1-b1) a/L) code + g, v'' = (b2/(1-b2) a/L) code + g^2.
+// bmq = fp32(q_b1 * fp32(a_m/127)), bvq likewise.  max|m''| (1-b1) is the stored block absmax; code = rint(m'' L/max|m''|).
+__device__ __forceinline__ void adamw_moments2_qs(f32x2 g, f32x2 code_m, f32x2 code_v, float bmq, float bvq, f32x2 &m, f32x2 &v) {
+    m = fma2(bc2(bmq), code_m, g);
+    v = fma2(bc2(bvq), code_v, mul2(g, g));
+}
+__device__ __forceinline__ void adamw_weight2_s(const AdamWScalars &h, f32x2 m, f32x2 v, f32x2 &w) {
+    const f32x2 sq = pk2(sqrt_fast(lo2(v)), sqrt_fast(hi2(v)));
+    const f32x2 denom = fma2(sq, bc2(h.q_c), bc2(h.q_eps));
+    const f32x2 ratio = mul2(m, pk2(rcp_fast(lo2(denom)), rcp_fast(hi2(denom))));
+    w = fma2(bc2(-h.step_size), ratio, mul2(bc2(h.decay), w));
 }
 // W' = (1 - lr wd) W - lr * (m'/bc1) / (sqrt(v'/bc2) + eps)          (Alg. 1 lines 9-10)
 // sqrt(v'/bc2) is evaluated as sqrt(v') * (1/sqrt(bc2)); W' uses the unrounded m', v'.

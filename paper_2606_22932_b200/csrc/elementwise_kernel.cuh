@@ -60,8 +60,8 @@ forge_adamw_from_g_kernel(const float *__restrict__ G, uint16_t *__restrict__ W,
             *reinterpret_cast<uint4 *>(static_cast<uint16_t *>(vp) + base) =
                 make_uint4(f32x2_to_bf16x2(v[0]), f32x2_to_bf16x2(v[1]), f32x2_to_bf16x2(v[2]), f32x2_to_bf16x2(v[3]));
         } else {
-            const float bm = __fmul_rn(hp.beta1, dequant_step(m_scale[base / 256], 127.0f));
-            const float bv = __fmul_rn(hp.beta2, dequant_step(v_scale[base / 256], 255.0f));
+            const float bm = __fmul_rn(hp.q_b1, dequant_step(m_scale[base / 256], 127.0f));     // scaled moments m'', v''
+            const float bv = __fmul_rn(hp.q_b2, dequant_step(v_scale[base / 256], 255.0f));
             const uint2 a = *reinterpret_cast<const uint2 *>(static_cast<const uint8_t *>(mp) + base);
             const uint2 c = *reinterpret_cast<const uint2 *>(static_cast<const uint8_t *>(vp) + base);
             f32x2 cm[4], cv[4];
@@ -71,8 +71,8 @@ forge_adamw_from_g_kernel(const float *__restrict__ G, uint16_t *__restrict__ W,
             codes4_to_f32(c.y, false, cv[2], cv[3]);
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
-                adamw_moments2_q(hp, g[e], cm[e], cv[e], bm, bv, m[e], v[e]);
-                adamw_weight2(hp, m[e], v[e], w[e]);
+                adamw_moments2_qs(g[e], cm[e], cv[e], bm, bv, m[e], v[e]);
+                adamw_weight2_s(hp, m[e], v[e], w[e]);
             }
         }
         *reinterpret_cast<uint4 *>(W + base) = make_uint4(f32x2_to_bf16x2(w[0]), f32x2_to_bf16x2(w[1]),
@@ -98,9 +98,9 @@ forge_adamw_from_g_kernel(const float *__restrict__ G, uint16_t *__restrict__ W,
             const uint32_t v1 = pack_codes4(quant_v2(v[2], inv_v, v_floor), quant_v2(v[3], inv_v, v_floor));
             *reinterpret_cast<uint2 *>(static_cast<uint8_t *>(mp) + base) = make_uint2(m0, m1);
             *reinterpret_cast<uint2 *>(static_cast<uint8_t *>(vp) + base) = make_uint2(v0, v1);
-            if ((threadIdx.x & 31) == 0) {
-                m_scale[base / 256] = a_m;
-                v_scale[base / 256] = a_v;
+            if ((threadIdx.x & 31) == 0) {          // stored absmax of m', v' = (1 - beta) max of the scaled moments
+                m_scale[base / 256] = __fmul_rn(hp.one_minus_beta1, a_m);
+                v_scale[base / 256] = __fmul_rn(hp.one_minus_beta2, a_v);
             }
         }
     }

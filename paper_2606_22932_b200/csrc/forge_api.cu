@@ -184,6 +184,11 @@ AdamWScalars make_scalars(int64_t step, float lr, float b1, float b2, float eps,
     h.inv_sqrt_bc2 = static_cast<float>(1.0 / std::sqrt(bc2));
     h.eps = eps;
     h.decay = static_cast<float>(1.0 - static_cast<double>(lr) * static_cast<double>(wd));
+    const double d1 = 1.0 - static_cast<double>(b1), d2 = 1.0 - static_cast<double>(b2);
+    h.q_b1 = static_cast<float>(static_cast<double>(b1) / d1);
+    h.q_b2 = static_cast<float>(static_cast<double>(b2) / d2);
+    h.q_c = static_cast<float>(std::sqrt(d2) / (std::sqrt(bc2) * d1));
+    h.q_eps = static_cast<float>(static_cast<double>(eps) / d1);
     return h;
 }
 

@@ -38,13 +38,9 @@ constexpr int BLOCK_M = 128;   // tile rows  (out)  = TMEM lanes
 constexpr int BLOCK_N = 256;   // tile cols  (in)   = TMEM columns = one int8 block per row
 constexpr int SUB = 32;        // epilogue sub-block: 32 rows (one warp's TMEM lanes) x 32 columns
 constexpr int kCtrlWarps = 4;
-#ifndef FORGE_INT8_WARPS_PER_QUAD
-#define FORGE_INT8_WARPS_PER_QUAD 2
-#endif
-// int8: warps per TMEM quadrant sharing a row (2 = the two warpgroups; 3 measured slower: 485 vs 461 us/layer)
-constexpr int kI8W = FORGE_INT8_WARPS_PER_QUAD;
-// nwg = epilogue warpgroups of the floating-point paths (2, or 4 when a chunk has four 32-column sub-blocks)
-__host__ __device__ constexpr int epi_warps(int mdt, int nwg = 2) { return mdt == 2 /*MDT_INT8*/ ? 4 * kI8W : 4 * nwg; }
+// nwg = epilogue warpgroups (2, or 4: the floating-point paths then need four 32-column sub-blocks per chunk; with
+// int8 moments nwg is the number of warps of one TMEM quadrant that share a row -- 3 measured slower: 485 vs 461 us/layer)
+__host__ __device__ constexpr int epi_warps(int /*mdt*/, int nwg = 2) { return 4 * nwg; }
 __host__ __device__ constexpr int block_threads(int mdt, int nwg = 2) { return (kCtrlWarps + epi_warps(mdt, nwg)) * 32; }
 // L2 eviction priority of the state stream (W, m, v loads and the in-place stores).  Measured on the cfg-1 layer:
 // evict_first for both 762 us, normal for both 729 us (fp32 moments; bf16 484 -> 459 us): the store that follows
@@ -118,10 +114,10 @@ struct KernelCfg {
     static constexpr int RB = BLOCK_M / CM, CB = BLOCK_N / CN, CHUNKS = RB * CB;
     static constexpr int SUBS = CN / SUB;                   // 32-column sub-blocks per chunk row
     static constexpr int WGS = SUBS >= NWG ? NWG : (SUBS >= 2 ? 2 : 1);   // warpgroups that share one chunk
-    static_assert(NWG == 2 || (NWG == 4 && SUBS >= 4 && MDT != MDT_INT8), "four epilogue warpgroups need four sub-blocks per chunk row");
+    static_assert(NWG == 2 || (NWG == 4 && (SUBS >= 4 || MDT == MDT_INT8)), "four epilogue warpgroups need four sub-blocks per chunk row");
     // chunks ci and ci + PERIOD are consumed by the same warps
     static constexpr int PERIOD = RB * (SUBS >= 2 ? 1 : 2);
-    static constexpr int DONE_COUNT = (CM / SUB) * (MDT == MDT_INT8 ? kI8W : WGS) * 32;
+    static constexpr int DONE_COUNT = (CM / SUB) * (MDT == MDT_INT8 ? NWG : WGS) * 32;
     // TMA boxes: at most 128 B per row (one swizzle span), CM rows
     static constexpr int W_BOX_COLS = CN < 64 ? CN : 64;
     static constexpr int W_ROW = W_BOX_COLS * 2;
@@ -143,7 +139,7 @@ struct KernelCfg {
     static constexpr int P1_BOX = 128 * P1_COLS;
     static constexpr int P1_STAGE = 2 * P1_BOX;
     static constexpr int kNumBars = 2 * kStages + 4 + 3 * kStateStages + 2 * P1_STAGES;
-    static constexpr int XCHG_BYTES = (MDT == MDT_INT8) ? 2 * kI8W * 1024 : 0;   // partial row maxima of the warps sharing a row, 2 buffers
+    static constexpr int XCHG_BYTES = (MDT == MDT_INT8) ? 2 * NWG * 1024 : 0;   // partial row maxima of the warps sharing a row, 2 buffers
     static constexpr int SMEM_BYTES = 1024 /*align slack*/ + kStages * ML_STAGE + kStateStages * ST_STAGE +
                                       P1_STAGES * P1_STAGE + kNumBars * 8 + 16 + XCHG_BYTES;
     static_assert(SMEM_BYTES <= 232448, "shared memory budget exceeded");
@@ -465,8 +461,8 @@ struct Int8Row {           // per-thread view of its row's 256-block in one tile
     float bm, bv;          // beta * (old absmax / levels): dequantisation folded into the moment update
     bool valid;
     __device__ __forceinline__ void finish(const AdamWScalars &hp) {
-        bm = __fmul_rn(hp.beta1, dequant_step(a_m, 127.0f));
-        bv = __fmul_rn(hp.beta2, dequant_step(a_v, 255.0f));
+        bm = __fmul_rn(hp.q_b1, dequant_step(a_m, 127.0f));      // scaled moments m'' = m'/(1-beta1), v'' = v'/(1-beta2)
+        bv = __fmul_rn(hp.q_b2, dequant_step(a_v, 255.0f));
     }
 };
 
@@ -478,7 +474,7 @@ __device__ __forceinline__ void int8_pass1(const AdamWScalars &hp, const Int8Row
     pm = 0.0f;
     pv = 0.0f;
     constexpr int kSubs = Cfg::P1_COLS / SUB;              // 32-column sub-blocks per chunk; sub-block t of the
-                                                           // row goes to warp t % kI8W of the quadrant
+                                                           // row goes to warp t % NWG of the quadrant
 #pragma unroll 1
     for (int c1 = 0; c1 < Cfg::P1_CHUNKS; ++c1) {
         const uint32_t i1 = titer * Cfg::P1_CHUNKS + c1, s = i1 % Cfg::P1_STAGES, ph = (i1 / Cfg::P1_STAGES) & 1u;
@@ -486,7 +482,7 @@ __device__ __forceinline__ void int8_pass1(const AdamWScalars &hp, const Int8Row
         if (!no_state) mbar_wait(S.bar_p1_full + 8 * s, ph);
 #pragma unroll 1
         for (int j32 = 0; j32 < (skip_math ? 0 : kSubs); ++j32) {
-            if ((c1 * kSubs + j32) % kI8W != wg) continue;
+            if ((c1 * kSubs + j32) % Cfg::NWG != wg) continue;
             uint32_t g[32];
             tmem_ld_32x32b_x32(taddr + c1 * Cfg::P1_COLS + j32 * SUB, g);
             const uint32_t o0 = swz<Cfg::P1_COLS>(row_t, 2 * j32), o1 = swz<Cfg::P1_COLS>(row_t, 2 * j32 + 1);
@@ -504,7 +500,7 @@ __device__ __forceinline__ void int8_pass1(const AdamWScalars &hp, const Int8Row
                     for (int e = 0; e < 2; ++e) {
                         const int gi = 16 * j + 4 * q + 2 * e;
                         f32x2 m, v;
-                        adamw_moments2_q(hp, pk2u(g[gi], g[gi + 1]), cm[e], cv[e], R.bm, R.bv, m, v);
+                        adamw_moments2_qs(pk2u(g[gi], g[gi + 1]), cm[e], cv[e], R.bm, R.bv, m, v);
                         pm = fmaxf(pm, fmaxf(fabsf(lo2(m)), fabsf(hi2(m))));
                         pv = fmaxf(pv, fmaxf(lo2(v), hi2(v)));           // v' >= 0
                     }
@@ -533,7 +529,7 @@ __device__ __forceinline__ void int8_pass2(const AdamWScalars &hp, const Int8Row
         else mbar_wait(bar_st_empty + 8 * s, ph ^ 1u);
 #pragma unroll 1
         for (int half = 0; half < Cfg::SUBS; ++half) {
-        if (skip_math || (cb * Cfg::SUBS + half) % kI8W != wg) continue;
+        if (skip_math || (cb * Cfg::SUBS + half) % Cfg::NWG != wg) continue;
         uint32_t g[32];
         tmem_ld_32x32b_x32(taddr + cb * Cfg::CN + half * SUB, g);
         const SubAddr<Cfg> a(sST + s * Cfg::ST_STAGE, half * SUB);
@@ -557,8 +553,8 @@ __device__ __forceinline__ void int8_pass2(const AdamWScalars &hp, const Int8Row
                 for (int e = 0; e < 2; ++e) {
                     const int gi = 16 * j + 4 * q + 2 * e;
                     f32x2 m, v, w = bf16x2_to_f32x2(ww[2 * q + e]);
-                    adamw_moments2_q(hp, pk2u(g[gi], g[gi + 1]), cm[e], cv[e], bm, bv, m, v);
-                    adamw_weight2(hp, m, v, w);
+                    adamw_moments2_qs(pk2u(g[gi], g[gi + 1]), cm[e], cv[e], bm, bv, m, v);
+                    adamw_weight2_s(hp, m, v, w);
                     wo[2 * q + e] = f32x2_to_bf16x2(w);
                     qm[e] = quant_m2(m, inv_m);
                     qv[e] = quant_v2(v, inv_v, v_floor);
@@ -978,14 +974,14 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                 int8_pass1<Cfg>(hp, R, titer, taddr, i8, row_t, wg, pm, pv, FORGE_DBG(P, DBG_NO_EPILOGUE),
                                 FORGE_DBG(P, DBG_NO_STATE));
                 // combine the two warpgroups' halves of the row (same TMEM quadrant: warps quad and 4 + quad)
-                const uint32_t xb = i8.xchg + (titer & 1u) * (kI8W * 1024u);
+                const uint32_t xb = i8.xchg + (titer & 1u) * (NWG * 1024u);
                 asm volatile("st.shared.v2.f32 [%0], {%1, %2};\n" ::"r"(xb + (wg * 128u + row_t) * 8u), "f"(pm), "f"(pv) : "memory");
-                asm volatile("bar.sync %0, %1;\n" ::"r"(1u + quad), "n"(kI8W * 32) : "memory");
+                asm volatile("bar.sync %0, %1;\n" ::"r"(1u + quad), "n"(NWG * 32) : "memory");
                 float a_m = pm, a_v = pv;
 #pragma unroll
-                for (int o = 1; o < kI8W; ++o) {
+                for (int o = 1; o < NWG; ++o) {
                     float om, ov;
-                    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];\n" : "=f"(om), "=f"(ov) : "r"(xb + (((wg + o) % kI8W) * 128u + row_t) * 8u));
+                    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];\n" : "=f"(om), "=f"(ov) : "r"(xb + (((wg + o) % NWG) * 128u + row_t) * 8u));
                     a_m = fmaxf(a_m, om);
                     a_v = fmaxf(a_v, ov);
                 }
@@ -993,8 +989,8 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                                               row_t, wg, FORGE_DBG(P, DBG_NO_EPILOGUE), FORGE_DBG(P, DBG_NO_STATE));
                 if (wg == 0 && R.valid) {
                     const ProblemDesc &pd = P.prob[decode_tile<CG>(P, tile, rank).p];
-                    pd.m_scale[R.sidx] = a_m;
-                    pd.v_scale[R.sidx] = a_v;
+                    pd.m_scale[R.sidx] = __fmul_rn(hp.one_minus_beta1, a_m);     // absmax of m', v' from the scaled maxima
+                    pd.v_scale[R.sidx] = __fmul_rn(hp.one_minus_beta2, a_v);
                 }
             }
             // this warp has drained the accumulator: tell the (leader's) MMA issuer

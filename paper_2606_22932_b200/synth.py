@@ -87,6 +87,33 @@ def make_layer(T: int, seed: int, shapes=LLAMA8B_LAYER, device="cpu", **kw) -> l
     return probs
 
 
+def random_int8_state(out: int, inn: int, seed: int, device="cpu", block: int = 256):
+    """Synthetic int8 blockwise optimizer state drawn DIRECTLY as codes and scales (no quantiser arithmetic: the timed
+    path is data-independent, and the parity tests seed theirs with the oracle's quantiser instead): m codes
+    ~ round(N(0, 40)) clipped to [-127, 127], v codes uniform in [1, 255], block scales of the cfg-1 magnitudes
+    (absmax of 256 draws of N(0, 1e-4) resp. |N(0, 1e-6)| is about 3 sigma).  Returns (m, v, m_scale, v_scale)."""
+    g = _gen(seed, device)
+    m = (torch.randn((out, inn), generator=g, dtype=torch.float32, device=device) * 40.0).round_().clamp_(-127, 127).to(torch.int8)
+    v = torch.randint(1, 256, (out, inn), generator=g, dtype=torch.int32, device=device).to(torch.uint8)
+    nb = inn // block
+    ms = (3e-4 + 1e-4 * torch.rand((out, nb), generator=g, dtype=torch.float32, device=device)).contiguous()
+    vs = (3e-6 + 1e-6 * torch.rand((out, nb), generator=g, dtype=torch.float32, device=device)).contiguous()
+    return m, v, ms, vs
+
+
+def random_fp8_state(out: int, inn: int, seed: int, device="cpu"):
+    """Synthetic e4m3 optimizer state drawn directly as codes (never the NaN code 0x7F / 0xFF) with one {scale, amax
+    out} pair per tensor.  Returns (m, v, m_scale, v_scale)."""
+    g = _gen(seed, device)
+    mag = torch.randint(0, 0x7F, (out, inn), generator=g, dtype=torch.int32, device=device)
+    sign = torch.randint(0, 2, (out, inn), generator=g, dtype=torch.int32, device=device) * 0x80
+    m = (mag | sign).to(torch.uint8)
+    v = torch.randint(1, 0x7F, (out, inn), generator=g, dtype=torch.int32, device=device).to(torch.uint8)
+    ms = torch.tensor([3e-4 / 448.0, 0.0], dtype=torch.float32, device=device)
+    vs = torch.tensor([3e-6 / 448.0, 0.0], dtype=torch.float32, device=device)
+    return m, v, ms, vs
+
+
 def config0_step_inputs(step: int, device="cpu"):
     """BASELINE.json cfg 0: fresh X[128,256] ~N(0,1), dY[128,384] ~N(0,1e-2) per step."""
     s = BASE_SEED + 7919 * step

@@ -1,0 +1,138 @@
+"""GPU parity at FULL size, every row: the configs[1] / configs[2] grouped launch (the configuration bench.py times)
+against the oracle element by element on every row of every projection, >= 1/16 of the rows of gate_proj at
+T = 2048 / 8192 (ring and direct dispatch paths) spread over all waves, and the edge cases include/forge.h promises
+(NaN / Inf propagation, an all-zero int8 block inside a full tile, the decay-only step dY = 0 of PAPER.md:292)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import forge_oracle as fo
+from paper_2606_22932_b200 import binding as fb
+from paper_2606_22932_b200 import synth
+import parity_util as pu
+from test_gpu_parity import DEV, HP, compare, gpu_state, hp_args, oracle_step
+
+pytestmark = pytest.mark.gpu
+ROW_CHUNK = 512
+
+
+@pytest.mark.parametrize("moment", ["fp32", "bf16", "int8"])
+def test_config1_2_whole_layer_every_row_against_the_oracle(moment):
+    """All 218 103 808 weight elements of the Llama-3.1-8B layer, one grouped launch, compared with the oracle row
+    chunk by row chunk (rows are independent; chunks only bound the host memory of the fp64 gradient)."""
+    layer = synth.make_layer(512, seed=synth.BASE_SEED + 1)
+    pairs = [gpu_state(p, moment) for p in layer]
+    ds = [d for d, _ in pairs]
+    before = fb.forge_launch_count()
+    fb.forge_wgrad_adamw_grouped(ds, 10, *pu.hp_tuple(HP), {"fp32": 0, "bf16": 1, "int8": 2}[moment])
+    torch.cuda.synchronize()
+    assert fb.forge_launch_count() - before == 1
+    stats = dict(n=0, w_equal=0, m_code_equal=0, v_code_equal=0)
+    for p, (d, o) in zip(layer, pairs):
+        host = {k: pu.to_np(d[k]) for k in d if k not in ("X", "dY")}        # one D2H per tensor
+        for r0 in range(0, p.out, ROW_CHUNK):
+            rows = (r0, min(p.out, r0 + ROW_CHUNK))
+            ref, G, E = oracle_step(o, moment, 10, rows)
+            view = {k: host[k][rows[0]:rows[1]] for k in host}
+            compare_host(view, ref, G, E, 512, moment, f"{moment} {p.name} rows {rows}", o["W"][rows[0]:rows[1]])
+            stats["n"] += G.size
+            stats["w_equal"] += int((view["W"] == ref["W"]).sum())
+            if moment == "int8":
+                stats["m_code_equal"] += int((view["m"] == ref["m"]).sum())
+                stats["v_code_equal"] += int((view["v"] == ref["v"]).sum())
+    pu.record("whole_layer", moment=moment, elements=stats["n"], w_bit_identical=stats["w_equal"] / stats["n"],
+              m_code_identical=stats["m_code_equal"] / stats["n"] if moment == "int8" else None,
+              v_code_identical=stats["v_code_equal"] / stats["n"] if moment == "int8" else None)
+    assert stats["n"] == 218103808
+
+
+def compare_host(view, ref, G, E, T, moment, label, W_prev):
+    """test_gpu_parity.compare on host arrays already copied back."""
+    tol = pu.Tol(G.shape)
+    e = tol.step(G, E, T, HP)
+    wprop = ref.get("_wprop", 0.0)
+    if moment == "int8":
+        pu.check_int8(view["W"], view["m"], view["v"], view["m_scale"], view["v_scale"], ref["W"], ref["m"], ref["v"],
+                      ref["m_scale"], ref["v_scale"], G, e, HP, label, W_prev=W_prev, w_prop=wprop)
+    else:
+        pu.check_fp(view["W"], view["m"], view["v"], ref["W"], ref["m"], ref["v"], G, e, tol, HP, moment, label, W_prev=W_prev,
+                    w_prop=wprop)
+
+
+@pytest.mark.parametrize("T", [2048, 8192])
+def test_config3_gate_one_sixteenth_of_the_rows_spread_over_all_waves(T):
+    """configs[3] at T = 2048 (large-T ring path) and T = 8192 (direct state path): 7 x 128 rows = 1/16 of gate_proj,
+    from the first tile to the last partial wave."""
+    p = synth.make_problem("gate", T, 14336, 4096, seed=synth.BASE_SEED + 3)
+    d, o = gpu_state(p, "fp32")
+    fb.forge_wgrad_adamw(d["X"], d["dY"], d["W"], d["m"], d["v"], 10, **HP)
+    torch.cuda.synchronize()
+    ranges = pu.spread_rows(14336, 16, 128)
+    assert sum(b - a for a, b in ranges) * 16 >= 14336 and ranges[0][0] == 0 and ranges[-1][1] == 14336
+    for rows in ranges:
+        ref, G, E = oracle_step(o, "fp32", 10, rows)
+        compare(d, ref, G, E, T, "fp32", rows, label=f"gate T={T} rows {rows}", W_prev=o["W"])
+
+
+# ------------------------------------------------------------------------------ edge cases ---
+def test_nan_and_inf_propagate_to_exactly_the_affected_row_and_column():
+    """include/forge.h: "NaN/Inf in the inputs propagate by IEEE rules (to the rows / columns of G they enter and
+    nowhere else)".  A NaN in dY[t, p] poisons row p of G, an Inf in X[t, q] column q (and NaN where it meets a
+    zero-sign cancellation); everything else must be bit-identical to the clean run."""
+    p = synth.make_problem("n", 300, 384, 768, seed=901)
+    clean, _ = gpu_state(p, "fp32")
+    fb.forge_wgrad_adamw(clean["X"], clean["dY"], clean["W"], clean["m"], clean["v"], 7, **HP)
+    d, _ = gpu_state(p, "fp32")
+    pr, qc = 200, 515                                    # second 128-row block; third 256-column tile... col 515 of 768
+    d["dY"][17, pr] = float("nan")
+    d["X"][250, qc] = float("inf")
+    fb.forge_wgrad_adamw(d["X"], d["dY"], d["W"], d["m"], d["v"], 7, **HP)
+    torch.cuda.synchronize()
+    touched = torch.zeros(384, 768, dtype=torch.bool, device=DEV)
+    touched[pr, :] = True
+    touched[:, qc] = True
+    for k in ("W", "m", "v"):
+        a, b = d[k].float(), clean[k].float()
+        assert torch.equal(d[k][~touched], clean[k][~touched]), f"{k}: poison leaked outside row {pr} / column {qc}"
+        assert torch.isnan(a[pr, :]).all(), f"{k}: row {pr} must be NaN"
+        col = a[:, qc]
+        assert (~torch.isfinite(col)).all(), f"{k}: column {qc} must be Inf or NaN"
+        assert torch.isfinite(b).all()
+
+
+def test_dy_zero_is_the_decay_only_step():
+    """PAPER.md:292 Remark 1: G = 0 gives m' = b1 m, v' = b2 v and W' from those (the decay-only step); against the
+    oracle on every element, and W moves by decay + the stale-moment update only."""
+    p = synth.make_problem("z", 256, 384, 512, seed=902)
+    p.dY.zero_()
+    for moment in ("fp32", "int8"):
+        d, o = gpu_state(p, moment)
+        fb.forge_wgrad_adamw(d["X"], d["dY"], d["W"], d["m"], d["v"], 10, m_scale=d.get("m_scale"), v_scale=d.get("v_scale"), **HP)
+        torch.cuda.synchronize()
+        ref, G, E = oracle_step(o, moment, 10)
+        assert not G.any() and not E.any()
+        compare(d, ref, G, E, 256, moment, label=f"dY=0 {moment}", W_prev=o["W"])
+        if moment == "fp32":
+            b1 = np.float64(np.float32(HP["beta1"]))
+            assert np.allclose(pu.to_np(d["m"]), b1 * p.m.numpy().astype(np.float64), rtol=1e-6, atol=0)
+
+
+def test_all_zero_int8_block_inside_a_full_tile():
+    """App. B / reading S6: a block whose new moments are all zero stores a = 0 and codes 0 (no division by the
+    scale); here rows 130..133 x columns 256..511 of a multi-tile problem have zero state AND zero gradient (their dY
+    columns are zero), in the middle of blocks that are busy."""
+    p = synth.make_problem("q", 200, 384, 768, seed=903)
+    p.dY[:, 130:134] = 0
+    p.m[130:134, 256:512] = 0
+    p.v[130:134, 256:512] = 0
+    d, o = gpu_state(p, "int8")
+    assert not o["m_scale"][130:134, 1].any() and not o["v_scale"][130:134, 1].any()
+    fb.forge_wgrad_adamw(d["X"], d["dY"], d["W"], d["m"], d["v"], 10, m_scale=d["m_scale"], v_scale=d["v_scale"], **HP)
+    torch.cuda.synchronize()
+    ref, G, E = oracle_step(o, "int8", 10)
+    compare(d, ref, G, E, 200, "int8", label="zero block", W_prev=o["W"])
+    assert not d["m"][130:134, 256:512].any() and not d["v"][130:134, 256:512].any()
+    assert not d["m_scale"][130:134, 1].any() and not d["v_scale"][130:134, 1].any()
+    assert torch.isfinite(d["W"].float()).all()
+    # the same rows' OTHER blocks carry state (zero gradient there too: pure decay of the codes)
+    assert d["m_scale"][130:134, 0].all() and d["v_scale"][130:134, 2].all()
