@@ -303,6 +303,11 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
         tiles += ((p.out + BLOCK_M * CG - 1) / (BLOCK_M * CG)) * d.tiles_n;   // (128*CG) x 256 work units
     }
     P.total_tiles = tiles;
+    // L2 eviction priority of the operand streams: evict_last for both.  Measured on gate_proj (profiles/r02_summary.md):
+    // dY evict_first is slower at every T (T = 8192: 764 vs 750 us, DRAM reads 2.48 vs 1.80 GB -- the sixteen pairs of a
+    // tile row do not read a dY line at the same instant), dY evict_normal is within noise (749 us, 1.90 GB).
+    P.pol_dy = env_int("FORGE_POLICY", 0) == 1 ? kEvictFirst : (env_int("FORGE_POLICY", 0) == 2 ? kEvictNormal : kEvictLast);
+    P.pol_x = kEvictLast;
     P.sr_seed_lo = static_cast<uint32_t>(sr_seed);
     P.debug = env_int("FORGE_ABLATE", 0);          // FORGE_PROFILING build only (constant 0 otherwise)
     int grid = dev.sm_count / CG;                  // persistent: one CTA (or CTA pair) per SM (pair)
@@ -387,10 +392,12 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
         if (variant == V_LARGE_T) return launch_fused<MDT_BF16, MODE_ADAMW, 64, 4, 2, 2, 64, 64>(probs, count, hp, dev, stream);
         return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
     case FORGE_MOMENT_INT8:
-        // measured (us / layer): 3 state slots + 80 KB operand ring + 64-column first-pass chunks 420; 3 slots + 48 KB ring 437;
-        // 2 slots 457-489 whatever the operand ring; 4 slots + 48 KB ring 442 (profiles/r01_summary.md)
+        // resident-tile epilogue (P1S = 0: the four 128 x 64 chunks of a tile stay in the state ring through both passes, no
+        // second read of the codes): 4 slots + 80 KB operand ring 428 us / layer against 440 for the streamed two-ring
+        // variant <32, 5, 3, .., 64, 2> on the same box; 5 slots + 48 KB operand ring 451 (mainloop starved); sixteen
+        // epilogue warps 487 (profiles/r02_summary.md)
         if (variant == V_LARGE_T) return launch_fused<MDT_INT8, MODE_ADAMW, 64, 2, 2, 2, 128, 64>(probs, count, hp, dev, stream);
-        return launch_fused<MDT_INT8, MODE_ADAMW, 32, 5, 3, 2, 128, 64, 64, 2>(probs, count, hp, dev, stream);
+        return launch_fused<MDT_INT8, MODE_ADAMW, 32, 5, 4, 2, 128, 64, 64, 0>(probs, count, hp, dev, stream);
     case FORGE_MOMENT_FP8:
         // 8 B/element of state: the T = 512 mainloop needs the deeper operand ring (96 KB) more than the state ring does
         return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 4, 2, 64, 128>(probs, count, hp, dev, stream);

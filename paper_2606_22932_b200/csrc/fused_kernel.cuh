@@ -24,6 +24,7 @@
 // with LBO = kBlockK*128 B between 64-wide MN blocks and SBO = 1024 B between 8-token groups.
 #pragma once
 #include <cstdint>
+#include <cstdio>
 #include <cuda.h>
 #include <cuda_runtime.h>
 
@@ -74,6 +75,7 @@ struct alignas(64) KernelParams {
     ProblemDesc prob[kMaxProblems];
     AdamWScalars hp;
     FamilyScalars fs;    // MODE_FAMILY only
+    uint64_t pol_dy, pol_x;   // L2 eviction priority of the dY / X operand loads (host: by token count, see launch_fused)
     int32_t num_problems;
     int32_t total_tiles;
     uint32_t sr_seed_lo; // MODE_ADAMW_SR
@@ -82,11 +84,15 @@ struct alignas(64) KernelParams {
                          // 4 = no epilogue math, 8 = no state stores (direct path only).  The product build never reads it.
 };
 enum : int { DBG_NO_MAINLOOP = 1, DBG_NO_STATE = 2, DBG_NO_EPILOGUE = 4, DBG_NO_STORE = 8 /* direct path only */,
-              DBG_NO_A = 16 /* CTA pairs: dY chunks loaded for the first ring pass only (operand traffic halved) */ };
+              DBG_NO_A = 16 /* CTA pairs: dY chunks loaded for the first ring pass only (operand traffic halved) */,
+              DBG_TIMING = 64 /* print per-role wait / work clocks (results unchanged) */ };
 #ifdef FORGE_PROFILING
 #define FORGE_DBG(P, bit) (((P).debug & (bit)) != 0)
+// FORGE_ABLATE bit 64: per-role clock accounting, printed by CTA 0 / 1 at exit (profiles/ only)
+#define FORGE_TIMED_WAIT(acc, stmt) do { const long long t_ = clock64(); stmt; (acc) += clock64() - t_; } while (0)
 #else
 #define FORGE_DBG(P, bit) false
+#define FORGE_TIMED_WAIT(acc, stmt) do { stmt; } while (0)
 #endif
 
 // CG = 1: one CTA per 128x256 tile.  CG = 2: a CTA pair (cluster of 2, tcgen05 cta_group::2) shares
@@ -117,7 +123,7 @@ struct KernelCfg {
     static_assert(NWG == 2 || (NWG == 4 && (SUBS >= 4 || MDT == MDT_INT8)), "four epilogue warpgroups need four sub-blocks per chunk row");
     // chunks ci and ci + PERIOD are consumed by the same warps
     static constexpr int PERIOD = RB * (SUBS >= 2 ? 1 : 2);
-    static constexpr int DONE_COUNT = (CM / SUB) * (MDT == MDT_INT8 ? NWG : WGS) * 32;
+    static constexpr int DONE_COUNT = (CM / SUB) * (MDT == MDT_INT8 ? NWG : WGS);   // one arrival per warp that works on a chunk
     // TMA boxes: at most 128 B per row (one swizzle span), CM rows
     static constexpr int W_BOX_COLS = CN < 64 ? CN : 64;
     static constexpr int W_ROW = W_BOX_COLS * 2;
@@ -470,7 +476,7 @@ struct Int8Row {           // per-thread view of its row's 256-block in one tile
 template <class Cfg>
 __device__ __forceinline__ void int8_pass1(const AdamWScalars &hp, const Int8Row &R, uint32_t titer, uint32_t taddr,
                                            const Int8Smem &S, uint32_t row_t, int wg, float &pm, float &pv,
-                                           bool skip_math, bool no_state) {
+                                           bool skip_math, bool no_state, long long &t_wait) {
     pm = 0.0f;
     pv = 0.0f;
     constexpr int kSubs = Cfg::P1_COLS / SUB;              // 32-column sub-blocks per chunk; sub-block t of the
@@ -479,7 +485,7 @@ __device__ __forceinline__ void int8_pass1(const AdamWScalars &hp, const Int8Row
     for (int c1 = 0; c1 < Cfg::P1_CHUNKS; ++c1) {
         const uint32_t i1 = titer * Cfg::P1_CHUNKS + c1, s = i1 % Cfg::P1_STAGES, ph = (i1 / Cfg::P1_STAGES) & 1u;
         const uint32_t am = S.p1 + s * Cfg::P1_STAGE, av = am + Cfg::P1_BOX;
-        if (!no_state) mbar_wait(S.bar_p1_full + 8 * s, ph);
+        if (!no_state) FORGE_TIMED_WAIT(t_wait, mbar_wait(S.bar_p1_full + 8 * s, ph));
 #pragma unroll 1
         for (int j32 = 0; j32 < (skip_math ? 0 : kSubs); ++j32) {
             if ((c1 * kSubs + j32) % Cfg::NWG != wg) continue;
@@ -507,7 +513,54 @@ __device__ __forceinline__ void int8_pass1(const AdamWScalars &hp, const Int8Row
                 }
             }
         }
-        mbar_arrive(S.bar_p1_empty + 8 * s);              // the codes have been read: slot reusable
+        __syncwarp();
+        if ((row_t & 31u) == 0) mbar_arrive(S.bar_p1_empty + 8 * s);   // this warp has read the codes: one arrival per warp
+    }
+}
+
+// pass 1, resident-tile variant (P1_STAGES == 0): there is no separate code ring -- the state ring holds every chunk of
+// the tile (W + codes, loaded ONCE) from its first use here until pass 2 has rewritten it in place, plus one or two
+// spare slots in which the next tile's first chunks arrive meanwhile.  The codes cross L2 -> SM once instead of twice.
+template <class Cfg, int kStateStages>
+__device__ __forceinline__ void int8_pass1_ring(const Int8Row &R, uint32_t titer, uint32_t taddr, uint32_t sST,
+                                                uint32_t bar_st_full, uint32_t row_t, int wg, float &pm, float &pv,
+                                                bool skip_math, long long &t_wait) {
+    pm = 0.0f;
+    pv = 0.0f;
+    const uint32_t rb = row_t / Cfg::CM, row = row_t % Cfg::CM;
+#pragma unroll 1
+    for (int cb = 0; cb < Cfg::CB; ++cb) {
+        const uint32_t ci = titer * Cfg::CHUNKS + cb * Cfg::RB + rb;
+        const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
+        FORGE_TIMED_WAIT(t_wait, mbar_wait(bar_st_full + 8 * s, ph));
+#pragma unroll 1
+        for (int half = 0; half < Cfg::SUBS; ++half) {
+            if (skip_math || (cb * Cfg::SUBS + half) % Cfg::NWG != wg) continue;
+            uint32_t g[32];
+            tmem_ld_32x32b_x32(taddr + cb * Cfg::CN + half * SUB, g);
+            const SubAddr<Cfg> a(sST + s * Cfg::ST_STAGE, half * SUB);
+            const uint32_t o0 = swz<Cfg::M_ROW>(row, a.pm), o1 = swz<Cfg::M_ROW>(row, a.pm + 1);
+            const uint4 mq[2] = {lds128(a.m + o0), lds128(a.m + o1)}, vq[2] = {lds128(a.v + o0), lds128(a.v + o1)};
+            tmem_ld_wait();
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const uint32_t mw[4] = {mq[j].x, mq[j].y, mq[j].z, mq[j].w}, vw[4] = {vq[j].x, vq[j].y, vq[j].z, vq[j].w};
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    f32x2 cm[2], cv[2];
+                    codes4_to_f32(mw[q], true, cm[0], cm[1]);
+                    codes4_to_f32(vw[q], false, cv[0], cv[1]);
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int gi = 16 * j + 4 * q + 2 * e;
+                        f32x2 m, v;
+                        adamw_moments2_qs(pk2u(g[gi], g[gi + 1]), cm[e], cv[e], R.bm, R.bv, m, v);
+                        pm = fmaxf(pm, fmaxf(fabsf(lo2(m)), fabsf(hi2(m))));
+                        pv = fmaxf(pv, fmaxf(lo2(v), hi2(v)));           // v' >= 0
+                    }
+                }
+            }
+        }
     }
 }
 
@@ -516,7 +569,7 @@ template <class Cfg, int kStateStages>
 __device__ __forceinline__ void int8_pass2(const AdamWScalars &hp, const Int8Row &R, float a_m, float a_v,
                                            uint32_t titer, uint32_t taddr, uint32_t sST, uint32_t bar_st_full,
                                            uint32_t bar_st_done, uint32_t bar_st_empty, uint32_t row_t, int wg,
-                                           bool skip_math, bool no_state) {
+                                           bool skip_math, bool no_state, long long &t_wait) {
     const uint32_t rb = row_t / Cfg::CM, row = row_t % Cfg::CM;
     const float bm = R.bm, bv = R.bv;
     const float inv_m = quant_inv_scale(a_m, 127.0f), inv_v = quant_inv_scale(a_v, 255.0f);
@@ -525,7 +578,7 @@ __device__ __forceinline__ void int8_pass2(const AdamWScalars &hp, const Int8Row
     for (int cb = 0; cb < Cfg::CB; ++cb) {
         const uint32_t ci = titer * Cfg::CHUNKS + cb * Cfg::RB + rb;
         const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
-        if (!no_state) mbar_wait(bar_st_full + 8 * s, ph);
+        if (!no_state) FORGE_TIMED_WAIT(t_wait, mbar_wait(bar_st_full + 8 * s, ph));
         else mbar_wait(bar_st_empty + 8 * s, ph ^ 1u);
 #pragma unroll 1
         for (int half = 0; half < Cfg::SUBS; ++half) {
@@ -568,8 +621,10 @@ __device__ __forceinline__ void int8_pass2(const AdamWScalars &hp, const Int8Row
             sts128(aw1, make_uint4(wo[4], wo[5], wo[6], wo[7]));
         }
         }
+        // every thread orders its own writes before the async proxy, the warp synchronises, one lane signals the storer
         fence_proxy_async_smem();
-        mbar_arrive(bar_st_done + 8 * s);
+        __syncwarp();
+        if ((row_t & 31u) == 0) mbar_arrive(bar_st_done + 8 * s);
     }
 }
 
@@ -686,7 +741,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         }
         for (int i = 0; i < Cfg::P1_STAGES; ++i) {
             mbar_init(bar_p1_full + 8 * i, 1);
-            mbar_init(bar_p1_empty + 8 * i, epi_warps(MDT, NWG) * 32);     // every epilogue thread reads its part of the chunk
+            mbar_init(bar_p1_empty + 8 * i, epi_warps(MDT, NWG));          // every epilogue warp reads its part of the chunk
         }
         mbar_fence_init();
     }
@@ -721,11 +776,11 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
 #pragma unroll
                         for (int i = 0; i < BLOCK_M / 64; ++i)
                             tma_load_2d(a + i * kBlockK * 128, &pd.map_dY, full, tc.tm * BLOCK_M + i * 64,
-                                        kb * kBlockK, kEvictLast);
+                                        kb * kBlockK, P.pol_dy);
 #pragma unroll
                         for (int i = 0; i < BLOCK_N / 64; ++i)
                             tma_load_2d(b + i * kBlockK * 128, &pd.map_X, full, tc.tn * BLOCK_N + i * 64,
-                                        kb * kBlockK, kEvictLast);
+                                        kb * kBlockK, P.pol_x);
                     } else {
                         // both CTAs' bytes are counted on the LEADER's full barrier
                         const bool no_a = FORGE_DBG(P, DBG_NO_A) && it >= kStages;
@@ -734,12 +789,12 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
 #pragma unroll
                         for (int i = 0; i < (no_a ? 0 : BLOCK_M / 64); ++i)
                             tma_load_2d_cg2(a + i * kBlockK * 128, &pd.map_dY, full, tc.tm * BLOCK_M + i * 64,
-                                            kb * kBlockK, kEvictLast);
+                                            kb * kBlockK, P.pol_dy);
 #pragma unroll
                         for (int i = 0; i < BLOCK_N / 128; ++i)   // this CTA's half of the 256 columns
                             tma_load_2d_cg2(b + i * kBlockK * 128, &pd.map_X, full,
                                             tc.tn * BLOCK_N + static_cast<int>(rank) * (BLOCK_N / 2) + i * 64,
-                                            kb * kBlockK, kEvictLast);
+                                            kb * kBlockK, P.pol_x);
                     }
                 }
             }
@@ -749,16 +804,20 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         if (lane == 0 && rank == 0 && !FORGE_DBG(P, DBG_NO_MAINLOOP)) {
             constexpr uint32_t idesc = make_idesc_bf16_f32_mnmn(BLOCK_M * CG, BLOCK_N);
             uint32_t it = 0, titer = 0;
+            [[maybe_unused]] long long t_acc = 0, t_ops = 0;
+#ifdef FORGE_PROFILING
+            const long long t_begin = clock64();
+#endif
             for (int tile = first_tile; tile < P.total_tiles; tile += tile_step, ++titer) {
                 const TileCoord tc = decode_tile<CG>(P, tile, rank);
                 const int num_kb = (P.prob[tc.p].T + kBlockK - 1) / kBlockK;
                 const uint32_t as = titer & 1u, aph = (titer >> 1) & 1u;
-                mbar_wait(bar_tm_empty + 8 * as, aph ^ 1u);   // epilogue has drained this buffer
+                FORGE_TIMED_WAIT(t_acc, mbar_wait(bar_tm_empty + 8 * as, aph ^ 1u));   // epilogue has drained this buffer
                 tc_fence_after();
                 const uint32_t tmem_d = tmem_base + as * BLOCK_N;
                 for (int kb = 0; kb < num_kb; ++kb, ++it) {
                     const uint32_t s = it % kStages, ph = (it / kStages) & 1u;
-                    mbar_wait(bar_ml_full + 8 * s, ph);
+                    FORGE_TIMED_WAIT(t_ops, mbar_wait(bar_ml_full + 8 * s, ph));
                     tc_fence_after();
                     const uint32_t a = sML + s * Cfg::ML_STAGE, b = a + Cfg::A_STAGE;
 #pragma unroll
@@ -777,10 +836,15 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                 if constexpr (CG == 2) umma_commit_cg2(bar_tm_full + 8 * as, 3);
                 else umma_commit(bar_tm_full + 8 * as);
             }
+#ifdef FORGE_PROFILING
+            if (FORGE_DBG(P, DBG_TIMING) && blockIdx.x < 2)
+                printf("cta %d MMA issuer tiles %u total %lld | wait accumulator free %lld | wait operands %lld\n", blockIdx.x, titer,
+                       clock64() - t_begin, t_acc, t_ops);
+#endif
         }
     } else if (warp == 2) {
         // ================= state loader (Alg. 1 line 6: load W_ij, m_ij, v_ij) ===================
-        if constexpr (MDT == MDT_INT8) {
+        if constexpr (MDT == MDT_INT8 && Cfg::P1_STAGES > 0) {
             if (lane == 0 && !FORGE_DBG(P, DBG_NO_STATE))
                 int8_loader<Cfg, kStateStages, CG>(P, rank, first_tile, tile_step, sST, bar_st_full, bar_st_empty, i8);
         } else if (!DIRECT && MODE != MODE_STORE_G && lane == 0 && !FORGE_DBG(P, DBG_NO_STATE)) {
@@ -876,9 +940,13 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
         const AdamWScalars hp = P.hp;
         Int8Row i8row{};
         uint32_t titer = 0;
+        [[maybe_unused]] long long t_tm = 0, t_w1 = 0, t_w2 = 0, t_p1 = 0, t_x = 0, t_p2 = 0;   // DBG_TIMING: wait / work clocks of this warp
+#ifdef FORGE_PROFILING
+        const long long t_begin = clock64();
+#endif
         for (int tile = first_tile; tile < P.total_tiles; tile += tile_step, ++titer) {
             const uint32_t as = titer & 1u, aph = (titer >> 1) & 1u;
-            if (!FORGE_DBG(P, DBG_NO_MAINLOOP)) mbar_wait(bar_tm_full + 8 * as, aph);
+            if (!FORGE_DBG(P, DBG_NO_MAINLOOP)) FORGE_TIMED_WAIT(t_tm, mbar_wait(bar_tm_full + 8 * as, aph));
             tc_fence_after();
             const uint32_t taddr = tmem_base + ((quad * 32u) << 16) + as * BLOCK_N;
             uint32_t sr_rowkey = 0, sr_col0 = 0;
@@ -928,7 +996,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                     const uint32_t ci = titer * CHUNKS + cb * Cfg::RB + rb;
                     const uint32_t s = ci % SSN, ph = (ci / SSN) & 1u;
                     const uint32_t base = sST + s * Cfg::ST_STAGE;
-                    if (MODE != MODE_STORE_G && !FORGE_DBG(P, DBG_NO_STATE)) mbar_wait(bar_st_full + 8 * s, ph);
+                    if (MODE != MODE_STORE_G && !FORGE_DBG(P, DBG_NO_STATE)) FORGE_TIMED_WAIT(t_w2, mbar_wait(bar_st_full + 8 * s, ph));
                     else mbar_wait(bar_st_empty + 8 * s, ph ^ 1u);
                     for (int j32 = (Cfg::SUBS >= 2 ? wg : 0); j32 < Cfg::SUBS; j32 += Cfg::WGS) {
                         uint32_t g[32];
@@ -949,8 +1017,9 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                             epi_sub_store_g<Cfg>(g, a, row);
                         }
                     }
-                    fence_proxy_async_smem();
-                    mbar_arrive(bar_st_done + 8 * s);
+                    fence_proxy_async_smem();             // each thread's writes -> async proxy; then one arrival per warp
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar_st_done + 8 * s);
                 }
                 if constexpr (MDT == MDT_FP8) {          // this step's amax of m', v' for the NEXT step's scale
 #pragma unroll
@@ -971,8 +1040,15 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                 if (tile + tile_step < P.total_tiles) i8row = int8_row<CG>(P, hp, tile + tile_step, rank, row_t);
                 R.finish(hp);
                 float pm, pv;
-                int8_pass1<Cfg>(hp, R, titer, taddr, i8, row_t, wg, pm, pv, FORGE_DBG(P, DBG_NO_EPILOGUE),
-                                FORGE_DBG(P, DBG_NO_STATE));
+                if constexpr (Cfg::P1_STAGES > 0)
+                    FORGE_TIMED_WAIT(t_p1, int8_pass1<Cfg>(hp, R, titer, taddr, i8, row_t, wg, pm, pv, FORGE_DBG(P, DBG_NO_EPILOGUE),
+                                                           FORGE_DBG(P, DBG_NO_STATE), t_w1));
+                else
+                    FORGE_TIMED_WAIT(t_p1, (int8_pass1_ring<Cfg, kStateStages>(R, titer, taddr, sST, bar_st_full, row_t, wg, pm, pv,
+                                                                               FORGE_DBG(P, DBG_NO_EPILOGUE), t_w1)));
+#ifdef FORGE_PROFILING
+                const long long t_x0 = clock64();
+#endif
                 // combine the two warpgroups' halves of the row (same TMEM quadrant: warps quad and 4 + quad)
                 const uint32_t xb = i8.xchg + (titer & 1u) * (NWG * 1024u);
                 asm volatile("st.shared.v2.f32 [%0], {%1, %2};\n" ::"r"(xb + (wg * 128u + row_t) * 8u), "f"(pm), "f"(pv) : "memory");
@@ -985,8 +1061,12 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                     a_m = fmaxf(a_m, om);
                     a_v = fmaxf(a_v, ov);
                 }
-                int8_pass2<Cfg, kStateStages>(hp, R, a_m, a_v, titer, taddr, sST, bar_st_full, bar_st_done, bar_st_empty,
-                                              row_t, wg, FORGE_DBG(P, DBG_NO_EPILOGUE), FORGE_DBG(P, DBG_NO_STATE));
+#ifdef FORGE_PROFILING
+                t_x += clock64() - t_x0;
+#endif
+                FORGE_TIMED_WAIT(t_p2, (int8_pass2<Cfg, kStateStages>(hp, R, a_m, a_v, titer, taddr, sST, bar_st_full, bar_st_done,
+                                                                      bar_st_empty, row_t, wg, FORGE_DBG(P, DBG_NO_EPILOGUE),
+                                                                      FORGE_DBG(P, DBG_NO_STATE), t_w2)));
                 if (wg == 0 && R.valid) {
                     const ProblemDesc &pd = P.prob[decode_tile<CG>(P, tile, rank).p];
                     pd.m_scale[R.sidx] = __fmul_rn(hp.one_minus_beta1, a_m);     // absmax of m', v' from the scaled maxima
@@ -1001,6 +1081,11 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                 else mbar_arrive(bar_tm_empty + 8 * as);
             }
         }
+#ifdef FORGE_PROFILING
+        if (FORGE_DBG(P, DBG_TIMING) && blockIdx.x < 2 && lane == 0 && (warp == 4 || warp == 9))
+            printf("cta %d warp %d tiles %u total %lld | wait G %lld | p1 %lld (wait codes %lld) | xchg %lld | p2/epi %lld (wait state %lld)\n",
+                   blockIdx.x, warp, titer, clock64() - t_begin, t_tm, t_p1, t_w1, t_x, t_p2, t_w2);
+#endif
     }
 
     __syncwarp();                                // lanes 1-31 of the single-thread roles rejoin lane 0

@@ -24,3 +24,12 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+def pytest_sessionstart(session):
+    """FORGE_TEST_PROFILING_LIB=1 runs the whole suite against libforge_b200_prof.so (the -DFORGE_PROFILING build), so
+    that a candidate instantiation selected with FORGE_CFG=<n> can be put through the parity tests before it is
+    promoted to the product dispatch table.  Unset (the default and what the driver runs): the product library."""
+    if os.environ.get("FORGE_TEST_PROFILING_LIB") == "1":
+        from paper_2606_22932_b200 import binding
+        binding.use_profiling_library(True)
