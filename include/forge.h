@@ -191,8 +191,8 @@ forge_status_t forge_wgrad_adamw_host(const void *X, const void *dY, void *W, vo
  * state (whole tile rows: the result is bit-identical to the device-resident call), so the download of one slice
  * overlaps the upload of the next (PCIe is full duplex) and the kernels.  Device scratch is allocated and
  * freed inside the call; synchronous on return.  All four moment dtypes (INT8: the block scales, FP8: the two
- * float[2] scale / amax pairs travel with the codes).  A tensor shared by several problems
- * (q/k/v read one X) is uploaded once per problem. */
+ * float[2] scale / amax pairs travel with the codes).  An operand shared by several problems of the call (q/k/v read
+ * one X: same host pointer and shape) is uploaded once. */
 forge_status_t forge_wgrad_adamw_grouped_host(const forge_problem_t *problems, int32_t count, int64_t step, float lr,
                                              float beta1, float beta2, float eps, float wd,
                                              forge_moment_dtype_t moment_dtype);

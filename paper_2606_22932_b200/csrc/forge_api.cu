@@ -998,8 +998,17 @@ forge_status_t forge_wgrad_adamw_grouped_host(const forge_problem_t *problems, i
         g.v = q; q += up(sz[i].bM);
         g.m_scale = sz[i].bS ? reinterpret_cast<float *>(q) : nullptr; q += up(sz[i].bS);
         g.v_scale = sz[i].bS ? reinterpret_cast<float *>(q) : nullptr;
-        FORGE_TRY(cudaMemcpyAsync(const_cast<void *>(g.X), p.X, sz[i].bX, cudaMemcpyHostToDevice, s_in));
-        FORGE_TRY(cudaMemcpyAsync(const_cast<void *>(g.dY), p.dY, sz[i].bY, cudaMemcpyHostToDevice, s_in));
+        // an operand shared with an earlier problem of the call (q / k / v read one X) is uploaded once
+        const void *shared_x = nullptr, *shared_dy = nullptr;
+        for (int kk = 0; kk < k; ++kk) {
+            const forge_problem_t &q0 = problems[order[kk]];
+            if (q0.X == p.X && q0.T == p.T && q0.in == p.in) shared_x = dp[order[kk]].X;
+            if (q0.dY == p.dY && q0.T == p.T && q0.out == p.out) shared_dy = dp[order[kk]].dY;
+        }
+        if (shared_x) g.X = shared_x;
+        else FORGE_TRY(cudaMemcpyAsync(const_cast<void *>(g.X), p.X, sz[i].bX, cudaMemcpyHostToDevice, s_in));
+        if (shared_dy) g.dY = shared_dy;
+        else FORGE_TRY(cudaMemcpyAsync(const_cast<void *>(g.dY), p.dY, sz[i].bY, cudaMemcpyHostToDevice, s_in));
         if (f8) {                                   // one {scale, amax} pair per tensor, shared by the slices
             FORGE_TRY(cudaMemcpyAsync(g.m_scale, p.m_scale, sz[i].bS, cudaMemcpyHostToDevice, s_in));
             FORGE_TRY(cudaMemcpyAsync(g.v_scale, p.v_scale, sz[i].bS, cudaMemcpyHostToDevice, s_in));

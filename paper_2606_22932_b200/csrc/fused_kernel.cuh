@@ -524,7 +524,7 @@ __device__ __forceinline__ void int8_pass1(const AdamWScalars &hp, const Int8Row
 template <class Cfg, int kStateStages>
 __device__ __forceinline__ void int8_pass1_ring(const Int8Row &R, uint32_t titer, uint32_t taddr, uint32_t sST,
                                                 uint32_t bar_st_full, uint32_t row_t, int wg, float &pm, float &pv,
-                                                bool skip_math, long long &t_wait) {
+                                                bool skip_math, bool no_state, long long &t_wait) {
     pm = 0.0f;
     pv = 0.0f;
     const uint32_t rb = row_t / Cfg::CM, row = row_t % Cfg::CM;
@@ -532,7 +532,7 @@ __device__ __forceinline__ void int8_pass1_ring(const Int8Row &R, uint32_t titer
     for (int cb = 0; cb < Cfg::CB; ++cb) {
         const uint32_t ci = titer * Cfg::CHUNKS + cb * Cfg::RB + rb;
         const uint32_t s = ci % kStateStages, ph = (ci / kStateStages) & 1u;
-        FORGE_TIMED_WAIT(t_wait, mbar_wait(bar_st_full + 8 * s, ph));
+        if (!no_state) FORGE_TIMED_WAIT(t_wait, mbar_wait(bar_st_full + 8 * s, ph));
 #pragma unroll 1
         for (int half = 0; half < Cfg::SUBS; ++half) {
             if (skip_math || (cb * Cfg::SUBS + half) % Cfg::NWG != wg) continue;
@@ -1045,7 +1045,8 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                                                            FORGE_DBG(P, DBG_NO_STATE), t_w1));
                 else
                     FORGE_TIMED_WAIT(t_p1, (int8_pass1_ring<Cfg, kStateStages>(R, titer, taddr, sST, bar_st_full, row_t, wg, pm, pv,
-                                                                               FORGE_DBG(P, DBG_NO_EPILOGUE), t_w1)));
+                                                                               FORGE_DBG(P, DBG_NO_EPILOGUE), FORGE_DBG(P, DBG_NO_STATE),
+                                                                               t_w1)));
 #ifdef FORGE_PROFILING
                 const long long t_x0 = clock64();
 #endif
