@@ -221,6 +221,20 @@ forge_status_t forge_adamw_from_g(const float *G, void *W, void *m, void *v,
                                   int64_t step, float lr, float beta1, float beta2, float eps, float wd,
                                   forge_moment_dtype_t moment_dtype, forge_stream_t stream);
 
+/* Tuning for the clock the caller expects the launches to run at.  Results are BIT-IDENTICAL in both settings (the
+ * instantiations differ only in chunk geometry and ring depths; same token order in the accumulator, same per-element
+ * arithmetic), so this is a pure performance choice, process-wide and thread-safe:
+ *   FORGE_TUNE_BOOST_CLOCK (default): best for short bursts of launches at the boost clock -- what a K-launch benchmark
+ *     times (fp32 moments, Llama-8B layer at T = 512: 729 us at 1965 MHz, 790-820 us once the board power-caps);
+ *   FORGE_TUNE_SUSTAINED_CLOCK: best under continuous load, when the board sits at its power cap and the SM clock is
+ *     ~1.5-1.6 GHz -- a training loop (the same layer: 745 us capped, 755 us at the boost clock).
+ * Only the fp32- and bf16-moment paths at T <= 1024 (and the two-state fp32 families) have a second instantiation.
+ * An explicit call, not an environment variable and not a heuristic: the library cannot see the clock cheaply and does
+ * not guess. */
+typedef enum { FORGE_TUNE_BOOST_CLOCK = 0, FORGE_TUNE_SUSTAINED_CLOCK = 1 } forge_tuning_t;
+forge_status_t forge_set_tuning(forge_tuning_t tuning);     /* FORGE_ERR_BAD_HYPERPARAM for any other value */
+forge_tuning_t forge_get_tuning(void);
+
 /* Device bytes the library itself holds between calls: a constant with no O(out*in) term (0). */
 size_t forge_workspace_bytes(void);
 /* Kernel launches issued by this library since load (for bench.py's gpu_launches). */

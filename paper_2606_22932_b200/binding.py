@@ -23,7 +23,7 @@ STATUS_NAMES = ["FORGE_OK", "FORGE_ERR_NULL_PTR", "FORGE_ERR_BAD_SHAPE", "FORGE_
                 "FORGE_ERR_CUDA"]
 EXPORTS = ["forge_wgrad_adamw", "forge_wgrad_adamw_grouped", "forge_wgrad_step_grouped", "forge_wgrad_accumulate_grouped", "forge_layer_backward_grouped", "forge_wgrad_adamw_sr_grouped", "forge_wgrad_adamw_host", "forge_wgrad_adamw_grouped_host",
            "forge_wgrad_store_g", "forge_wgrad_store_g_grouped", "forge_adamw_from_g", "forge_workspace_bytes", "forge_launch_count",
-           "forge_last_cuda_error", "forge_last_kernel", "forge_status_string", "forge_version"]
+           "forge_last_cuda_error", "forge_last_kernel", "forge_set_tuning", "forge_get_tuning", "forge_status_string", "forge_version"]
 
 
 class ForgeError(RuntimeError):
@@ -102,6 +102,9 @@ def lib() -> ctypes.CDLL:
         L.forge_launch_count.restype = ctypes.c_uint64
         L.forge_last_cuda_error.restype = ctypes.c_int
         L.forge_last_kernel.restype = ctypes.c_char_p
+        L.forge_set_tuning.restype = ctypes.c_int
+        L.forge_set_tuning.argtypes = [ctypes.c_int]
+        L.forge_get_tuning.restype = ctypes.c_int
         L.forge_status_string.restype = ctypes.c_char_p
         L.forge_status_string.argtypes = [ctypes.c_int]
         L.forge_version.restype = ctypes.c_int
@@ -269,6 +272,18 @@ def forge_adamw_from_g(G, W, m, v, step, lr, beta1, beta2, eps, wd, m_scale=None
     if check:
         _check(st, "forge_adamw_from_g")
     return st
+
+
+TUNE_BOOST_CLOCK, TUNE_SUSTAINED_CLOCK = 0, 1
+
+
+def forge_set_tuning(tuning: int) -> None:
+    """include/forge.h forge_set_tuning: which clock the caller expects (bit-identical results either way)."""
+    _check(lib().forge_set_tuning(int(tuning)), "forge_set_tuning")
+
+
+def forge_get_tuning() -> int:
+    return int(lib().forge_get_tuning())
 
 
 def forge_launch_count() -> int:

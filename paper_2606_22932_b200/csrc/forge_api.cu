@@ -25,7 +25,8 @@ using namespace forge;
 
 std::atomic<uint64_t> g_launches{0};
 std::atomic<int> g_last_cuda_error{0};
-std::atomic<const char *> g_last_kernel{""};     // signature of the instantiation the last launch used (forge_last_kernel)
+std::atomic<const char *> g_last_kernel{""};
+std::atomic<int> g_tuning{FORGE_TUNE_BOOST_CLOCK};   // forge_set_tuning: explicit, process-wide, bit-identical either way     // signature of the instantiation the last launch used (forge_last_kernel)
 
 forge_status_t cuda_fail(cudaError_t e) {
     g_last_cuda_error.store(static_cast<int>(e));
@@ -386,10 +387,17 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
         // T > 1024: 128 KB operand ring; the 80 KB left for the state go further as 4 x 20 KB (32 x 64) than as 2 x 40 KB
         if (variant == V_DIRECT) return launch_fused<MDT_FP32, MODE_ADAMW, 64, 6, 0, 2, 64, 128>(probs, count, hp, dev, stream);
         if (variant == V_LARGE_T) return launch_fused<MDT_FP32, MODE_ADAMW, 64, 4, 4, 2, 32, 64>(probs, count, hp, dev, stream);
+        // 64 x 128 chunks: 729 us / layer at the boost clock, 790-820 under the power cap; 128 x 64 chunks with a 48 KB
+        // operand ring: 755 / 745 (profiles/r02_summary.md).  No geometry tried wins both; the caller says which clock
+        // it expects (forge_set_tuning), the library does not guess.  Bit-identical.
+        if (g_tuning.load(std::memory_order_relaxed) == FORGE_TUNE_SUSTAINED_CLOCK)
+            return launch_fused<MDT_FP32, MODE_ADAMW, 32, 3, 2, 2, 128, 64>(probs, count, hp, dev, stream);
         return launch_fused<MDT_FP32, MODE_ADAMW, 32, 4, 2, 2, 64, 128>(probs, count, hp, dev, stream);
     case FORGE_MOMENT_BF16:
         if (variant == V_DIRECT) return launch_fused<MDT_BF16, MODE_ADAMW, 64, 6, 0, 2, 64, 64>(probs, count, hp, dev, stream);
         if (variant == V_LARGE_T) return launch_fused<MDT_BF16, MODE_ADAMW, 64, 4, 2, 2, 64, 64>(probs, count, hp, dev, stream);
+        if (g_tuning.load(std::memory_order_relaxed) == FORGE_TUNE_SUSTAINED_CLOCK)      // 478 / 483 us against 457 / 498
+            return launch_fused<MDT_BF16, MODE_ADAMW, 64, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
         return launch_fused<MDT_BF16, MODE_ADAMW, 32, 4, 4, 2, 64, 64>(probs, count, hp, dev, stream);
     case FORGE_MOMENT_INT8:
         // resident-tile epilogue (P1S = 0: the four 128 x 64 chunks of a tile stay in the state ring through both passes, no
@@ -503,8 +511,11 @@ forge_status_t dispatch_family(const forge_problem_t *probs, int count, int nst,
         return launch_fused<MDT, MODE_FAMILY, 64, 4, 4, 2, 32, 128, 128, 2, 1>(probs, count, hp, dev, stream, &fs);
     }
     if (big) return launch_fused<MDT, MODE_FAMILY, 64, 4, 2, 2, 64, 64, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
-    if (MDT == MDT_FP32)        // two fp32 states: AdamW's byte count and AdamW's instantiation
+    if (MDT == MDT_FP32) {      // two fp32 states: AdamW's byte count and AdamW's two instantiations
+        if (g_tuning.load(std::memory_order_relaxed) == FORGE_TUNE_SUSTAINED_CLOCK)
+            return launch_fused<MDT, MODE_FAMILY, 32, 3, 2, 2, 128, 64, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
         return launch_fused<MDT, MODE_FAMILY, 32, 4, 2, 2, 64, 128, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
+    }
     return launch_fused<MDT, MODE_FAMILY, 32, 4, 4, 2, 64, 64, 128, 2, 2>(probs, count, hp, dev, stream, &fs);
 }
 
@@ -1064,6 +1075,13 @@ forge_status_t forge_wgrad_adamw_grouped_host(const forge_problem_t *problems, i
     if (rc != FORGE_OK) return rc;
     return e == cudaSuccess ? FORGE_OK : cuda_fail(e);
 }
+
+forge_status_t forge_set_tuning(forge_tuning_t tuning) {
+    if (tuning != FORGE_TUNE_BOOST_CLOCK && tuning != FORGE_TUNE_SUSTAINED_CLOCK) return FORGE_ERR_BAD_HYPERPARAM;
+    g_tuning.store(static_cast<int>(tuning), std::memory_order_relaxed);
+    return FORGE_OK;
+}
+forge_tuning_t forge_get_tuning(void) { return static_cast<forge_tuning_t>(g_tuning.load(std::memory_order_relaxed)); }
 
 size_t forge_workspace_bytes(void) { return 0; }
 uint64_t forge_launch_count(void) { return g_launches.load(); }

@@ -330,6 +330,30 @@ def test_stray_profiling_environment_cannot_change_a_product_result():
     assert not torch.equal(outs[0][0]["W"], ps[0].W.to(DEV))
 
 
+def test_tuning_for_the_sustained_clock_is_bit_identical():
+    """forge_set_tuning (include/forge.h): the instantiations for the boost and for the power-capped clock give the same
+    bits, fp32 and bf16 moments, grouped launch, ragged shapes; an unknown value is rejected and changes nothing."""
+    ps = [synth.make_problem("a", 512, 640, 768, 21), synth.make_problem("b", 200, 136, 264, 22), synth.make_problem("c", 512, 1024, 1536, 23)]
+    for moment in ("fp32", "bf16"):
+        outs, kernels = [], []
+        for tuning in (fb.TUNE_BOOST_CLOCK, fb.TUNE_SUSTAINED_CLOCK):
+            fb.forge_set_tuning(tuning)
+            try:
+                assert fb.forge_get_tuning() == tuning
+                devs = [gpu_state(p, moment)[0] for p in ps]
+                fb.forge_wgrad_adamw_grouped(devs, *hp_args(4), fb.FP32 if moment == "fp32" else fb.BF16)
+                torch.cuda.synchronize()
+                kernels.append(fb.lib().forge_last_kernel())
+            finally:
+                fb.forge_set_tuning(fb.TUNE_BOOST_CLOCK)
+            outs.append(devs)
+        assert kernels[0] != kernels[1]                    # two different instantiations did run
+        for a, b in zip(outs[0], outs[1]):
+            for k in ("W", "m", "v"):
+                assert torch.equal(a[k], b[k]), (moment, k)
+    assert fb.lib().forge_set_tuning(7) == 4 and fb.forge_get_tuning() == fb.TUNE_BOOST_CLOCK
+
+
 def test_chunk_geometries_are_bit_identical():
     """Every instantiation sums the tokens in the same order and applies the same per-element update, so the chunk shape
     and ring depths are invisible in the results (FORGE_CFG, profiling build): grouped launch, ragged shapes."""
