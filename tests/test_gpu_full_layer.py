@@ -74,6 +74,34 @@ def test_config3_gate_one_sixteenth_of_the_rows_spread_over_all_waves(T):
         compare(d, ref, G, E, T, "fp32", rows, label=f"gate T={T} rows {rows}", W_prev=o["W"])
 
 
+def test_layer_backward_full_llama_layer_dgrad_and_update_against_the_oracle():
+    """forge_layer_backward_grouped on the whole cfg-1 layer (the configuration bench.py's `layer_backward` leg times):
+    one dgrad launch over 304 pair-tiles of depth 1024 ... 14336 in the longest-first order, then the fused launch.
+    Every dX element against the oracle's fp64 dY.W from the PRE-update weights; W, m, v bit-identical to the plain
+    grouped call (whose own parity is the test above)."""
+    layer = synth.make_layer(512, seed=synth.BASE_SEED + 1)
+    probs = [dict(X=p.X.to(DEV), dY=p.dY.to(DEV), W=p.W.to(DEV).clone(), m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone()) for p in layer]
+    twins = [dict(X=d["X"], dY=d["dY"], W=p.W.to(DEV).clone(), m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone()) for p, d in zip(layer, probs)]
+    dXs = [torch.full((p.T, p.inn), float("nan"), dtype=torch.bfloat16, device=DEV) for p in layer]
+    n0 = fb.forge_launch_count()
+    fb.forge_layer_backward_grouped(probs, dXs, *hp_args(10), fb.FP32)
+    assert fb.forge_launch_count() - n0 == 2
+    fb.forge_wgrad_adamw_grouped(twins, *hp_args(10), fb.FP32)
+    torch.cuda.synchronize()
+    for p, d, t, dX in zip(layer, probs, twins, dXs):
+        for k in ("W", "m", "v"):
+            assert torch.equal(d[k], t[k]), (p.name, k)
+        dYf, Wf = fo.bf16_to_f64(synth.bf16_bits(p.dY)), fo.bf16_to_f64(synth.bf16_bits(p.W))
+        ref = fo.dgrad(synth.bf16_bits(p.dY), synth.bf16_bits(p.W))
+        got = fo.bf16_to_f64(synth.bf16_bits(dX))
+        bound = p.out * 2.0 ** -23 * (np.abs(dYf) @ np.abs(Wf))
+        bad = np.abs(got - ref) > pu.bf16_ulp(ref) + bound
+        assert not bad.any(), (p.name, int(bad.sum()), float(np.abs(got - ref).max()))
+        exact = float((synth.bf16_bits(dX) == fo.f64_to_bf16(ref)).mean())
+        pu.record("dgrad_layer", name=p.name, dx_bit_identical=exact)
+        assert exact > 0.98, (p.name, exact)
+
+
 # ------------------------------------------------------------------------------ edge cases ---
 def test_nan_and_inf_propagate_to_exactly_the_affected_row_and_column():
     """include/forge.h: "NaN/Inf in the inputs propagate by IEEE rules (to the rows / columns of G they enter and
