@@ -57,6 +57,8 @@ def use_profiling_library(on: bool) -> None:
     """Route every call of this module through libforge_b200_prof.so (the -DFORGE_PROFILING build: FORGE_CFG /
     FORGE_GRID / FORGE_ABLATE are honoured there and nowhere else).  For profiles/ commands and two tests only."""
     global _lib, _profiling
+    if on and not os.path.exists(_build.PROF_LIB_PATH):
+        _build.build(profiling=True)        # tests / profiles on a box that received only the product library
     _profiling = bool(on)
     _lib = None
 
