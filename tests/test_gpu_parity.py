@@ -380,6 +380,39 @@ def test_chunk_geometries_are_bit_identical():
     assert not torch.equal(outs[0][0]["W"], ps[0].W.to(DEV))
 
 
+def test_grouped_call_is_cuda_graph_capturable_and_replays_bitwise():
+    """The ABI enqueues on the caller's stream, allocates nothing and synchronises nothing, so a layer's call (and the
+    layer-backward call: dgrad launch + fused launch) can be captured into a CUDA graph and replayed: the replay applies
+    the same step to whatever the buffers hold, bit-identical to the eager call on the same state."""
+    ps = [synth.make_problem("a", 512, 640, 768, 41), synth.make_problem("b", 200, 136, 264, 42)]
+    eager = [dict(X=p.X.to(DEV), dY=p.dY.to(DEV), W=p.W.to(DEV).clone(), m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone()) for p in ps]
+    graph = [dict(X=d["X"], dY=d["dY"], W=p.W.to(DEV).clone(), m=p.m.to(DEV).clone(), v=p.v.to(DEV).clone()) for p, d in zip(ps, eager)]
+    dX_e = [torch.zeros(p.T, p.inn, dtype=torch.bfloat16, device=DEV) for p in ps]
+    dX_g = [torch.zeros(p.T, p.inn, dtype=torch.bfloat16, device=DEV) for p in ps]
+    fb.forge_layer_backward_grouped(eager, dX_e, *hp_args(6), fb.FP32)           # warm-up: function attributes are set
+    for d, p in zip(eager, ps):
+        d["W"].copy_(p.W.to(DEV)); d["m"].copy_(p.m.to(DEV)); d["v"].copy_(p.v.to(DEV))
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        g.capture_begin()
+        fb.forge_layer_backward_grouped(graph, dX_g, *hp_args(6), fb.FP32, stream=side)
+        g.capture_end()
+    torch.cuda.synchronize()
+    for d, p in zip(graph, ps):
+        assert torch.equal(d["W"], p.W.to(DEV))                                   # capture did not execute anything
+    for _ in range(2):                                                             # two replays = two eager calls
+        g.replay()
+        fb.forge_layer_backward_grouped(eager, dX_e, *hp_args(6), fb.FP32)
+    torch.cuda.synchronize()
+    for a, b, x, y in zip(eager, graph, dX_e, dX_g):
+        for k in ("W", "m", "v"):
+            assert torch.equal(a[k], b[k]), k
+        assert torch.equal(x, y)
+    assert not torch.equal(graph[0]["W"], ps[0].W.to(DEV))
+
+
 # ------------------------------------------------------------------------------ properties ---
 def test_lr_zero_keeps_w_and_inputs_untouched_moments_move():
     p = synth.make_problem("x", 256, 256, 512, seed=13)
