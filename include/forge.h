@@ -68,7 +68,9 @@ typedef enum {
  *         (App. B with BASELINE.json's 256-blocks); m code = rint(m'*127/a) in
  *         [-127,127] (int8), v code = max(1, rint(v'*255/a)) in [1,255] (uint8) when a > 0,
  *         all codes 0 when a == 0; the stored scale is a = max|x| over the block (fp32).
- *         Dequantised value = code*a/127 (m) or code*a/255 (v).  Requantised every step.
+ *         Dequantised value = code*a/127 (m) or code*a/255 (v).  Requantised every step.  The codes (and the FP8
+ *         codes below) cannot hold NaN / Inf: a non-finite gradient element still makes W' non-finite by IEEE rules, the
+ *         code stored for its m', v' and the block scale it contributes to are unspecified.
  * In every mode the update arithmetic and G are fp32 and W' is computed from the unrounded
  * m', v' ("the update arithmetic and the gradient remain fp32 throughout"). */
 typedef enum {
