@@ -216,10 +216,11 @@ def layer_cpu():
     return synth.make_layer(512, seed=synth.BASE_SEED + 1)
 
 
-@pytest.mark.parametrize("family", ["momentum", "lion", "sgd"])
-def test_full_layer_family_grouped_sampled_rows(layer_cpu, family):
+@pytest.mark.parametrize("family,every_row", [("momentum", True), ("lion", False), ("sgd", False)])
+def test_full_layer_family_grouped_sampled_rows(layer_cpu, family, every_row):
     """The 7 projections of a Llama-3.1-8B layer at full size in ONE grouped launch (the configuration
-    `bench.py --optimizer` times); the oracle is exact on a deterministic sample of rows (rows are independent)."""
+    `bench.py --optimizer` times); the oracle is exact on a deterministic sample of rows (rows are independent) --
+    for SGD with momentum on EVERY row of the layer."""
     kw = dict(beta1=0.9, beta2=0.99, eps=1e-8, wd=0.05, momentum=0.9, nesterov=False)
     lr = 1e-4 if family == "lion" else 1e-2
     ns = fb.FAMILY_STATES[family]
@@ -231,7 +232,8 @@ def test_full_layer_family_grouped_sampled_rows(layer_cpu, family):
     assert fb.forge_launch_count() - n0 == 1
     for p, d in zip(layer_cpu, devs):
         dYb, Xb = synth.bf16_bits(p.dY), synth.bf16_bits(p.X)
-        for r0, r1 in pu.sample_rows(p.out):
+        ranges = [(r0, min(p.out, r0 + 512)) for r0 in range(0, p.out, 512)] if every_row else pu.sample_rows(p.out)
+        for r0, r1 in ranges:
             G, E = fo.wgrad(dYb, Xb, rows=(r0, r1), with_abs=True)
             Wo = synth.bf16_bits(p.W[r0:r1]).copy()
             Wprev = fo.bf16_to_f64(Wo)
