@@ -133,9 +133,18 @@ def _check(status: int, where: str):
         raise ForgeError(status, where)
 
 
+def _dense(where: str, **tensors):
+    """The single-problem entries and the state pointers of forge_problem_t carry no pitch: a strided view would be
+    read as if it were dense.  Rejected here with the library's own BAD_SHAPE status."""
+    for name, t in tensors.items():
+        if t is not None and not t.is_contiguous():
+            raise ForgeError(2, f"{where}: {name} must be contiguous (use the grouped entry for strided operand views)")
+
+
 def forge_wgrad_adamw(X, dY, W, m, v, step, lr, beta1, beta2, eps, wd, m_scale=None, v_scale=None,
                       moment_dtype=None, stream=None, check=True) -> int:
     """include/forge.h forge_wgrad_adamw (Algorithm 1). In place on W, m, v."""
+    _dense("forge_wgrad_adamw", X=X, dY=dY, W=W, m=m, v=v, m_scale=m_scale, v_scale=v_scale)
     T, inn = X.shape
     out = dY.shape[1]
     mdt = moment_dtype_of(m) if moment_dtype is None else moment_dtype
@@ -158,6 +167,7 @@ def make_problem_array(problems):
         arr[i].m = None if m is None else m.data_ptr()
         arr[i].v = None if v is None else v.data_ptr()
         ms, vs = g("m_scale"), g("v_scale")
+        _dense("forge_problem_t", W=W, m=m, v=v, m_scale=ms, v_scale=vs)
         arr[i].m_scale = None if ms is None else ms.data_ptr()
         arr[i].v_scale = None if vs is None else vs.data_ptr()
         arr[i].T, arr[i].in_ = X.shape
@@ -228,6 +238,7 @@ def forge_wgrad_accumulate_grouped(problems, mu, state_dtype=FP32, stream=None, 
 def forge_wgrad_adamw_host(X, dY, W, m, v, step, lr, beta1, beta2, eps, wd, m_scale=None, v_scale=None,
                            check=True) -> int:
     """Host-buffer entry (CPU tensors, ideally pinned): H2D, fused step, D2H inside the call."""
+    _dense("forge_wgrad_adamw_host", X=X, dY=dY, W=W, m=m, v=v, m_scale=m_scale, v_scale=v_scale)
     T, inn = X.shape
     out = dY.shape[1]
     st = lib().forge_wgrad_adamw_host(_ptr(X), _ptr(dY), _ptr(W), _ptr(m), _ptr(v), _ptr(m_scale), _ptr(v_scale),
@@ -248,6 +259,7 @@ def forge_wgrad_adamw_grouped_host(problems, step, lr, beta1, beta2, eps, wd, mo
 
 def forge_wgrad_store_g(X, dY, G, stream=None, check=True) -> int:
     """Store-G: G[out,in] fp32 = dY^T X; the DP bucket producer and the fused kernel's test twin."""
+    _dense("forge_wgrad_store_g", X=X, dY=dY, G=G)
     T, inn = X.shape
     out = dY.shape[1]
     st = lib().forge_wgrad_store_g(_ptr(X), _ptr(dY), _ptr(G), T, out, inn, _stream(stream))
@@ -268,6 +280,7 @@ def forge_wgrad_store_g_grouped(problems, stream=None, check=True, _arr=None) ->
 def forge_adamw_from_g(G, W, m, v, step, lr, beta1, beta2, eps, wd, m_scale=None, v_scale=None, stream=None,
                        check=True) -> int:
     """The update from a materialised fp32 G: dp.py's reduced bucket, and the fused kernel's test twin."""
+    _dense("forge_adamw_from_g", G=G, W=W, m=m, v=v, m_scale=m_scale, v_scale=v_scale)
     out, inn = W.shape
     st = lib().forge_adamw_from_g(_ptr(G), _ptr(W), _ptr(m), _ptr(v), _ptr(m_scale), _ptr(v_scale), out, inn,
                                   int(step), lr, beta1, beta2, eps, wd, moment_dtype_of(m), _stream(stream))
