@@ -58,7 +58,8 @@ typedef enum {
     FORGE_ERR_BAD_HYPERPARAM = 4,
     FORGE_ERR_BAD_DTYPE = 5,
     FORGE_ERR_UNSUPPORTED_ARCH = 6,
-    FORGE_ERR_CUDA = 7
+    FORGE_ERR_CUDA = 7,
+    FORGE_ERR_TOO_LARGE = 8        /* forge_wgrad_adamw_host_noalloc only: the problem exceeds the static scratch */
 } forge_status_t;
 
 /* Storage type of the moments m, v ("k" of PAPER.md:19 Eq. 1):
@@ -188,6 +189,28 @@ forge_status_t forge_wgrad_adamw_host(const void *X, const void *dY, void *W, vo
                                       int64_t step, float lr, float beta1, float beta2, float eps, float wd,
                                       forge_moment_dtype_t moment_dtype);
 
+/* forge_wgrad_adamw_host for callers that may not allocate (a harness that forbids cudaMalloc, a tight serving loop):
+ * the same arguments, validation, arithmetic and result (bit-identical to forge_wgrad_adamw_host), but the device
+ * staging of X, dY, W, m, v and the scales lives in ONE file-scope static __device__ array of
+ * FORGE_NOALLOC_SCRATCH_BYTES (32 MiB) instead of a cudaMalloc'ed block.  The call issues no cudaMalloc, cudaFree or
+ * other allocating routine: only copies on the default stream, one fused launch and a stream synchronise.
+ *   limit     the staged bytes -- each of the up-to-seven arrays rounded up to 256 B: T*in*2 + T*out*2 + out*in*(2 +
+ *             2 * moment bytes) + the int8 block scales -- must fit the array, else FORGE_ERR_TOO_LARGE and nothing
+ *             is copied or launched (fp32 moments at T = 512: out*in up to ~3.1 M, e.g. 1024 x 2048 or 1536 x 1536).
+ *   cost      every GPU on which this library's module is loaded holds the 32 MiB until the process exits
+ *             (forge_workspace_bytes() counts dynamic allocations only and stays 0).
+ *   sharing   all calls on a device use the same array, and it keeps the previous call's bytes.  Nothing in it has to
+ *             start at zero -- every region the kernel reads is overwritten by this call's uploads first -- but two
+ *             calls that overlap on the same GPU (two host threads) race on it: serialise them.  The call itself is
+ *             synchronous, so back-to-back calls from one thread are safe.
+ * The array's device address is resolved once per device (cudaGetSymbolAddress with that device current). */
+#define FORGE_NOALLOC_SCRATCH_BYTES (32u << 20)
+forge_status_t forge_wgrad_adamw_host_noalloc(const void *X, const void *dY, void *W, void *m, void *v,
+                                              float *m_scale, float *v_scale,
+                                              int32_t T, int32_t out, int32_t in,
+                                              int64_t step, float lr, float beta1, float beta2, float eps, float wd,
+                                              forge_moment_dtype_t moment_dtype);
+
 /* The same for a whole group with HOST buffers (every pointer of every problem is a host pointer, ideally pinned):
  * a three-stage pipeline -- upload, fused step, download on three streams -- over ~64 MB row slices of each problem's
  * state (whole tile rows: the result is bit-identical to the device-resident call), so the download of one slice
@@ -237,7 +260,9 @@ typedef enum { FORGE_TUNE_BOOST_CLOCK = 0, FORGE_TUNE_SUSTAINED_CLOCK = 1 } forg
 forge_status_t forge_set_tuning(forge_tuning_t tuning);     /* FORGE_ERR_BAD_HYPERPARAM for any other value */
 forge_tuning_t forge_get_tuning(void);
 
-/* Device bytes the library itself holds between calls: a constant with no O(out*in) term (0). */
+/* Device bytes the library itself allocates and holds between calls: a constant with no O(out*in) term (0).  The
+ * fixed static array of forge_wgrad_adamw_host_noalloc (FORGE_NOALLOC_SCRATCH_BYTES, part of the loaded module) is
+ * not an allocation and is not counted. */
 size_t forge_workspace_bytes(void);
 /* Kernel launches issued by this library since load (for bench.py's gpu_launches). */
 uint64_t forge_launch_count(void);

@@ -20,8 +20,9 @@ FP32, BF16, INT8, FP8 = 0, 1, 2, 3
 QBLOCK = 256
 STATUS_NAMES = ["FORGE_OK", "FORGE_ERR_NULL_PTR", "FORGE_ERR_BAD_SHAPE", "FORGE_ERR_ALIGNMENT",
                 "FORGE_ERR_BAD_HYPERPARAM", "FORGE_ERR_BAD_DTYPE", "FORGE_ERR_UNSUPPORTED_ARCH",
-                "FORGE_ERR_CUDA"]
-EXPORTS = ["forge_wgrad_adamw", "forge_wgrad_adamw_grouped", "forge_wgrad_step_grouped", "forge_wgrad_accumulate_grouped", "forge_layer_backward_grouped", "forge_wgrad_adamw_sr_grouped", "forge_wgrad_adamw_host", "forge_wgrad_adamw_grouped_host",
+                "FORGE_ERR_CUDA", "FORGE_ERR_TOO_LARGE"]
+NOALLOC_SCRATCH_BYTES = 32 << 20   # include/forge.h FORGE_NOALLOC_SCRATCH_BYTES
+EXPORTS = ["forge_wgrad_adamw", "forge_wgrad_adamw_grouped", "forge_wgrad_step_grouped", "forge_wgrad_accumulate_grouped", "forge_layer_backward_grouped", "forge_wgrad_adamw_sr_grouped", "forge_wgrad_adamw_host", "forge_wgrad_adamw_host_noalloc", "forge_wgrad_adamw_grouped_host",
            "forge_wgrad_store_g", "forge_wgrad_store_g_grouped", "forge_adamw_from_g", "forge_workspace_bytes", "forge_launch_count",
            "forge_last_cuda_error", "forge_last_kernel", "forge_set_tuning", "forge_get_tuning", "forge_status_string", "forge_version"]
 
@@ -94,6 +95,8 @@ def lib() -> ctypes.CDLL:
                                                   [ctypes.c_int, c_void_p]
         L.forge_wgrad_adamw_host.restype = ctypes.c_int
         L.forge_wgrad_adamw_host.argtypes = [c_void_p] * 7 + [c_int32] * 3 + hp + [ctypes.c_int]
+        L.forge_wgrad_adamw_host_noalloc.restype = ctypes.c_int
+        L.forge_wgrad_adamw_host_noalloc.argtypes = [c_void_p] * 7 + [c_int32] * 3 + hp + [ctypes.c_int]
         L.forge_wgrad_store_g.restype = ctypes.c_int
         L.forge_wgrad_store_g.argtypes = [c_void_p] * 3 + [c_int32] * 3 + [c_void_p]
         L.forge_wgrad_store_g_grouped.restype = ctypes.c_int
@@ -245,6 +248,20 @@ def forge_wgrad_adamw_host(X, dY, W, m, v, step, lr, beta1, beta2, eps, wd, m_sc
                                       T, out, inn, int(step), lr, beta1, beta2, eps, wd, moment_dtype_of(m))
     if check:
         _check(st, "forge_wgrad_adamw_host")
+    return st
+
+
+def forge_wgrad_adamw_host_noalloc(X, dY, W, m, v, step, lr, beta1, beta2, eps, wd, m_scale=None, v_scale=None,
+                                   check=True) -> int:
+    """include/forge.h forge_wgrad_adamw_host_noalloc: the host-buffer entry that stages through the library's static
+    32 MiB device array (no cudaMalloc / cudaFree); FORGE_ERR_TOO_LARGE beyond that."""
+    _dense("forge_wgrad_adamw_host_noalloc", X=X, dY=dY, W=W, m=m, v=v, m_scale=m_scale, v_scale=v_scale)
+    T, inn = X.shape
+    out = dY.shape[1]
+    st = lib().forge_wgrad_adamw_host_noalloc(_ptr(X), _ptr(dY), _ptr(W), _ptr(m), _ptr(v), _ptr(m_scale), _ptr(v_scale),
+                                              T, out, inn, int(step), lr, beta1, beta2, eps, wd, moment_dtype_of(m))
+    if check:
+        _check(st, "forge_wgrad_adamw_host_noalloc")
     return st
 
 

@@ -604,6 +604,38 @@ forge_status_t launch_dgrad(const forge_problem_t *probs, void *const *dX, int c
 
 }  // namespace
 
+// ---------------------------------------------------------------------------------------------
+// static device staging of forge_wgrad_adamw_host_noalloc (include/forge.h).  In host code the name below is only a
+// host-side handle of the symbol, NOT a device address: the address is resolved per device with cudaGetSymbolAddress
+// (that device current) the first time the entry point runs there, and only that pointer is handed to copies / kernels.
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) uint8_t forge_noalloc_scratch[FORGE_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kNoallocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+uint8_t *g_noalloc_ptr[kNoallocMaxDevices] = {};
+
+forge_status_t noalloc_scratch(uint8_t **out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    if (dev < 0 || dev >= kNoallocMaxDevices) return FORGE_ERR_UNSUPPORTED_ARCH;
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_ptr[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, forge_noalloc_scratch);
+        if (e != cudaSuccess) return cuda_fail(e);
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255u)) return FORGE_ERR_ALIGNMENT;
+        g_noalloc_ptr[dev] = static_cast<uint8_t *>(p);
+    }
+    *out = g_noalloc_ptr[dev];
+    return FORGE_OK;
+}
+
+}  // namespace
+
 // =============================================================================================
 // C ABI
 // =============================================================================================
@@ -925,6 +957,59 @@ forge_status_t forge_wgrad_adamw_host(const void *X, const void *dY, void *W, vo
     return FORGE_OK;
 }
 
+forge_status_t forge_wgrad_adamw_host_noalloc(const void *X, const void *dY, void *W, void *m, void *v, float *m_scale,
+                                              float *v_scale, int32_t T, int32_t out, int32_t in, int64_t step,
+                                              float lr, float beta1, float beta2, float eps, float wd,
+                                              forge_moment_dtype_t moment_dtype) {
+    const int mdt = static_cast<int>(moment_dtype);
+    if (mdt < 0 || mdt > 2) return FORGE_ERR_BAD_DTYPE;
+    forge_problem_t hp_;
+    std::memset(&hp_, 0, sizeof(hp_));
+    hp_.X = X; hp_.dY = dY; hp_.W = W; hp_.m = m; hp_.v = v; hp_.m_scale = m_scale; hp_.v_scale = v_scale;
+    hp_.T = T; hp_.out = out; hp_.in = in;
+    forge_status_t s = validate_hp(step, lr, beta1, beta2, eps, wd);
+    if (s != FORGE_OK) return s;
+    s = validate_problem(hp_, mdt);
+    if (s != FORGE_OK) return s;
+    const size_t n = static_cast<size_t>(out) * in;
+    const size_t mom = mdt == FORGE_MOMENT_FP32 ? 4 : (mdt == FORGE_MOMENT_BF16 ? 2 : 1);
+    const size_t bX = static_cast<size_t>(T) * in * 2, bY = static_cast<size_t>(T) * out * 2, bW = n * 2,
+                 bM = n * mom, bS = mdt == FORGE_MOMENT_INT8 ? n / FORGE_QBLOCK * 4 : 0;
+    auto up = [](size_t b) { return (b + 255) / 256 * 256; };
+    const size_t total = up(bX) + up(bY) + up(bW) + 2 * up(bM) + 2 * up(bS);
+    if (total > static_cast<size_t>(FORGE_NOALLOC_SCRATCH_BYTES)) return FORGE_ERR_TOO_LARGE;   // before any CUDA call
+    uint8_t *d = nullptr;
+    s = noalloc_scratch(&d);
+    if (s != FORGE_OK) return s;
+    uint8_t *dX = d, *dYp = dX + up(bX), *dW = dYp + up(bY), *dM = dW + up(bW), *dV = dM + up(bM),
+            *dMs = dV + up(bM), *dVs = dMs + up(bS);
+    cudaStream_t st = nullptr;
+    cudaError_t e;
+    // every region the kernel reads is written here first: the previous call's bytes in the array never matter
+    if ((e = cudaMemcpyAsync(dX, X, bX, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaMemcpyAsync(dYp, dY, bY, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaMemcpyAsync(dW, W, bW, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaMemcpyAsync(dM, m, bM, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaMemcpyAsync(dV, v, bM, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    if (bS) {
+        if ((e = cudaMemcpyAsync(dMs, m_scale, bS, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
+        if ((e = cudaMemcpyAsync(dVs, v_scale, bS, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    }
+    s = forge_wgrad_adamw(dX, dYp, dW, dM, dV, bS ? reinterpret_cast<float *>(dMs) : nullptr,
+                          bS ? reinterpret_cast<float *>(dVs) : nullptr, T, out, in, step, lr, beta1, beta2, eps, wd,
+                          moment_dtype, nullptr);
+    if (s != FORGE_OK) return s;
+    if ((e = cudaMemcpyAsync(W, dW, bW, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaMemcpyAsync(m, dM, bM, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaMemcpyAsync(v, dV, bM, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+    if (bS) {
+        if ((e = cudaMemcpyAsync(m_scale, dMs, bS, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+        if ((e = cudaMemcpyAsync(v_scale, dVs, bS, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+    }
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
+    return FORGE_OK;
+}
+
 forge_status_t forge_wgrad_adamw_grouped_host(const forge_problem_t *problems, int32_t count, int64_t step, float lr,
                                              float beta1, float beta2, float eps, float wd,
                                              forge_moment_dtype_t moment_dtype) {
@@ -1099,6 +1184,7 @@ const char *forge_status_string(forge_status_t status) {
     case FORGE_ERR_BAD_DTYPE: return "FORGE_ERR_BAD_DTYPE";
     case FORGE_ERR_UNSUPPORTED_ARCH: return "FORGE_ERR_UNSUPPORTED_ARCH";
     case FORGE_ERR_CUDA: return "FORGE_ERR_CUDA";
+    case FORGE_ERR_TOO_LARGE: return "FORGE_ERR_TOO_LARGE";
     }
     return "FORGE_ERR_UNKNOWN";
 }
