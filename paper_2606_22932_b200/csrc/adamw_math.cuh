@@ -18,15 +18,18 @@ namespace forge {
 struct AdamWScalars {
     float beta1, one_minus_beta1;   // 1-beta exact in fp32 (Sterbenz)
     float beta2, one_minus_beta2;
-    float step_size;                // lr / (1 - beta1^t)
-    float inv_sqrt_bc2;             // 1 / sqrt(1 - beta2^t)
-    float eps;
+    // W' = (1 - lr wd) W - step m' / (sqrt(v') c + eps), step = lr/(1-beta1^t), c = 1/sqrt(1-beta2^t), is evaluated as
+    // decay W + m' * rcp(nd_c sqrt(v') + nd_eps) with the step size folded into the (negated) denominator: one multiply
+    // less per element and one rounding less.  lr = 0 (or a step size too small for fp32): nd_c = 0, nd_eps = -inf,
+    // the reciprocal is -0 and W' = decay W.
+    float nd_c;                     // -(1/sqrt(1-beta2^t)) / step
+    float nd_eps;                   // -eps / step
     float decay;                    // 1 - lr*wd   (decoupled decay on the pre-update W)
     // int8 moments work on the SCALED moments m'' = m'/(1-beta1), v'' = v'/(1-beta2) (adamw_moments2_qs): one FMA
     // each instead of a multiply and an FMA; the codes are scale-invariant and the factors fold into constants
     float q_b1, q_b2;               // beta/(1-beta)
-    float q_c;                      // sqrt(1-beta2) / (sqrt(1-beta2^t) (1-beta1)):  m'/(sqrt(v'/bc2)+eps) = m''/(sqrt(v'') q_c + q_eps)
-    float q_eps;                    // eps/(1-beta1)
+    float nq_c;                     // -sqrt(1-beta2) / (sqrt(1-beta2^t) (1-beta1) step):  m'/(sqrt(v'/bc2)+eps) = m''/(sqrt(v'') q_c + q_eps)
+    float nq_eps;                   // -eps / ((1-beta1) step)
 };
 
 // ------------------------------------------------------------------ packed fp32 pairs ------
@@ -104,17 +107,16 @@ __device__ __forceinline__ void adamw_moments2_qs(f32x2 g, f32x2 code_m, f32x2 c
 }
 __device__ __forceinline__ void adamw_weight2_s(const AdamWScalars &h, f32x2 m, f32x2 v, f32x2 &w) {
     const f32x2 sq = pk2(sqrt_fast(lo2(v)), sqrt_fast(hi2(v)));
-    const f32x2 denom = fma2(sq, bc2(h.q_c), bc2(h.q_eps));
-    const f32x2 ratio = mul2(m, pk2(rcp_fast(lo2(denom)), rcp_fast(hi2(denom))));
-    w = fma2(bc2(-h.step_size), ratio, mul2(bc2(h.decay), w));
+    const f32x2 nden = fma2(sq, bc2(h.nq_c), bc2(h.nq_eps));
+    w = fma2(m, pk2(rcp_fast(lo2(nden)), rcp_fast(hi2(nden))), mul2(bc2(h.decay), w));
 }
 // W' = (1 - lr wd) W - lr * (m'/bc1) / (sqrt(v'/bc2) + eps)          (Alg. 1 lines 9-10)
-// sqrt(v'/bc2) is evaluated as sqrt(v') * (1/sqrt(bc2)); W' uses the unrounded m', v'.
+// sqrt(v'/bc2) is evaluated as sqrt(v') * (1/sqrt(bc2)); the step size lr/bc1 is folded into the denominator (see
+// AdamWScalars); W' uses the unrounded m', v'.
 __device__ __forceinline__ void adamw_weight2(const AdamWScalars &h, f32x2 m, f32x2 v, f32x2 &w) {
     const f32x2 sq = pk2(sqrt_fast(lo2(v)), sqrt_fast(hi2(v)));
-    const f32x2 denom = fma2(sq, bc2(h.inv_sqrt_bc2), bc2(h.eps));
-    const f32x2 ratio = mul2(m, pk2(rcp_fast(lo2(denom)), rcp_fast(hi2(denom))));
-    w = fma2(bc2(-h.step_size), ratio, mul2(bc2(h.decay), w));
+    const f32x2 nden = fma2(sq, bc2(h.nd_c), bc2(h.nd_eps));
+    w = fma2(m, pk2(rcp_fast(lo2(nden)), rcp_fast(hi2(nden))), mul2(bc2(h.decay), w));
 }
 __device__ __forceinline__ void adamw_update2(const AdamWScalars &h, f32x2 g, f32x2 &w, f32x2 &m, f32x2 &v) {
     adamw_moments2(h, g, m, v);

@@ -181,15 +181,21 @@ AdamWScalars make_scalars(int64_t step, float lr, float b1, float b2, float eps,
     h.one_minus_beta1 = 1.0f - b1;
     h.beta2 = b2;
     h.one_minus_beta2 = 1.0f - b2;
-    h.step_size = static_cast<float>(static_cast<double>(lr) / bc1);
-    h.inv_sqrt_bc2 = static_cast<float>(1.0 / std::sqrt(bc2));
-    h.eps = eps;
     h.decay = static_cast<float>(1.0 - static_cast<double>(lr) * static_cast<double>(wd));
     const double d1 = 1.0 - static_cast<double>(b1), d2 = 1.0 - static_cast<double>(b2);
     h.q_b1 = static_cast<float>(static_cast<double>(b1) / d1);
     h.q_b2 = static_cast<float>(static_cast<double>(b2) / d2);
-    h.q_c = static_cast<float>(std::sqrt(d2) / (std::sqrt(bc2) * d1));
-    h.q_eps = static_cast<float>(static_cast<double>(eps) / d1);
+    // the step size lr / bc1 folded into the negated denominator (adamw_math.cuh); no step (lr = 0, or a quotient that
+    // leaves the fp32 range): 0 * sqrt(v') - inf, whose reciprocal is -0
+    const double step_size = static_cast<double>(lr) / bc1;
+    const double c = 1.0 / std::sqrt(bc2);
+    auto fold = [&](double coeff, double e, float &nc, float &ne) {
+        nc = step_size > 0.0 ? static_cast<float>(-coeff / step_size) : 0.0f;
+        ne = step_size > 0.0 ? static_cast<float>(-e / step_size) : -INFINITY;
+        if (!std::isfinite(nc) || !std::isfinite(ne)) { nc = 0.0f; ne = -INFINITY; }
+    };
+    fold(c, static_cast<double>(eps), h.nd_c, h.nd_eps);
+    fold(std::sqrt(d2) * c / d1, static_cast<double>(eps) / d1, h.nq_c, h.nq_eps);
     return h;
 }
 
@@ -304,11 +310,19 @@ forge_status_t launch_fused(const forge_problem_t *probs, int count, const AdamW
         tiles += ((p.out + BLOCK_M * CG - 1) / (BLOCK_M * CG)) * d.tiles_n;   // (128*CG) x 256 work units
     }
     P.total_tiles = tiles;
-    // L2 eviction priority of the operand streams: evict_last for both.  Measured on gate_proj (profiles/r02_summary.md):
-    // dY evict_first is slower at every T (T = 8192: 764 vs 750 us, DRAM reads 2.48 vs 1.80 GB -- the sixteen pairs of a
-    // tile row do not read a dY line at the same instant), dY evict_normal is within noise (749 us, 1.90 GB).
-    P.pol_dy = env_int("FORGE_POLICY", 0) == 1 ? kEvictFirst : (env_int("FORGE_POLICY", 0) == 2 ? kEvictNormal : kEvictLast);
-    P.pol_x = kEvictLast;
+    // L2 eviction priority of the operand streams: evict_last for X; for dY evict_last, except evict_normal at
+    // 2048 <= T < 8192.  Measured on gate_proj (profiles/r02_summary.md): dY evict_first is slower at every T (T = 8192:
+    // 764 vs 750 us, DRAM reads 2.48 vs 1.80 GB -- the sixteen pairs of a tile row do not read a dY line at the same
+    // instant); dY evict_normal is 2.2 % faster at T = 2048 (275.3 vs 281.4 us, three alternating runs each), 0.8 % at
+    // T = 4096, equal at T = 512 and T = 8192.
+    {
+        const int pol = env_int("FORGE_POLICY", -1);   // FORGE_PROFILING build only: 0 both evict_last, 1 dY first, 2 dY normal, 3 X normal, 4 both normal
+        int max_T = 0;
+        for (int i = 0; i < count; ++i) max_T = std::max(max_T, static_cast<int>(probs[i].T));
+        const bool dy_normal = pol < 0 ? (max_T >= 2048 && max_T < 8192) : (pol == 2 || pol == 4);
+        P.pol_dy = pol == 1 ? kEvictFirst : (dy_normal ? kEvictNormal : kEvictLast);
+        P.pol_x = (pol == 3 || pol == 4) ? kEvictNormal : kEvictLast;
+    }
     P.sr_seed_lo = static_cast<uint32_t>(sr_seed);
     P.debug = env_int("FORGE_ABLATE", 0);          // FORGE_PROFILING build only (constant 0 otherwise)
     int grid = dev.sm_count / CG;                  // persistent: one CTA (or CTA pair) per SM (pair)
