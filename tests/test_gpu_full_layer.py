@@ -233,3 +233,46 @@ def test_all_zero_int8_block_inside_a_full_tile():
     assert torch.isfinite(d["W"].float()).all()
     # the same rows' OTHER blocks carry state (zero gradient there too: pure decay of the codes)
     assert d["m_scale"][130:134, 0].all() and d["v_scale"][130:134, 2].all()
+
+
+@pytest.mark.parametrize("hp_over, label", [
+    (dict(lr=0.0), "lr = 0"),                       # no step: W' = (1 - 0) W bit for bit, moments still move
+    (dict(lr=1e-30, wd=0.0), "lr = 1e-30"),         # a huge but finite folded denominator
+    (dict(lr=1e-44, wd=0.0), "lr = 1e-44"),         # subnormal lr: c / step leaves the fp32 range, the no-step constants take over
+    (dict(lr=1.0, wd=0.0), "lr = 1"),               # the largest step size the folded denominator sees
+    (dict(eps=0.0), "eps = 0"),                     # the denominator is sqrt(v_hat) alone (v' > 0 everywhere here)
+    (dict(eps=1e-3, beta1=0.0), "eps = 1e-3, beta1 = 0"),
+])
+def test_step_size_folded_into_the_denominator_edge_hyperparameters(hp_over, label):
+    """The kernels evaluate W' = decay W + m' * rcp(-(sqrt(v') c + eps) / step) (adamw_math.cuh): the hyper-parameter
+    corners of that folding -- no step at all, a step too small for fp32, a large one, eps = 0 -- against the oracle's
+    plain Alg. 1 lines 9-10, fp32 and int8 moments, steps 1 and 50."""
+    hp = dict(HP, **hp_over)
+    p = synth.make_problem("h", 200, 384, 768, seed=910)
+    for moment in ("fp32", "int8"):
+        for step in (1, 50):
+            d, o = gpu_state(p, moment)
+            W0 = d["W"].clone()
+            fb.forge_wgrad_adamw(d["X"], d["dY"], d["W"], d["m"], d["v"], step, m_scale=d.get("m_scale"),
+                                 v_scale=d.get("v_scale"), **hp)
+            torch.cuda.synchronize()
+            G, E = fo.wgrad(o["dY"], o["X"], with_abs=True)
+            W, m, v = o["W"].copy(), o["m"].copy(), o["v"].copy()
+            tol = pu.Tol(G.shape)
+            e = tol.step(G, E, 200, hp)
+            args = (step,) + pu.hp_tuple(hp)
+            if moment == "fp32":
+                wprop = pu.w_propagated("fp32", W, m, v, G, e, step, hp)
+                fo.adamw_fp32(W, m, v, G, *args)
+                pu.check_fp(pu.to_np(d["W"]), pu.to_np(d["m"]), pu.to_np(d["v"]), W, m, v, G, e, tol, hp, "fp32",
+                            f"{label} fp32 step {step}", W_prev=o["W"], w_prop=wprop)
+            else:
+                ms, vs = o["m_scale"].copy(), o["v_scale"].copy()
+                wprop = pu.w_propagated("int8", W, m, v, G, e, step, hp, (ms, vs))
+                fo.adamw_int8(W, m, v, ms, vs, G, *args)
+                pu.check_int8(pu.to_np(d["W"]), pu.to_np(d["m"]), pu.to_np(d["v"]), pu.to_np(d["m_scale"]),
+                              pu.to_np(d["v_scale"]), W, m, v, ms, vs, G, e, hp, f"{label} int8 step {step}",
+                              W_prev=o["W"], w_prop=wprop)
+            assert torch.isfinite(d["W"].float()).all()
+            if hp["lr"] < 1e-20:
+                assert torch.equal(d["W"], W0), f"{label} {moment}: W must not move"
