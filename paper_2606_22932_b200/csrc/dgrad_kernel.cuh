@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(kDgThreads, 1)
 forge_dgrad_kernel(const __grid_constant__ DgradParams P) {
     using Cfg = DgradCfg<kStages>;
     const uint32_t rank = cluster_ctarank();
-    extern __shared__ uint8_t smem_raw[];
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t sML = smem_base;
     const uint32_t sOUT = sML + kStages * Cfg::STAGE;

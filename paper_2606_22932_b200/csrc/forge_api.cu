@@ -417,9 +417,11 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
         // resident-tile epilogue (P1S = 0: the four 128 x 64 chunks of a tile stay in the state ring through both passes, no
         // second read of the codes): 4 slots + 80 KB operand ring 428 us / layer against 440 for the streamed two-ring
         // variant <32, 5, 3, .., 64, 2> on the same box; 5 slots + 48 KB operand ring 451 (mainloop starved); sixteen
-        // epilogue warps 487 (profiles/r02_summary.md)
+        // epilogue warps 487 (profiles/r02_summary.md).  The epilogue warps wait for G 5-14 % of the time (the T = 512
+        // mainloop is bound by operand bytes in flight), so the ring takes every byte the SM has left: six 16 KB stages
+        // next to the 128 KB tile (413 us against 422 with five; 3 x 32 KB: 417)
         if (variant == V_LARGE_T) return launch_fused<MDT_INT8, MODE_ADAMW, 64, 2, 2, 2, 128, 64>(probs, count, hp, dev, stream);
-        return launch_fused<MDT_INT8, MODE_ADAMW, 32, 5, 4, 2, 128, 64, 64, 0>(probs, count, hp, dev, stream);
+        return launch_fused<MDT_INT8, MODE_ADAMW, 32, 6, 4, 2, 128, 64, 64, 0>(probs, count, hp, dev, stream);
     case FORGE_MOMENT_FP8:
         // 8 B/element of state: the T = 512 mainloop needs the deeper operand ring (96 KB) more than the state ring does
         return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 4, 2, 64, 128>(probs, count, hp, dev, stream);

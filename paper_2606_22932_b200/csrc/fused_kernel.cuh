@@ -145,8 +145,13 @@ struct KernelCfg {
     static constexpr int P1_BOX = 128 * P1_COLS;
     static constexpr int P1_STAGE = 2 * P1_BOX;
     static constexpr int kNumBars = 2 * kStages + 4 + 3 * kStateStages + 2 * P1_STAGES;
-    static constexpr int XCHG_BYTES = (MDT == MDT_INT8) ? 2 * NWG * 1024 : 0;   // partial row maxima of the warps sharing a row, 2 buffers
-    static constexpr int SMEM_BYTES = 1024 /*align slack*/ + kStages * ML_STAGE + kStateStages * ST_STAGE +
+    // partial row maxima of the warps sharing a row.  Two buffers (alternating by tile) with the code ring; ONE with the
+    // resident tile: a warp can only write the next tile's maxima after the next tile's first chunk has been loaded, which
+    // needs every warp's arrival on that slot in pass 2 of this tile, i.e. after every warp has read this tile's maxima.
+    static constexpr int XCHG_BUFS = (MDT == MDT_INT8 && P1S_ == 0) ? 1 : 2;
+    static constexpr int XCHG_BYTES = (MDT == MDT_INT8) ? XCHG_BUFS * NWG * 1024 : 0;
+    // the dynamic shared memory is declared __align__(1024) (checked at kernel entry): no alignment slack is reserved
+    static constexpr int SMEM_BYTES = kStages * ML_STAGE + kStateStages * ST_STAGE +
                                       P1_STAGES * P1_STAGE + kNumBars * 8 + 16 + XCHG_BYTES;
     static_assert(SMEM_BYTES <= 232448, "shared memory budget exceeded");
     static_assert(kBlockK % 16 == 0 && kBlockK >= 16, "kBlockK must be a multiple of UMMA_K");
@@ -703,8 +708,9 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
     constexpr uint32_t SSN = DIRECT ? 1 : kStateStages;
     static_assert(!DIRECT || (MODE == MODE_ADAMW && (MDT == MDT_FP32 || MDT == MDT_BF16)), "the direct state path is AdamW, fp32 / bf16 moments");
     const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;   // rank 0 = the pair's leader
-    extern __shared__ uint8_t smem_raw[];
-    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    const uint32_t smem_base = smem_u32(smem_raw);
+    if (smem_base & 1023u) __trap();   // the swizzled TMA / UMMA layouts need 1024-byte aligned stages
     const uint32_t sML = smem_base;                                   // mainloop ring
     const uint32_t sST = sML + kStages * Cfg::ML_STAGE;               // state ring
     const uint32_t sP1 = sST + kStateStages * Cfg::ST_STAGE;          // INT8: first-pass code ring
@@ -1051,7 +1057,7 @@ forge_fused_kernel(const __grid_constant__ KernelParams P) {
                 const long long t_x0 = clock64();
 #endif
                 // combine the two warpgroups' halves of the row (same TMEM quadrant: warps quad and 4 + quad)
-                const uint32_t xb = i8.xchg + (titer & 1u) * (NWG * 1024u);
+                const uint32_t xb = i8.xchg + (Cfg::XCHG_BUFS == 2 ? (titer & 1u) * (NWG * 1024u) : 0u);
                 asm volatile("st.shared.v2.f32 [%0], {%1, %2};\n" ::"r"(xb + (wg * 128u + row_t) * 8u), "f"(pm), "f"(pv) : "memory");
                 asm volatile("bar.sync %0, %1;\n" ::"r"(1u + quad), "n"(NWG * 32) : "memory");
                 float a_m = pm, a_v = pv;
