@@ -423,8 +423,10 @@ forge_status_t dispatch_fused(const forge_problem_t *probs, int count, int mdt, 
         if (variant == V_LARGE_T) return launch_fused<MDT_INT8, MODE_ADAMW, 64, 2, 2, 2, 128, 64>(probs, count, hp, dev, stream);
         return launch_fused<MDT_INT8, MODE_ADAMW, 32, 6, 4, 2, 128, 64, 64, 0>(probs, count, hp, dev, stream);
     case FORGE_MOMENT_FP8:
-        // 8 B/element of state: the T = 512 mainloop needs the deeper operand ring (96 KB) more than the state ring does
-        return launch_fused<MDT_FP8, MODE_ADAMW, 64, 3, 4, 2, 64, 128>(probs, count, hp, dev, stream);
+        // 8 B/element of state: the T = 512 mainloop needs operand bytes in flight more than the state ring needs slots
+        // (the epilogue warps wait for G 10-12 % of the time): 4 x 32 KB of operands + 3 slots of 128 x 64 345 us against
+        // 353 for 3 x 32 KB + 4 slots of 64 x 128; 5 x 32 KB + 2 slots 385; 16 KB stages 361-385 (profiles/r02_summary.md)
+        return launch_fused<MDT_FP8, MODE_ADAMW, 64, 4, 3, 2, 128, 64>(probs, count, hp, dev, stream);
     default:
         return FORGE_ERR_BAD_DTYPE;
     }
